@@ -1,0 +1,120 @@
+/* vla_ternary.h -- C ABI of libvlaternary.so (sm_100a only).
+ *
+ * The ternary-weight linear layer of arxiv/paper_2606_08094 ("vla.cpp"), Section III-D, Eq. 4
+ * (PAPER.md lines 71-82):
+ *
+ *     alpha_m = max(||x_m||_inf, 1e-5) / 127
+ *     a_mj    = clip( round( x_mj / alpha_m ) )            int8, round-half-to-even
+ *     y_mn    = alpha_m * beta_g(n) * sum_j a_mj q_nj      q in {-1,0,+1}, int32 accumulation
+ *
+ * with the weights "packed four two-bit codes per byte" and the result written
+ * as fp32 or as bf16 with round-to-nearest-even.
+ *
+ * Conventions (all entry points):
+ *  - Every pointer is a DEVICE pointer owned by the caller unless the argument says "host".
+ *    The library allocates nothing persistent and creates no streams.
+ *  - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default stream)
+ *    and capturable in a CUDA graph, except vla_ternary_pack, which synchronises the stream.
+ *  - Layouts: W logical [N,K] (row n = output channel, K contiguous); X [M,K] row-major;
+ *    Y [M,N] row-major.
+ *  - Shapes: M >= 1; K % 128 == 0; N % 128 == 0; K <= 65536 (else VLA_ERR_SHAPE).
+ *  - Every pointer must be 16-byte aligned (VLA_ERR_ALIGN).
+ *  - Inputs must be finite; NaN/Inf are not checked (result unspecified, memory-safe).
+ *  - Arguments are validated on the host before any launch.  A non-zero status leaves the
+ *    outputs unspecified but in bounds.  No exceptions cross the ABI.  There is no CPU fallback:
+ *    on a device that is not compute capability 10.x the compute calls return VLA_ERR_ARCH.
+ */
+#ifndef VLA_TERNARY_H
+#define VLA_TERNARY_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    VLA_OK = 0,
+    VLA_ERR_NULL = 1,       /* a required pointer is NULL */
+    VLA_ERR_SHAPE = 2,      /* M/N/K outside the supported set, or not supported by the forced path */
+    VLA_ERR_ALIGN = 3,      /* a pointer is not 16-byte aligned */
+    VLA_ERR_VALUE = 4,      /* vla_ternary_pack: an element outside {-1,0,+1} */
+    VLA_ERR_DTYPE = 5,      /* unknown vla_dtype / vla_path value */
+    VLA_ERR_WORKSPACE = 6,  /* workspace NULL or smaller than vla_ternary_workspace_bytes */
+    VLA_ERR_ARCH = 7,       /* current device is not sm_100 */
+    VLA_ERR_CUDA = 8        /* a CUDA runtime/driver call failed (launch error, etc.) */
+} vla_status;
+
+typedef enum {
+    VLA_F32 = 0,            /* y fp32 */
+    VLA_BF16 = 1,           /* y bf16, round-to-nearest-even of the fp32 value */
+    VLA_I32 = 2             /* raw int32 accumulators sum_j a_mj q_nj, no scaling (parity/debug) */
+} vla_dtype;
+
+typedef enum {
+    VLA_PATH_AUTO = 0,      /* library chooses by M (table in DESIGN.md, justified by ncu) */
+    VLA_PATH_SMALL_ALU = 1, /* in-register decode + dp4a on the integer ALUs; M <= 16 */
+    VLA_PATH_SMALL_TC = 2,  /* in-register decode + warp-level int8 MMA; M <= 64 */
+    VLA_PATH_LARGE = 3      /* TMA -> decode warps -> tcgen05.mma kind::i8 -> TMEM; any M */
+} vla_path;
+
+/* Bytes of the packed form of an [N,K] ternary tensor: exactly N*K/4 (four 2-bit codes per byte,
+ * PAPER.md line 73; no padding at supported shapes).  0 if the shape is not supported. */
+size_t vla_ternary_packed_bytes(int N, int K);
+
+/* Bytes of scratch vla_ternary_gemm / vla_ternary_linear need for (M,N,K,path); a multiple of 256.
+ * vla_ternary_linear uses it for the quantised activations when xq_opt / x_scale_opt are NULL. */
+size_t vla_ternary_workspace_bytes(int M, int N, int K, vla_path path);
+
+/* Weight packer (offline, once per tensor).
+ *   w            [N,K] int8, every element in {-1,0,+1}
+ *   packed       packed_bytes >= vla_ternary_packed_bytes(N,K); layout is private to the library
+ *                (tile-permuted 2-bit two's-complement codes), defined only by pack/unpack
+ * SYNCHRONISES `stream`.  Returns VLA_ERR_VALUE if any element is outside {-1,0,+1}
+ * (packed is then unspecified). */
+vla_status vla_ternary_pack(const int8_t* w, int N, int K, void* packed, size_t packed_bytes, void* stream);
+
+/* Inverse of vla_ternary_pack: w[N,K] int8.  unpack(pack(W)) == W. */
+vla_status vla_ternary_unpack(const void* packed, int N, int K, int8_t* w, void* stream);
+
+/* Activation quantiser, Eq. 4 lines 1-2, per row m:
+ *   alpha_m = fmaxf(absmax_m, 1e-5f) / 127.0f          (fp32 division, round-to-nearest)
+ *   a_mj    = clamp(rint(x_mj / alpha_m), -127, 127)    (fp32 division, round-half-to-even)
+ *   x_bf16  [M,K] bf16          xq [M,K] int8          x_scale [M] fp32 (= alpha_m) */
+vla_status vla_act_quant(const void* x_bf16, int M, int K, int8_t* xq, float* x_scale, void* stream);
+
+/* Ternary GEMM + dequant epilogue, Eq. 4 line 3:
+ *   acc_mn = sum_j xq_mj * q_nj  (int32, exact);  y_mn = (float)acc_mn * (x_scale_m * w_scale)
+ *   packed     from vla_ternary_pack for the same (N,K)
+ *   w_scale    device pointer to ONE fp32 (beta, the per-tensor checkpoint scale); unused for VLA_I32
+ *   xq         [M,K] int8, x_scale [M] fp32 (from vla_act_quant; x_scale unused for VLA_I32)
+ *   out        [M,N] of out_dtype
+ *   workspace  >= vla_ternary_workspace_bytes(M,N,K,path) bytes (may be NULL if that is 0) */
+vla_status vla_ternary_gemm(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
+                            int M, int N, int K, void* out, vla_dtype out_dtype, vla_path path,
+                            void* workspace, size_t workspace_bytes, void* stream);
+
+/* Eq. 4 end to end with the activation quant fused into the call: x_bf16 [M,K] -> out [M,N].
+ *   xq_opt / x_scale_opt   optional outputs ([M,K] int8, [M] fp32): also return the quantised
+ *                          activations; when NULL they live in `workspace`. */
+vla_status vla_ternary_linear(const void* packed, const float* w_scale, const void* x_bf16,
+                              int M, int N, int K, void* out, vla_dtype out_dtype, vla_path path,
+                              int8_t* xq_opt, float* x_scale_opt,
+                              void* workspace, size_t workspace_bytes, void* stream);
+
+/* The path VLA_PATH_AUTO resolves to for (M,N,K). */
+vla_path vla_ternary_auto_path(int M, int N, int K);
+
+/* Measurement aid (not on the hot path): issue `mmas_per_cta` back-to-back
+ * tcgen05.mma.cta_group::1.kind::i8 (M=128, N=256, K=32) per CTA on `ctas` CTAs with no loads,
+ * and return the elapsed milliseconds through the HOST pointer ms_out.  Gives the box's INT8
+ * tensor-pipe ceiling: ops = 2*128*256*32 * mmas_per_cta * ctas.  Synchronises the device. */
+vla_status vla_i8_mma_issue_probe(int ctas, int mmas_per_cta, float* ms_out /*host*/);
+
+const char* vla_status_string(vla_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VLA_TERNARY_H */

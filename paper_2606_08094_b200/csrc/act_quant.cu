@@ -1,0 +1,93 @@
+// act_quant.cu -- per-token absmax int8 activation quantiser, Eq. 4 lines 1-2.
+//   alpha_m = fmaxf(absmax_m, 1e-5f) / 127.0f        true fp32 division (reading R1)
+//   a_mj    = clamp(rint(x_mj / alpha_m), +-127)     true fp32 division, round-half-to-even (R1-R3)
+// One CTA per row: the row (<= 16 KB of bf16 for K <= 8192) is read with 128-bit loads into registers,
+// reduced to its absmax (warp shuffles + one smem hop), then quantised from the registers: one pass
+// over HBM.  Rows longer than the register window are re-read (they hit L1/L2).
+#include <cuda_bf16.h>
+#include "common.cuh"
+#include "kernels.h"
+
+namespace vla {
+
+constexpr int AQ_THREADS = 256;
+constexpr int AQ_VEC_PER_THREAD = 4;                    // 4 x 8 bf16 per thread in registers -> K <= 8192
+
+__device__ __forceinline__ float bf16lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
+
+__device__ __forceinline__ float absmax8(uint4 v, float m) {
+    m = fmaxf(m, fabsf(bf16lo(v.x))); m = fmaxf(m, fabsf(bf16hi(v.x)));
+    m = fmaxf(m, fabsf(bf16lo(v.y))); m = fmaxf(m, fabsf(bf16hi(v.y)));
+    m = fmaxf(m, fabsf(bf16lo(v.z))); m = fmaxf(m, fabsf(bf16hi(v.z)));
+    m = fmaxf(m, fabsf(bf16lo(v.w))); m = fmaxf(m, fabsf(bf16hi(v.w)));
+    return m;
+}
+
+__device__ __forceinline__ uint32_t q1(float x, float alpha) {
+    float t = __fdiv_rn(x, alpha);
+    int r = __float2int_rn(t);                           // round-half-to-even
+    r = max(-127, min(127, r));
+    return (uint32_t)r & 0xFFu;
+}
+
+__device__ __forceinline__ uint2 quant8(uint4 v, float alpha) {
+    uint2 o;
+    o.x = q1(bf16lo(v.x), alpha) | (q1(bf16hi(v.x), alpha) << 8) | (q1(bf16lo(v.y), alpha) << 16) | (q1(bf16hi(v.y), alpha) << 24);
+    o.y = q1(bf16lo(v.z), alpha) | (q1(bf16hi(v.z), alpha) << 8) | (q1(bf16lo(v.w), alpha) << 16) | (q1(bf16hi(v.w), alpha) << 24);
+    return o;
+}
+
+__global__ void __launch_bounds__(AQ_THREADS) act_quant_kernel(const uint4* __restrict__ x, int K,
+                                                               uint2* __restrict__ xq, float* __restrict__ x_scale) {
+    __shared__ float s_max[AQ_THREADS / 32];
+    pdl_wait();                                          // x may be the previous kernel's output
+    const int row = blockIdx.x;
+    const int nvec = K / 8;
+    const uint4* xr = x + (size_t)row * nvec;
+    uint2* qr = xq + (size_t)row * nvec;
+
+    uint4 v[AQ_VEC_PER_THREAD];
+    float m = 0.0f;
+#pragma unroll
+    for (int i = 0; i < AQ_VEC_PER_THREAD; ++i) {
+        int idx = threadIdx.x + i * AQ_THREADS;
+        v[i] = (idx < nvec) ? xr[idx] : make_uint4(0, 0, 0, 0);
+    }
+#pragma unroll
+    for (int i = 0; i < AQ_VEC_PER_THREAD; ++i) m = absmax8(v[i], m);
+    for (int idx = threadIdx.x + AQ_VEC_PER_THREAD * AQ_THREADS; idx < nvec; idx += AQ_THREADS) m = absmax8(xr[idx], m);
+
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+    if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = m;
+    __syncthreads();
+    m = s_max[0];
+#pragma unroll
+    for (int i = 1; i < AQ_THREADS / 32; ++i) m = fmaxf(m, s_max[i]);
+
+    const float alpha = __fdiv_rn(fmaxf(m, 1e-5f), 127.0f);
+    if (threadIdx.x == 0) x_scale[row] = alpha;
+    pdl_launch_dependents();
+#pragma unroll
+    for (int i = 0; i < AQ_VEC_PER_THREAD; ++i) {
+        int idx = threadIdx.x + i * AQ_THREADS;
+        if (idx < nvec) qr[idx] = quant8(v[i], alpha);
+    }
+    for (int idx = threadIdx.x + AQ_VEC_PER_THREAD * AQ_THREADS; idx < nvec; idx += AQ_THREADS) qr[idx] = quant8(xr[idx], alpha);
+}
+
+cudaError_t launch_act_quant(const void* x_bf16, int M, int K, int8_t* xq, float* x_scale, cudaStream_t s) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)M);
+    cfg.blockDim = dim3(AQ_THREADS);
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, act_quant_kernel, (const uint4*)x_bf16, K, (uint2*)xq, x_scale);
+}
+
+}  // namespace vla

@@ -1,0 +1,20 @@
+// kernels.h -- host-side launchers of the CUDA kernels (internal to libvlaternary.so).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace vla {
+
+cudaError_t launch_pack(const int8_t* w, int N, int K, void* packed, int* bad_flag, cudaStream_t s);
+cudaError_t launch_unpack(const void* packed, int N, int K, int8_t* w, cudaStream_t s);
+cudaError_t launch_act_quant(const void* x_bf16, int M, int K, int8_t* xq, float* x_scale, cudaStream_t s);
+
+// out_dtype: 0 fp32, 1 bf16, 2 raw int32 (vla_dtype)
+cudaError_t launch_gemm_small(bool use_mma, const void* packed, const float* w_scale, const int8_t* xq,
+                              const float* x_scale, int M, int N, int K, void* out, int out_dtype, cudaStream_t s);
+cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
+                              int M, int N, int K, void* out, int out_dtype, cudaStream_t s);
+cudaError_t run_i8_mma_probe(int ctas, int mmas_per_cta, float* ms_out);
+
+}  // namespace vla
