@@ -1,0 +1,467 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the ternary-linear hot path (arxiv/paper_2606_08094 Eq. 4) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload decode|prefill] [--impl reference]
+
+Workload (BASELINE.json configs[1], the default): the four BitNet-2B-class linears
+(K,N) in {(2560,2560),(2560,640),(2560,6912),(6912,2560)} at M in {1,8,16}; a STEP is one pass of the
+whole hot path (activation quant -> packed-weight decode -> int8 contraction -> dequant epilogue, i.e.
+vla_ternary_linear with bf16 output) over all 12 points.  `--workload prefill` is configs[2] (M=544, fp32
+out).  The metric is BASELINE.json's: algorithmic HBM GB/s (packed weights + bf16 activations in + outputs
+out) with the TOPS (2MNK) beside it and the roofline fraction of the
+dominant kernel.  Weights are kept COLD: every step reads its packed weights from the next slot of a ring
+of copies whose total size exceeds twice the L2, so the GB/s are HBM GB/s, not L2 GB/s.
+
+Timing: the launches of a step are captured in CUDA graphs (the paper's own remedy for dispatch overhead,
+PAPER.md line 56) and replayed; CUDA events on the launching stream; barrier + synchronize on both sides;
+max over ranks.  Multi-GPU: the path runs on one GPU (BASELINE.json north_star) -> replicas only, weak
+scaling, no collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+NOMINAL_HBM_GBS = 8000.0           # BASELINE.json north_star "~8 TB/s"
+NOMINAL_INT8_TOPS = 4500.0         # dense int8, datasheet (same rate as fp8)
+
+
+# ----------------------------------------------------------------------------- workload description
+def workload_points(name):
+    """[(M, shape_idx)] of one step, in execution order."""
+    from paper_2606_08094_b200 import synth
+    if name == "decode":
+        return [(M, si) for M in synth.DECODE_M for si in range(len(synth.MODEL_SHAPES))]
+    if name == "prefill":
+        return [(synth.PREFILL_M, si) for si in range(len(synth.MODEL_SHAPES))]
+    raise ValueError(name)
+
+
+def out_elem_bytes(workload):
+    return 2 if workload == "decode" else 4       # configs[1]: bf16 output; configs[2]: fp32 output
+
+
+def point_bytes(M, K, N, out_bytes, fused_quant=True):
+    """Algorithmic bytes of one call: packed W + beta + X in + Y out."""
+    x_in = 2 * M * K if fused_quant else M * K + 4 * M
+    return N * K // 4 + 4 + x_in + M * N * out_bytes
+
+
+def point_ops(M, K, N):
+    return 2 * M * N * K
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d.get("bf16_tflops", 0.0)),
+                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", 0.0)), source="measured")
+    return dict(hbm_gbs=FALLBACK_HBM_GBS, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+
+
+def ncu_traffic(kernel_key):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(kernel_key)
+    return None
+
+
+# ----------------------------------------------------------------------------- clocks sampler
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [t.strip() for t in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                    samples=len(sm))
+
+
+# ----------------------------------------------------------------------------- reference arm (the oracle)
+def oracle_step_inputs(workload):
+    from paper_2606_08094_b200 import synth
+    pts = []
+    cache = {}
+    for (M, si) in workload_points(workload):
+        c = synth.config1_point(si, M) if workload == "decode" else synth.config2_point(si)
+        if si in cache:
+            c["w"] = cache[si]
+        cache[si] = c["w"]
+        pts.append(c)
+    return pts
+
+
+def oracle_time_steps(workload, pts, steps, budget_s=None, row_cap=None):
+    """Times the oracle, as it stands, on `steps` passes over the points (optionally only the first row_cap
+    rows of each point's activations: a bounded sample).  Returns (seconds, steps_done, bytes, ops)."""
+    from oracle import oracle as orc
+    ob = out_elem_bytes(workload)
+    nbytes = nops = 0
+    t0 = time.perf_counter()
+    done = 0
+    for _ in range(steps):
+        for c in pts:
+            x = c["x"] if row_cap is None else c["x"][:row_cap]
+            M = x.shape[0]
+            orc.ternary_linear(x, c["w"], c["beta"], want_y64=False)
+            nbytes += point_bytes(M, c["K"], c["N"], ob)
+            nops += point_ops(M, c["K"], c["N"])
+        done += 1
+        if budget_s is not None and time.perf_counter() - t0 > budget_s:
+            break
+    return time.perf_counter() - t0, done, nbytes, nops
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import oracle as orc
+    orc.build()
+    pts = oracle_step_inputs(args.workload)
+    cap = None if args.workload == "decode" else 32      # prefill: 32 of the 544 rows per point per step
+    oracle_time_steps(args.workload, pts, min(args.warmup, 1), row_cap=cap)
+    sec, done, nbytes, nops = oracle_time_steps(args.workload, pts, args.steps, budget_s=150.0, row_cap=cap)
+    val = nbytes / sec / 1e9
+    sample = "all 12 points, all rows" if cap is None else "first %d rows of each of the 4 points" % cap
+    line = {
+        "impl": "reference", "metric": "ternary_linear_algorithmic_hbm_gbs", "value": val, "unit": "GB/s",
+        "n_gpus": args.gpus, "steps": done, "warmup": min(args.warmup, 1), "ms_per_step": sec / done * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8*ternary->int32",
+        "data": "synthetic", "tops": nops / sec / 1e12,
+        "config": {"workload": "configs[1] decode" if args.workload == "decode" else "configs[2] prefill M=544"},
+        "cpu_baseline": {"value": val, "unit": "GB/s", "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- distributed plumbing
+def dist_setup(n_gpus):
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        dist.init_process_group(backend=backend)
+    return world, rank, local
+
+
+def dist_barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def reduce_max_and_sum(world, t_local, units_local, device):
+    """max over ranks of the time, sum over ranks of the units (replicas: whole-job units / slowest rank)."""
+    import torch
+    if world == 1:
+        return t_local, units_local
+    import torch.distributed as dist
+    t = torch.tensor([t_local], dtype=torch.float64, device=device)
+    u = torch.tensor([units_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ----------------------------------------------------------------------------- GPU arm
+class GpuWorkload:
+    """Device-resident state of one workload: a ring of packed-weight copies per shape (cold weights), and per
+    point the activation / output / workspace buffers plus pinned host mirrors for the end-to-end leg."""
+
+    def __init__(self, vla, workload, device):
+        import torch
+        from paper_2606_08094_b200 import synth
+        self.vla, self.torch, self.workload, self.device = vla, torch, workload, device
+        self.points = workload_points(workload)
+        self.out_dtype = vla.VLA_BF16 if workload == "decode" else vla.VLA_F32
+        self.out_bytes = out_elem_bytes(workload)
+        self.uses = max(1, len(self.points) // len(synth.MODEL_SHAPES))       # times a shape is used per step
+        l2 = torch.cuda.get_device_properties(device).L2_cache_size
+        per_copy = sum(n * k // 4 for (k, n) in synth.MODEL_SHAPES)
+        copies = -(-2 * l2 // per_copy)
+        copies = -(-copies // self.uses) * self.uses
+        self.copies, self.rev_steps, self.l2 = copies, copies // self.uses, l2
+        self.ring, self.beta = [], []
+        xs_full = {}
+        for si, (K, N) in enumerate(synth.MODEL_SHAPES):
+            c = synth.config1_point(si, max(synth.DECODE_M)) if workload == "decode" else synth.config2_point(si)
+            w = torch.from_numpy(c["w"]).to(device)
+            packed = vla.pack_weights(w)
+            self.ring.append(packed.unsqueeze(0).repeat(copies, 1).contiguous())
+            self.beta.append(torch.tensor([float(c["beta"])], dtype=torch.float32, device=device))
+            xs_full[si] = c["x"]
+            del w
+        self.buf = []
+        for (M, si) in self.points:
+            K, N = synth.MODEL_SHAPES[si]
+            xb = np.ascontiguousarray(xs_full[si][:M])
+            x_host = torch.from_numpy(xb.view(np.int16)).view(torch.bfloat16).pin_memory()
+            dt = torch.bfloat16 if self.out_dtype == vla.VLA_BF16 else torch.float32
+            ws_bytes = vla.vla_ternary_host_workspace_bytes(M, N, K, self.out_dtype)
+            self.buf.append(dict(
+                M=M, K=K, N=N, si=si, x=x_host.to(device), x_host=x_host,
+                out=torch.empty((M, N), dtype=dt, device=device), out_host=torch.empty((M, N), dtype=dt).pin_memory(),
+                xq=torch.empty((M, K), dtype=torch.int8, device=device),
+                xs=torch.empty((M,), dtype=torch.float32, device=device),
+                ws=torch.empty(ws_bytes, dtype=torch.uint8, device=device), ws_bytes=ws_bytes))
+        self.step_bytes = sum(point_bytes(b["M"], b["K"], b["N"], self.out_bytes) for b in self.buf)
+        self.step_ops = sum(point_ops(b["M"], b["K"], b["N"]) for b in self.buf)
+        self.gemm_bytes = sum(point_bytes(b["M"], b["K"], b["N"], self.out_bytes, fused_quant=False) for b in self.buf)
+        self.h2d = sum(2 * b["M"] * b["K"] for b in self.buf)
+        self.d2h = sum(self.out_bytes * b["M"] * b["N"] for b in self.buf)
+
+    def slot(self, step, pi):
+        return (step * self.uses + pi // 4) % self.copies
+
+    def launch_point(self, pi, step, mode="linear"):
+        b, vla = self.buf[pi], self.vla
+        packed = self.ring[b["si"]][self.slot(step, pi)]
+        if mode == "linear":          # the whole hot path: quant fused into the call
+            vla.vla_ternary_linear(packed, self.beta[b["si"]], b["x"], b["M"], b["N"], b["K"], b["out"], self.out_dtype,
+                                   vla.VLA_PATH_AUTO, b["xq"], b["xs"], b["ws"], b["ws_bytes"])
+        elif mode == "gemm":          # the dominant kernel alone, on pre-quantised activations
+            vla.vla_ternary_gemm(packed, self.beta[b["si"]], b["xq"], b["xs"], b["M"], b["N"], b["K"], b["out"],
+                                 self.out_dtype, vla.VLA_PATH_AUTO, b["ws"], b["ws_bytes"])
+        elif mode == "host":          # end to end: pinned host x -> device -> kernels -> pinned host y, synchronised
+            vla.vla_ternary_linear_host(packed, self.beta[b["si"]], b["x_host"], b["M"], b["N"], b["K"], b["out_host"],
+                                        self.out_dtype, vla.VLA_PATH_AUTO, b["ws"], b["ws_bytes"])
+
+    def launch_step(self, step, mode="linear", only=None):
+        for pi in range(len(self.buf)):
+            if only is None or pi == only:
+                self.launch_point(pi, step, mode)
+
+    def capture(self, steps, mode="linear", only=None):
+        """CUDA graph of `steps` = [step indices]; returns (graph, kernels launched per replay)."""
+        torch = self.torch
+        n0 = self.vla.vla_launch_count()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for s in steps:
+                self.launch_step(s, mode, only)
+        return g, self.vla.vla_launch_count() - n0
+
+
+def time_replays(torch, plan):
+    """plan: list of graphs to replay in order.  Returns milliseconds (CUDA events on the current stream)."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for g in plan:
+        g.replay()
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def run_gpu(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path (use --impl reference for the oracle)")
+    from paper_2606_08094_b200 import binding as vla
+    world, rank, local = dist_setup(args.gpus)
+    device = torch.device("cuda", local)
+    torch.cuda.set_device(device)
+    wl = GpuWorkload(vla, args.workload, device)
+    rev = wl.rev_steps
+
+    # warm-up, eager (also sets function attributes outside any capture)
+    for s in range(max(args.warmup, 3)):
+        wl.launch_step(s)
+        wl.launch_step(s, "gemm")
+    torch.cuda.synchronize()
+
+    g_rev, n_rev = wl.capture(list(range(rev)))
+    singles = {}
+    plan, launches = [], 0
+    full, rem = divmod(args.steps, rev)
+    plan += [g_rev] * full
+    launches += n_rev * full
+    for s in range(rem):
+        singles[s], n1 = wl.capture([s])
+        plan.append(singles[s])
+        launches += n1
+    warm_plan = [g_rev] * max(1, -(-args.warmup // rev))
+    time_replays(torch, warm_plan)
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.12)
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    ms_local = time_replays(torch, plan)
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    clocks = sampler.stop() if rank == 0 else None
+    ms, total_bytes = reduce_max_and_sum(world, ms_local, float(wl.step_bytes) * args.steps, device)
+    _, total_ops = reduce_max_and_sum(world, ms_local, float(wl.step_ops) * args.steps, device)
+
+    # ---- end-to-end leg: host buffers through the C ABI, copies inside the timed region
+    e2e_steps = max(3, min(args.steps, args.e2e_steps))
+    for s in range(3):
+        wl.launch_step(s, "host")
+    torch.cuda.synchronize()
+    dist_barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for s in range(e2e_steps):
+        wl.launch_step(s, "host")
+    e1.record()
+    e1.synchronize()
+    dist_barrier(world)
+    e2e_ms, e2e_bytes = reduce_max_and_sum(world, e0.elapsed_time(e1), float(wl.step_bytes) * e2e_steps, device)
+
+    if rank != 0:
+        return 0
+
+    # ---- roofline of the dominant kernel (the GEMM), timed alone on pre-quantised activations, cold ring
+    pk = peaks()
+    g_gemm, n_gemm = wl.capture(list(range(rev)), "gemm")
+    time_replays(torch, [g_gemm] * 2)
+    reps = max(3, min(200, int(2e5 / max(1, n_gemm))))
+    gemm_ms = time_replays(torch, [g_gemm] * reps)
+    per_launch_s = gemm_ms * 1e-3 / (reps * n_gemm)
+    if args.workload == "decode":
+        alg = wl.gemm_bytes / len(wl.buf)                     # average algorithmic bytes per GEMM launch
+        achieved = alg / per_launch_s / 1e9
+        roof = {"bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / pk["hbm_gbs"], "traffic": ncu_traffic("gemm_small"),
+                "kernel": "gemm_small_kernel", "peak_source": pk["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
+                "alg_bytes_per_launch": alg, "us_per_launch": per_launch_s * 1e6,
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
+    else:
+        alg = wl.step_ops / len(wl.buf)
+        achieved = alg / per_launch_s / 1e12
+        peak_i8 = pk["bf16_tflops"] * 2.0                     # int8 : bf16 = 4.5 : 2.25 nominal
+        roof = {"bound": "tensor", "achieved": achieved, "peak": peak_i8, "unit": "TOP/s",
+                "frac": achieved / peak_i8, "traffic": ncu_traffic("gemm_large"),
+                "kernel": "gemm_large_kernel", "peak_source": pk["source"] + " bf16_tflops x 2 (int8:bf16 nominal ratio)",
+                "alg_ops_per_launch": alg, "us_per_launch": per_launch_s * 1e6,
+                "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS}
+
+    # ---- per-point table (the metric is "vs M"): each point alone, whole hot path, cold ring
+    table = []
+    if not args.no_points:
+        for pi, b in enumerate(wl.buf):
+            g, n = wl.capture(list(range(rev)), "linear", only=pi)
+            time_replays(torch, [g])
+            r = max(3, min(50, int(5e4 / rev)))
+            t = time_replays(torch, [g] * r) * 1e-3 / (r * rev)
+            by, op = point_bytes(b["M"], b["K"], b["N"], wl.out_bytes), point_ops(b["M"], b["K"], b["N"])
+            t_roof = max(by / (pk["hbm_gbs"] * 1e9), op / (pk["bf16_tflops"] * 2e12))
+            table.append({"M": b["M"], "K": b["K"], "N": b["N"], "us": t * 1e6, "GBs": by / t / 1e9,
+                          "TOPS": op / t / 1e12, "roofline_frac": t_roof / t,
+                          "path": int(vla.vla_ternary_auto_path(b["M"], b["N"], b["K"]))})
+            del g
+
+    # ---- the oracle on this box's host cores, bounded sample
+    from oracle import oracle as orc
+    orc.build()
+    pts = oracle_step_inputs(args.workload)
+    cap = None if args.workload == "decode" else 32
+    oracle_time_steps(args.workload, pts, 1, row_cap=cap)
+    sec, done, nbytes, nops = oracle_time_steps(args.workload, pts, 10 ** 6, budget_s=args.cpu_budget, row_cap=cap)
+    cpu = {"value": nbytes / sec / 1e9, "unit": "GB/s", "cores": orc.num_threads(), "kind": "oracle",
+           "sample": ("%d full steps (all 12 points, all rows)" % done) if cap is None
+           else ("%d steps of the first %d rows of each of the 4 points" % (done, cap)),
+           "tops": nops / sec / 1e12, "seconds": sec}
+
+    value = total_bytes / (ms * 1e-3) / 1e9
+    line = {
+        "metric": "ternary_linear_algorithmic_hbm_gbs", "value": value, "unit": "GB/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int8*ternary->int32", "data": "synthetic",
+        "tops": total_ops / (ms * 1e-3) / 1e12,
+        "config": {"workload": "configs[1] decode: 4 BitNet-2B linears x M in {1,8,16}, fused quant, bf16 out"
+                   if args.workload == "decode" else "configs[2] prefill: 4 BitNet-2B linears at M=544, fused quant, fp32 out",
+                   "cold_weights": "ring of %d packed copies per shape (%.0f MB > 2 x L2 %.0f MB), next slot every use"
+                   % (wl.copies, wl.copies * sum(r.shape[1] for r in wl.ring) / 1e6, wl.l2 / 1e6),
+                   "launch": "CUDA graphs of %d steps + PDL" % rev, "parallelism": "replicas" if world > 1 else "single"},
+        "clocks": clocks, "gpu_launches": launches,
+        "e2e": {"value": e2e_bytes / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": wl.h2d,
+                "d2h_bytes_per_step": wl.d2h, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+        "roofline": roof, "cpu_baseline": cpu, "points": table,
+        "step_roofline_frac_hbm": value / pk["hbm_gbs"],
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=4000)
+    ap.add_argument("--warmup", type=int, default=16)
+    ap.add_argument("--workload", choices=["decode", "prefill"], default="decode")
+    ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
+    ap.add_argument("--e2e-steps", type=int, default=200)
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle timing for cpu_baseline")
+    ap.add_argument("--no-points", action="store_true", help="skip the per-point table")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

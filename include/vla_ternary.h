@@ -103,6 +103,19 @@ vla_status vla_ternary_linear(const void* packed, const float* w_scale, const vo
                               int8_t* xq_opt, float* x_scale_opt,
                               void* workspace, size_t workspace_bytes, void* stream);
 
+/* Host-buffer form of vla_ternary_linear (the end-to-end call a serving process makes; the weights stay
+ * resident in HBM: "holds weights resident"):
+ *   x_bf16_host  HOST [M,K] bf16 (pinned memory for an asynchronous copy)
+ *   out_host     HOST [M,N] of out_dtype
+ *   workspace    DEVICE, >= vla_ternary_host_workspace_bytes(M,N,K,out_dtype,path): staging for x and out
+ *                plus the quantised activations
+ * Copies x host->device, runs Eq. 4 in the kernels, copies out device->host, all on `stream`, and
+ * SYNCHRONISES `stream` before returning. */
+size_t vla_ternary_host_workspace_bytes(int M, int N, int K, vla_dtype out_dtype, vla_path path);
+vla_status vla_ternary_linear_host(const void* packed, const float* w_scale, const void* x_bf16_host,
+                                   int M, int N, int K, void* out_host, vla_dtype out_dtype, vla_path path,
+                                   void* workspace, size_t workspace_bytes, void* stream);
+
 /* The path VLA_PATH_AUTO resolves to for (M,N,K). */
 vla_path vla_ternary_auto_path(int M, int N, int K);
 
@@ -113,6 +126,9 @@ vla_path vla_ternary_auto_path(int M, int N, int K);
 vla_status vla_i8_mma_issue_probe(int ctas, int mmas_per_cta, float* ms_out /*host*/);
 
 const char* vla_status_string(vla_status s);
+
+/* Number of kernels this library has launched so far in this process (instrumentation for benchmarks). */
+unsigned long long vla_launch_count(void);
 
 #ifdef __cplusplus
 }

@@ -1,0 +1,178 @@
+"""Thin ctypes binding of libvlaternary.so (include/vla_ternary.h) -- argument marshalling only.
+
+Every function has the name and argument order of its C entry point, takes torch CUDA tensors (or
+raw integer device pointers) for the device buffers, passes `tensor.data_ptr()` and the current
+torch CUDA stream, and raises VlaError on a non-zero vla_status.  Nothing is computed here: every
+step of Eq. 4 runs in the library's kernels.  There is no fallback: if the
+shared library cannot be loaded the import of this module fails.
+"""
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+VLA_OK = 0
+(VLA_ERR_NULL, VLA_ERR_SHAPE, VLA_ERR_ALIGN, VLA_ERR_VALUE, VLA_ERR_DTYPE, VLA_ERR_WORKSPACE,
+ VLA_ERR_ARCH, VLA_ERR_CUDA) = range(1, 9)
+VLA_F32, VLA_BF16, VLA_I32 = 0, 1, 2
+VLA_PATH_AUTO, VLA_PATH_SMALL_ALU, VLA_PATH_SMALL_TC, VLA_PATH_LARGE = 0, 1, 2, 3
+
+_TORCH_DTYPE = {VLA_F32: torch.float32, VLA_BF16: torch.bfloat16, VLA_I32: torch.int32}
+
+EXPORTS = [
+    "vla_ternary_packed_bytes", "vla_ternary_workspace_bytes", "vla_ternary_pack", "vla_ternary_unpack",
+    "vla_act_quant", "vla_ternary_gemm", "vla_ternary_linear", "vla_ternary_linear_host",
+    "vla_ternary_host_workspace_bytes",
+    "vla_ternary_auto_path", "vla_i8_mma_issue_probe", "vla_status_string", "vla_launch_count",
+]
+
+
+class VlaError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        super().__init__("%s: %s" % (where, vla_status_string(status)))
+
+
+def _load():
+    so = _build.SO
+    if not os.path.exists(so):
+        _build.build()          # needs nvcc; raises if the toolchain is missing -- no fallback
+    lib = ctypes.CDLL(so)
+    vp, i, sz, st = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_int
+    lib.vla_ternary_packed_bytes.restype = sz
+    lib.vla_ternary_packed_bytes.argtypes = [i, i]
+    lib.vla_ternary_workspace_bytes.restype = sz
+    lib.vla_ternary_workspace_bytes.argtypes = [i, i, i, i]
+    lib.vla_ternary_pack.restype = st
+    lib.vla_ternary_pack.argtypes = [vp, i, i, vp, sz, vp]
+    lib.vla_ternary_unpack.restype = st
+    lib.vla_ternary_unpack.argtypes = [vp, i, i, vp, vp]
+    lib.vla_act_quant.restype = st
+    lib.vla_act_quant.argtypes = [vp, i, i, vp, vp, vp]
+    lib.vla_ternary_gemm.restype = st
+    lib.vla_ternary_gemm.argtypes = [vp, vp, vp, vp, i, i, i, vp, i, i, vp, sz, vp]
+    lib.vla_ternary_linear.restype = st
+    lib.vla_ternary_linear.argtypes = [vp, vp, vp, i, i, i, vp, i, i, vp, vp, vp, sz, vp]
+    lib.vla_ternary_linear_host.restype = st
+    lib.vla_ternary_linear_host.argtypes = [vp, vp, vp, i, i, i, vp, i, i, vp, sz, vp]
+    lib.vla_ternary_host_workspace_bytes.restype = sz
+    lib.vla_ternary_host_workspace_bytes.argtypes = [i, i, i, i, i]
+    lib.vla_ternary_auto_path.restype = i
+    lib.vla_ternary_auto_path.argtypes = [i, i, i]
+    lib.vla_i8_mma_issue_probe.restype = st
+    lib.vla_i8_mma_issue_probe.argtypes = [i, i, ctypes.POINTER(ctypes.c_float)]
+    lib.vla_status_string.restype = ctypes.c_char_p
+    lib.vla_status_string.argtypes = [st]
+    lib.vla_launch_count.restype = ctypes.c_ulonglong
+    lib.vla_launch_count.argtypes = []
+    return lib
+
+
+_lib = _load()
+LIB_PATH = _build.SO
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    return t.data_ptr()
+
+
+def _stream(stream):
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _check(status, where):
+    if status != VLA_OK:
+        raise VlaError(status, where)
+
+
+def vla_status_string(status):
+    return _lib.vla_status_string(int(status)).decode()
+
+
+def vla_ternary_packed_bytes(N, K):
+    return int(_lib.vla_ternary_packed_bytes(N, K))
+
+
+def vla_ternary_workspace_bytes(M, N, K, path=VLA_PATH_AUTO):
+    return int(_lib.vla_ternary_workspace_bytes(M, N, K, path))
+
+
+def vla_ternary_auto_path(M, N, K):
+    return int(_lib.vla_ternary_auto_path(M, N, K))
+
+
+def vla_launch_count():
+    """Number of kernels this library has launched in this process (for bench.py's gpu_launches)."""
+    return int(_lib.vla_launch_count())
+
+
+def vla_ternary_pack(w, N, K, packed, packed_bytes=None, stream=None):
+    if packed_bytes is None:
+        packed_bytes = packed.numel() * packed.element_size()
+    _check(_lib.vla_ternary_pack(_ptr(w), N, K, _ptr(packed), packed_bytes, _stream(stream)), "vla_ternary_pack")
+
+
+def vla_ternary_unpack(packed, N, K, w, stream=None):
+    _check(_lib.vla_ternary_unpack(_ptr(packed), N, K, _ptr(w), _stream(stream)), "vla_ternary_unpack")
+
+
+def vla_act_quant(x_bf16, M, K, xq, x_scale, stream=None):
+    _check(_lib.vla_act_quant(_ptr(x_bf16), M, K, _ptr(xq), _ptr(x_scale), _stream(stream)), "vla_act_quant")
+
+
+def vla_ternary_gemm(packed, w_scale, xq, x_scale, M, N, K, out, out_dtype, path=VLA_PATH_AUTO,
+                     workspace=None, workspace_bytes=0, stream=None):
+    _check(_lib.vla_ternary_gemm(_ptr(packed), _ptr(w_scale), _ptr(xq), _ptr(x_scale), M, N, K, _ptr(out),
+                                 out_dtype, path, _ptr(workspace), workspace_bytes, _stream(stream)),
+           "vla_ternary_gemm")
+
+
+def vla_ternary_linear(packed, w_scale, x_bf16, M, N, K, out, out_dtype, path=VLA_PATH_AUTO,
+                       xq_opt=None, x_scale_opt=None, workspace=None, workspace_bytes=0, stream=None):
+    _check(_lib.vla_ternary_linear(_ptr(packed), _ptr(w_scale), _ptr(x_bf16), M, N, K, _ptr(out), out_dtype, path,
+                                   _ptr(xq_opt), _ptr(x_scale_opt), _ptr(workspace), workspace_bytes,
+                                   _stream(stream)), "vla_ternary_linear")
+
+
+def vla_ternary_host_workspace_bytes(M, N, K, out_dtype, path=VLA_PATH_AUTO):
+    return int(_lib.vla_ternary_host_workspace_bytes(M, N, K, out_dtype, path))
+
+
+def vla_ternary_linear_host(packed, w_scale, x_bf16_host, M, N, K, out_host, out_dtype, path,
+                            workspace, workspace_bytes, stream=None):
+    """x_bf16_host / out_host: HOST tensors (pinned for asynchronous copies).  Synchronises the stream."""
+    _check(_lib.vla_ternary_linear_host(_ptr(packed), _ptr(w_scale), _ptr(x_bf16_host), M, N, K, _ptr(out_host),
+                                        out_dtype, path, _ptr(workspace), workspace_bytes, _stream(stream)),
+           "vla_ternary_linear_host")
+
+
+def vla_i8_mma_issue_probe(ctas, mmas_per_cta):
+    ms = ctypes.c_float(0.0)
+    _check(_lib.vla_i8_mma_issue_probe(ctas, mmas_per_cta, ctypes.byref(ms)), "vla_i8_mma_issue_probe")
+    return float(ms.value)
+
+
+# ------------------------------------------------------------------ conveniences (allocation only)
+def pack_weights(w_i8):
+    """int8 [N,K] CUDA tensor -> uint8 packed tensor of vla_ternary_packed_bytes(N,K) bytes."""
+    N, K = w_i8.shape
+    nbytes = vla_ternary_packed_bytes(N, K)
+    if nbytes == 0:
+        raise VlaError(VLA_ERR_SHAPE, "pack_weights")
+    packed = torch.empty(nbytes, dtype=torch.uint8, device=w_i8.device)
+    vla_ternary_pack(w_i8.contiguous(), N, K, packed, nbytes)
+    return packed
+
+
+def empty_out(M, N, out_dtype, device="cuda"):
+    return torch.empty((M, N), dtype=_TORCH_DTYPE[out_dtype], device=device)

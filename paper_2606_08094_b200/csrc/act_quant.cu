@@ -87,6 +87,7 @@ cudaError_t launch_act_quant(const void* x_bf16, int M, int K, int8_t* xq, float
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
+    count_launch();
     return cudaLaunchKernelEx(&cfg, act_quant_kernel, (const uint4*)x_bf16, K, (uint2*)xq, x_scale);
 }
 

@@ -2,7 +2,14 @@
 // Nothing here computes: every step of the path runs in the kernels of pack.cu, act_quant.cu,
 // gemm_small.cu and gemm_large.cu.
 #include "../../include/vla_ternary.h"
+#include <atomic>
 #include "kernels.h"
+
+namespace vla {
+static std::atomic<unsigned long long> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+unsigned long long launch_count() { return g_launches.load(std::memory_order_relaxed); }
+}  // namespace vla
 
 namespace {
 
@@ -170,6 +177,40 @@ vla_status vla_ternary_linear(const void* packed, const float* w_scale, const vo
     if (st != VLA_OK) return st;
     return vla_ternary_gemm(packed, w_scale, xq, xs, M, N, K, out, out_dtype, path, nullptr, 0, stream);
 }
+
+size_t vla_ternary_host_workspace_bytes(int M, int N, int K, vla_dtype out_dtype, vla_path path) {
+    size_t inner = vla_ternary_workspace_bytes(M, N, K, path);
+    if (inner == 0 || (int)out_dtype < 0 || (int)out_dtype > 2) return 0;
+    size_t esz = (out_dtype == VLA_BF16) ? 2 : 4;
+    return inner + round256((size_t)M * K * 2) + round256((size_t)M * N * esz);
+}
+
+vla_status vla_ternary_linear_host(const void* packed, const float* w_scale, const void* x_bf16_host,
+                                   int M, int N, int K, void* out_host, vla_dtype out_dtype, vla_path path,
+                                   void* workspace, size_t workspace_bytes, void* stream) {
+    if (!x_bf16_host || !out_host) return VLA_ERR_NULL;
+    if ((int)out_dtype < 0 || (int)out_dtype > 2 || (int)path < 0 || (int)path > 3) return VLA_ERR_DTYPE;
+    if (M < 1 || !shape_ok(N, K)) return VLA_ERR_SHAPE;
+    const size_t need = vla_ternary_host_workspace_bytes(M, N, K, out_dtype, path);
+    if (!workspace || workspace_bytes < need) return VLA_ERR_WORKSPACE;
+    if (!aligned16(workspace)) return VLA_ERR_ALIGN;
+    const size_t inner = vla_ternary_workspace_bytes(M, N, K, path);
+    const size_t xbytes = (size_t)M * K * 2, obytes = (size_t)M * N * ((out_dtype == VLA_BF16) ? 2 : 4);
+    uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+    void* x_dev = ws + inner;
+    void* out_dev = ws + inner + round256(xbytes);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(x_dev, x_bf16_host, xbytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return from_cuda(e);
+    vla_status st = vla_ternary_linear(packed, w_scale, x_dev, M, N, K, out_dev, out_dtype, path, nullptr, nullptr,
+                                       workspace, inner, stream);
+    if (st != VLA_OK) return st;
+    e = cudaMemcpyAsync(out_host, out_dev, obytes, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    return from_cuda(e);
+}
+
+unsigned long long vla_launch_count(void) { return vla::launch_count(); }
 
 vla_status vla_i8_mma_issue_probe(int ctas, int mmas_per_cta, float* ms_out) {
     if (!ms_out) return VLA_ERR_NULL;

@@ -227,6 +227,7 @@ cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const in
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
+    count_launch();
     return cudaLaunchKernelEx(&cfg, gemm_large_kernel, tm, (const uint8_t*)packed, w_scale, x_scale, out,
                               M, N, K, TN, cols, out_dtype);
 }
@@ -265,6 +266,7 @@ cudaError_t run_i8_mma_probe(int ctas, int mmas_per_cta, float* ms_out) {
     cudaEvent_t a, b;
     cudaEventCreate(&a);
     cudaEventCreate(&b);
+    count_launch(2);
     i8_mma_probe_kernel<<<ctas, 64, smem>>>(mmas_per_cta);      // warm-up
     cudaEventRecord(a);
     i8_mma_probe_kernel<<<ctas, 64, smem>>>(mmas_per_cta);

@@ -222,6 +222,7 @@ static cudaError_t launch_one(const void* packed, const float* w_scale, const in
     }
     cfg.attrs = at;
     cfg.numAttrs = na;
+    count_launch();
     return cudaLaunchKernelEx(&cfg, gemm_small_kernel<MTOK, USE_MMA>, (const uint8_t*)packed, w_scale, xq, x_scale,
                               M, N, K, out, out_dtype, kq_per_cta, ksplit);
 }

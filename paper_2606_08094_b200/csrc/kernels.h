@@ -6,6 +6,10 @@
 
 namespace vla {
 
+// every launcher bumps this once per kernel it launches (vla_launch_count)
+void count_launch(int n = 1);
+unsigned long long launch_count();
+
 cudaError_t launch_pack(const int8_t* w, int N, int K, void* packed, int* bad_flag, cudaStream_t s);
 cudaError_t launch_unpack(const void* packed, int N, int K, int8_t* w, cudaStream_t s);
 cudaError_t launch_act_quant(const void* x_bf16, int M, int K, int8_t* xq, float* x_scale, cudaStream_t s);

@@ -61,12 +61,14 @@ __global__ void unpack_kernel(const uint32_t* __restrict__ packed, int N, int K,
 
 cudaError_t launch_pack(const int8_t* w, int N, int K, void* packed, int* bad_flag, cudaStream_t s) {
     size_t nwords = (size_t)N * K / 16;
+    count_launch();
     pack_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, s>>>(w, N, K, (uint32_t*)packed, bad_flag);
     return cudaGetLastError();
 }
 
 cudaError_t launch_unpack(const void* packed, int N, int K, int8_t* w, cudaStream_t s) {
     size_t nwords = (size_t)N * K / 16;
+    count_launch();
     unpack_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, s>>>((const uint32_t*)packed, N, K, w);
     return cudaGetLastError();
 }

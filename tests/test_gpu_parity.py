@@ -1,0 +1,321 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle, element by
+element on the same seeded inputs.  Bars (BASELINE.json north_star): int8 activations, fp32 alpha and
+int32 accumulators bit-exact; fp32 outputs within 1e-6 relative of the fp64 reference; bf16 outputs
+within 1 bf16 ulp of RNE(fp64 reference).  With the canonical operation order of DESIGN.md (readings
+R1, R6) the fp32 and bf16 outputs are also bit-identical to the oracle's, which is asserted too.
+"""
+import ctypes
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_08094_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL_F32 = 1e-6          # north_star: "fp32 outputs must agree within 1e-6 relative"
+
+
+@pytest.fixture(scope="module")
+def vla():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_2606_08094_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def dev_bf16(bits_u16):
+    return torch.from_numpy(np.ascontiguousarray(bits_u16).view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def bf16_bits_of(t):
+    return t.view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def bf16_ulp_distance(a_bits, b_bits):
+    """distance in units of bf16 ulps between two arrays of finite bf16 bit patterns (monotone integer map)"""
+    def key(b):
+        b = b.astype(np.int32)
+        return np.where(b & 0x8000, -(b & 0x7FFF), b & 0x7FFF)
+    return np.abs(key(a_bits) - key(b_bits))
+
+
+def run_gemm(vla, packed, beta, xq, xs, M, N, K, out_dtype, path):
+    out = vla.empty_out(M, N, out_dtype)
+    ws_bytes = vla.vla_ternary_workspace_bytes(M, N, K, path)
+    ws = torch.empty(max(ws_bytes, 16), dtype=torch.uint8, device="cuda")
+    vla.vla_ternary_gemm(packed, beta, xq, xs, M, N, K, out, out_dtype, path, ws, ws_bytes)
+    torch.cuda.synchronize()
+    return out
+
+
+def check_outputs(vla, oracle, packed, w, beta, x_bits, M, N, K, path):
+    """act_quant + gemm (all three output dtypes) on `path` vs the oracle."""
+    ref = oracle.ternary_linear(x_bits, w, beta)
+    x = dev_bf16(x_bits)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(x, M, K, xq, xs)
+    torch.cuda.synchronize()
+    assert np.array_equal(xq.cpu().numpy(), ref["a"]), "int8 activations differ"
+    assert np.array_equal(xs.cpu().numpy().view(np.uint32), ref["alpha"].view(np.uint32)), "alpha differs"
+    beta_d = dev(np.array([beta], np.float32))
+
+    acc = run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_I32, path).cpu().numpy()
+    bad = np.argwhere(acc != ref["acc"])
+    assert bad.size == 0, "int32 accumulators differ at %d places, first %s: got %d want %d" % (
+        len(bad), bad[0], acc[tuple(bad[0])], ref["acc"][tuple(bad[0])])
+
+    y = run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_F32, path).cpu().numpy()
+    y64 = ref["y64"]
+    err = np.abs(y.astype(np.float64) - y64)
+    assert np.all(err <= REL_TOL_F32 * np.abs(y64)), "fp32 output outside 1e-6 relative"
+    assert np.all(y[ref["acc"] == 0] == 0.0)
+    assert np.array_equal(y.view(np.uint32), ref["y32"].view(np.uint32)), "fp32 output not bit-identical"
+
+    yb = bf16_bits_of(run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_BF16, path))
+    want = oracle.f32_to_bf16(y64.astype(np.float32))
+    assert bf16_ulp_distance(yb, want).max() <= 1, "bf16 output more than 1 ulp from RNE(reference)"
+    assert np.array_equal(yb, ref["ybf16"]), "bf16 output not bit-identical"
+    return ref
+
+
+def paths_for(vla, M):
+    p = [vla.VLA_PATH_LARGE]
+    if M <= 16:
+        p.append(vla.VLA_PATH_SMALL_ALU)
+    if M <= 32:
+        p.append(vla.VLA_PATH_SMALL_TC)
+    return p
+
+
+# ---------------------------------------------------------------- packer
+@pytest.mark.parametrize("N,K", [(128, 128), (256, 256), (384, 640), (2560, 2560), (640, 2560)])
+def test_pack_unpack_round_trip(vla, N, K):
+    w = synth.ternary_weights(N, K, 0.35, 42 + N + K)
+    wd = dev(w)
+    packed = vla.pack_weights(wd)
+    assert packed.numel() == N * K // 4
+    back = torch.full((N, K), 99, dtype=torch.int8, device="cuda")
+    vla.vla_ternary_unpack(packed, N, K, back)
+    torch.cuda.synchronize()
+    assert torch.equal(back, wd)
+
+
+def test_pack_rejects_non_ternary(vla):
+    w = synth.ternary_weights(128, 256, 0.3, 1)
+    for bad in (2, -2, 127, -128):
+        w2 = w.copy()
+        w2[77, 133] = bad
+        with pytest.raises(vla.VlaError) as e:
+            vla.pack_weights(dev(w2))
+        assert e.value.status == vla.VLA_ERR_VALUE
+
+
+# ---------------------------------------------------------------- quantiser
+@pytest.mark.parametrize("M,K", [(1, 128), (8, 256), (16, 2560), (13, 6912), (544, 2560), (37, 8192), (3, 16384)])
+def test_act_quant_bit_exact(vla, oracle, M, K):
+    x_bits = synth.activations(M, K, 900 + M + K, outlier_frac=0.01)
+    a_ref, al_ref = oracle.act_quant(x_bits)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(x_bits), M, K, xq, xs)
+    torch.cuda.synchronize()
+    assert np.array_equal(xq.cpu().numpy(), a_ref)
+    assert np.array_equal(xs.cpu().numpy().view(np.uint32), al_ref.view(np.uint32))
+
+
+def test_act_quant_special_rows(vla, oracle):
+    """ties (0.8125, 0.40625 -> 127, 63 under true division), all-zero row, tiny row, heavy tails, negatives."""
+    K = 128
+    rows = np.zeros((6, K), np.float32)
+    rows[0, :2] = [0.8125, 0.40625]
+    rows[1, :4] = [1.0, -0.5, 0.25, 2.0]
+    rows[3, :3] = [3e-6, -1e-6, 2e-6]
+    rows[4] = np.random.default_rng(5).standard_t(3.0, K).astype(np.float32) * 50
+    rows[5] = -np.abs(np.random.default_rng(6).standard_normal(K).astype(np.float32))
+    x_bits = synth._f32_to_bf16_bits(rows)
+    a_ref, al_ref = oracle.act_quant(x_bits)
+    assert a_ref[0, :2].tolist() == [127, 63]
+    xq = torch.empty((6, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((6,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(x_bits), 6, K, xq, xs)
+    torch.cuda.synchronize()
+    assert np.array_equal(xq.cpu().numpy(), a_ref)
+    assert np.array_equal(xs.cpu().numpy().view(np.uint32), al_ref.view(np.uint32))
+    assert xq[2].abs().max().item() == 0
+
+
+# ---------------------------------------------------------------- GEMM paths
+def test_config0_smoke_all_paths(vla, oracle):
+    c = synth.config0()
+    packed = vla.pack_weights(dev(c["w"]))
+    for path in paths_for(vla, c["M"]) + [vla.VLA_PATH_AUTO]:
+        check_outputs(vla, oracle, packed, c["w"], c["beta"], c["x"], c["M"], c["N"], c["K"], path)
+
+
+@pytest.mark.parametrize("M", [1, 2, 3, 5, 8, 11, 16, 17, 32, 33, 100, 128, 129, 300])
+@pytest.mark.parametrize("N,K", [(128, 128), (384, 640), (640, 1152)])
+def test_small_shapes_ragged_m(vla, oracle, M, N, K):
+    """several tiles and ragged tails in every dimension the kernels tile (M, N/128, K/128)"""
+    w = synth.ternary_weights(N, K, 0.33, 7 * N + K)
+    x = synth.activations(M, K, 31 * M + K, dist="student_t3")
+    packed = vla.pack_weights(dev(w))
+    for path in paths_for(vla, M):
+        check_outputs(vla, oracle, packed, w, np.float32(0.037), x, M, N, K, path)
+
+
+@pytest.mark.parametrize("shape_idx", [0, 1, 2, 3])
+@pytest.mark.parametrize("M", [1, 8, 16])
+def test_config1_decode_points(vla, oracle, shape_idx, M):
+    c = synth.config1_point(shape_idx, M)
+    packed = vla.pack_weights(dev(c["w"]))
+    for path in paths_for(vla, M) + [vla.VLA_PATH_AUTO]:
+        check_outputs(vla, oracle, packed, c["w"], c["beta"], c["x"], M, c["N"], c["K"], path)
+
+
+@pytest.mark.parametrize("shape_idx", [0, 1, 2, 3])
+def test_config2_prefill_points_fused_linear(vla, oracle, shape_idx):
+    """configs[2]: M=544 with the quant fused into the call (vla_ternary_linear), fp32 output."""
+    c = synth.config2_point(shape_idx)
+    M, N, K = c["M"], c["N"], c["K"]
+    packed = vla.pack_weights(dev(c["w"]))
+    ref = check_outputs(vla, oracle, packed, c["w"], c["beta"], c["x"], M, N, K, vla.VLA_PATH_LARGE)
+    out = vla.empty_out(M, N, vla.VLA_F32)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    ws_bytes = vla.vla_ternary_workspace_bytes(M, N, K)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
+    beta_d = dev(np.array([c["beta"]], np.float32))
+    vla.vla_ternary_linear(packed, beta_d, dev_bf16(c["x"]), M, N, K, out, vla.VLA_F32, vla.VLA_PATH_AUTO,
+                           xq, xs, ws, ws_bytes)
+    torch.cuda.synchronize()
+    assert np.array_equal(xq.cpu().numpy(), ref["a"])
+    assert np.array_equal(out.cpu().numpy().view(np.uint32), ref["y32"].view(np.uint32))
+    # same call with the quantised activations kept in the workspace
+    out2 = vla.empty_out(M, N, vla.VLA_F32)
+    vla.vla_ternary_linear(packed, beta_d, dev_bf16(c["x"]), M, N, K, out2, vla.VLA_F32, vla.VLA_PATH_AUTO,
+                           None, None, ws, ws_bytes)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2)
+
+
+def test_sweep_shape_8192_sampled(vla, oracle):
+    """configs[4] largest shape at M=512: full int32 parity (the oracle needs ~34 G MACs: seconds on 8 cores)."""
+    c = synth.config4_point(512, 3, 1, 1)
+    M, N, K = 512, c["N"], c["K"]
+    packed = vla.pack_weights(dev(c["w"]))
+    a_ref, al_ref = oracle.act_quant(c["x"])
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(c["x"]), M, K, xq, xs)
+    assert np.array_equal(xq.cpu().numpy(), a_ref)
+    beta_d = dev(np.array([c["beta"]], np.float32))
+    acc = run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_I32, vla.VLA_PATH_LARGE).cpu().numpy()
+    # sampled rows of the output (every 37th token), each a full row of N dot products
+    rows = np.arange(0, M, 37)
+    ref = oracle.contract(a_ref[rows], c["w"])
+    assert np.array_equal(acc[rows], ref)
+
+
+# ---------------------------------------------------------------- invariants through the CUDA path
+@pytest.mark.parametrize("M", [8, 64])
+def test_unit_vector_activations_return_w_columns(vla, M):
+    """x_m = c * e_j  ->  acc_mn = 127 * w_nj exactly: catches any K permutation in the packed layout."""
+    N, K = 256, 512
+    w = synth.ternary_weights(N, K, 0.3, 77)
+    packed = vla.pack_weights(dev(w))
+    rng = np.random.default_rng(3)
+    js = rng.choice(K, size=M, replace=False)
+    x = np.zeros((M, K), np.float32)
+    x[np.arange(M), js] = rng.uniform(0.5, 3.0, M).astype(np.float32)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(synth._f32_to_bf16_bits(x)), M, K, xq, xs)
+    beta_d = dev(np.array([1.0], np.float32))
+    for path in paths_for(vla, M):
+        acc = run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_I32, path).cpu().numpy()
+        assert np.array_equal(acc, 127 * w[:, js].T.astype(np.int32))
+
+
+def test_all_ones_weights_return_row_sums(vla):
+    M, N, K = 16, 256, 640
+    for val in (1, -1, 0):
+        w = np.full((N, K), val, np.int8)
+        packed = vla.pack_weights(dev(w))
+        x_bits = synth.activations(M, K, 11)
+        xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+        xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+        vla.vla_act_quant(dev_bf16(x_bits), M, K, xq, xs)
+        rows = xq.cpu().numpy().astype(np.int64).sum(axis=1) * val
+        beta_d = dev(np.array([1.0], np.float32))
+        for path in paths_for(vla, M):
+            acc = run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_I32, path).cpu().numpy()
+            assert np.array_equal(acc, np.repeat(rows[:, None], N, axis=1))
+
+
+def test_extreme_accumulators(vla):
+    """|acc| reaches 127*K: all activations saturate at +-127 and W = sign pattern (K = 8192, the sweep's max)."""
+    M, N, K = 4, 128, 8192
+    x = np.ones((M, K), np.float32)
+    x[1] = -1.0
+    x[2, ::2] = -1.0
+    w = np.ones((N, K), np.int8)
+    w[1::2] = -1
+    packed = vla.pack_weights(dev(w))
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(synth._f32_to_bf16_bits(x)), M, K, xq, xs)
+    want = xq.cpu().numpy().astype(np.int64) @ w.T.astype(np.int64)
+    assert np.abs(want).max() == 127 * K
+    beta_d = dev(np.array([1.0], np.float32))
+    for path in paths_for(vla, M):
+        acc = run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_I32, path).cpu().numpy()
+        assert np.array_equal(acc, want)
+
+
+# ---------------------------------------------------------------- host-buffer entry point + errors on a GPU
+def test_linear_host_round_trip(vla, oracle):
+    c = synth.config1_point(1, 8)
+    M, N, K = c["M"], c["N"], c["K"]
+    packed = vla.pack_weights(dev(c["w"]))
+    ref = oracle.ternary_linear(c["x"], c["w"], c["beta"])
+    xh = torch.from_numpy(c["x"].view(np.int16)).view(torch.bfloat16).pin_memory()
+    oh = torch.empty((M, N), dtype=torch.bfloat16).pin_memory()
+    nb = vla.vla_ternary_host_workspace_bytes(M, N, K, vla.VLA_BF16)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    beta_d = dev(np.array([c["beta"]], np.float32))
+    vla.vla_ternary_linear_host(packed, beta_d, xh, M, N, K, oh, vla.VLA_BF16, vla.VLA_PATH_AUTO, ws, nb)
+    assert np.array_equal(oh.view(torch.int16).numpy().view(np.uint16), ref["ybf16"])
+
+
+def test_errors_on_device(vla):
+    w = dev(synth.ternary_weights(128, 128, 0.3, 1))
+    packed = vla.pack_weights(w)
+    out = vla.empty_out(8, 128, vla.VLA_F32)
+    xq = torch.zeros((8, 128), dtype=torch.int8, device="cuda")
+    xs = torch.ones((8,), dtype=torch.float32, device="cuda")
+    beta = torch.ones((1,), dtype=torch.float32, device="cuda")
+    with pytest.raises(vla.VlaError) as e:
+        vla.vla_ternary_gemm(packed, beta, xq, xs, 64, 128, 128, out, vla.VLA_F32, vla.VLA_PATH_SMALL_ALU)
+    assert e.value.status == vla.VLA_ERR_SHAPE
+    with pytest.raises(vla.VlaError) as e:
+        vla.vla_ternary_gemm(packed, beta, xq.data_ptr() + 1, xs, 8, 128, 128, out, vla.VLA_F32)
+    assert e.value.status == vla.VLA_ERR_ALIGN
+    launches = vla.vla_launch_count()
+    vla.vla_ternary_gemm(packed, beta, xq, xs, 8, 128, 128, out, vla.VLA_F32)
+    torch.cuda.synchronize()
+    assert vla.vla_launch_count() > launches
+    assert torch.all(out == 0)
+
+
+def test_library_is_the_loaded_native_code(vla):
+    """the in-tree .so is what the process mapped (no silent eager fallback exists)"""
+    maps = open("/proc/self/maps").read()
+    assert os.path.basename(vla.LIB_PATH) in maps
