@@ -116,6 +116,60 @@ vla_status vla_ternary_linear_host(const void* packed, const float* w_scale, con
                                    int M, int N, int K, void* out_host, vla_dtype out_dtype, vla_path path,
                                    void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---------------------------------------------------------------------------------------------------
+ * Programs: a whole list of small-M ternary linears in ONE persistent launch.
+ *
+ * "graphs and buffers persist across same-shape requests ... GPU graph capture" removes
+ * dispatch overhead.  On B200 one launch costs more than ten times the HBM time of a BitNet-2B weight
+ * tensor, so the library goes one step further: a program is compiled once and then executed by a single
+ * persistent kernel (csrc/gemm_program.cu) that streams the packed weights of every stage back to back
+ * and synchronises only where a stage reads what an earlier stage wrote.
+ *
+ * A STAGE is one activation matrix x [M,K] bf16 (1 <= M <= 16, K % 128 == 0, K <= 8192) and n_linears
+ * (1..16) ternary linears that all consume it, each with its own packed W [N,K], scale beta and output:
+ * the per-output-group scales beta_g(n) of Eq. 4, e.g. q|k|v or gate|up.
+ * Every stage runs Eq. 4 end to end: absmax int8 quant of x, int32 contraction, dequant to out_dtype.
+ *   depends = 0   x is written before the launch (quantised up front)
+ *   depends = 1   x is (part of) the output of EARLIER stages of this program: the stage starts only
+ *                 after every earlier stage has completed on the whole grid
+ * All pointers inside the descriptors are DEVICE pointers, 16-byte aligned, and must stay valid for as
+ * long as the program is run.  The descriptor arrays themselves are HOST memory.
+ */
+typedef struct {
+    const void* packed;     /* from vla_ternary_pack for (N, K of the stage) */
+    const float* w_scale;   /* device pointer to one fp32 (beta) */
+    void* out;              /* [M,N] of out_dtype */
+    int N;                  /* N % 128 == 0 */
+    int out_dtype;          /* vla_dtype */
+} vla_prog_linear;
+
+typedef struct {
+    const void* x_bf16;     /* [M,K] bf16 */
+    int M, K;
+    int depends;            /* 0 or 1, see above */
+    int n_linears;
+    const vla_prog_linear* linears;   /* HOST array of n_linears entries */
+    int8_t* xq_opt;         /* optional: also return the quantised activations [M,K] int8 (NULL: kept inside the program) */
+    float* x_scale_opt;     /* optional: alpha [M] fp32 */
+} vla_prog_stage;
+
+/* Device bytes a compiled program needs (descriptor tables, barrier counters, quantised activations);
+ * a multiple of 256.  0 if any stage is invalid. */
+size_t vla_program_bytes(const vla_prog_stage* stages /*host*/, int n_stages);
+
+/* Compiles `stages` into prog_dev (device memory, >= vla_program_bytes, 256-byte aligned).
+ * SYNCHRONISES `stream`.  VLA_ERR_SHAPE / _NULL / _ALIGN / _DTYPE as for the single calls. */
+vla_status vla_program_build(const vla_prog_stage* stages /*host*/, int n_stages, void* prog_dev, size_t prog_bytes,
+                             void* stream);
+
+/* Runs a compiled program: ONE kernel launch, asynchronous on `stream`, capturable in a CUDA graph.
+ * Returns VLA_ERR_VALUE if prog_dev was not produced by vla_program_build in this process.
+ * Runs of the same program must not overlap in time (they share its counters and activations). */
+vla_status vla_program_run(const void* prog_dev, void* stream);
+
+/* Forgets a compiled program (the caller then frees prog_dev). */
+vla_status vla_program_release(const void* prog_dev);
+
 /* The path VLA_PATH_AUTO resolves to for (M,N,K). */
 vla_path vla_ternary_auto_path(int M, int N, int K);
 

@@ -26,7 +26,19 @@ EXPORTS = [
     "vla_act_quant", "vla_ternary_gemm", "vla_ternary_linear", "vla_ternary_linear_host",
     "vla_ternary_host_workspace_bytes",
     "vla_ternary_auto_path", "vla_i8_mma_issue_probe", "vla_status_string", "vla_launch_count",
+    "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_release",
 ]
+
+
+class vla_prog_linear(ctypes.Structure):
+    _fields_ = [("packed", ctypes.c_void_p), ("w_scale", ctypes.c_void_p), ("out", ctypes.c_void_p),
+                ("N", ctypes.c_int), ("out_dtype", ctypes.c_int)]
+
+
+class vla_prog_stage(ctypes.Structure):
+    _fields_ = [("x_bf16", ctypes.c_void_p), ("M", ctypes.c_int), ("K", ctypes.c_int), ("depends", ctypes.c_int),
+                ("n_linears", ctypes.c_int), ("linears", ctypes.POINTER(vla_prog_linear)),
+                ("xq_opt", ctypes.c_void_p), ("x_scale_opt", ctypes.c_void_p)]
 
 
 class VlaError(RuntimeError):
@@ -67,6 +79,15 @@ def _load():
     lib.vla_status_string.argtypes = [st]
     lib.vla_launch_count.restype = ctypes.c_ulonglong
     lib.vla_launch_count.argtypes = []
+    ps = ctypes.POINTER(vla_prog_stage)
+    lib.vla_program_bytes.restype = sz
+    lib.vla_program_bytes.argtypes = [ps, i]
+    lib.vla_program_build.restype = st
+    lib.vla_program_build.argtypes = [ps, i, vp, sz, vp]
+    lib.vla_program_run.restype = st
+    lib.vla_program_run.argtypes = [vp, vp]
+    lib.vla_program_release.restype = st
+    lib.vla_program_release.argtypes = [vp]
     return lib
 
 
@@ -162,7 +183,57 @@ def vla_i8_mma_issue_probe(ctas, mmas_per_cta):
     return float(ms.value)
 
 
+def _marshal_stages(stages):
+    """stages: list of dicts {x, M, K, depends, linears: [{packed, w_scale, out, N, out_dtype}], xq_opt, x_scale_opt}
+    -> (ctypes array of vla_prog_stage, keep-alive list)."""
+    arr = (vla_prog_stage * len(stages))()
+    keep = []
+    for si, sd in enumerate(stages):
+        lins = (vla_prog_linear * len(sd["linears"]))()
+        for li, ld in enumerate(sd["linears"]):
+            lins[li] = vla_prog_linear(_ptr(ld["packed"]), _ptr(ld["w_scale"]), _ptr(ld["out"]), int(ld["N"]),
+                                       int(ld["out_dtype"]))
+        keep.append(lins)
+        arr[si] = vla_prog_stage(_ptr(sd["x"]), int(sd["M"]), int(sd["K"]), int(sd.get("depends", 0)), len(lins), lins,
+                                 _ptr(sd.get("xq_opt")), _ptr(sd.get("x_scale_opt")))
+    return arr, keep
+
+
+def vla_program_bytes(stages):
+    arr, _keep = _marshal_stages(stages)
+    return int(_lib.vla_program_bytes(arr, len(stages)))
+
+
+def vla_program_build(stages, prog_dev, prog_bytes=None, stream=None):
+    arr, _keep = _marshal_stages(stages)
+    if prog_bytes is None:
+        prog_bytes = prog_dev.numel() * prog_dev.element_size()
+    _check(_lib.vla_program_build(arr, len(stages), _ptr(prog_dev), prog_bytes, _stream(stream)), "vla_program_build")
+
+
+def vla_program_run(prog_dev, stream=None):
+    _check(_lib.vla_program_run(_ptr(prog_dev), _stream(stream)), "vla_program_run")
+
+
+def vla_program_release(prog_dev):
+    _check(_lib.vla_program_release(_ptr(prog_dev)), "vla_program_release")
+
+
 # ------------------------------------------------------------------ conveniences (allocation only)
+def compile_program(stages, device="cuda"):
+    """Allocates the device buffer of a program and compiles `stages` into it; returns the buffer (a uint8 tensor
+    that must be kept alive, together with every tensor the stages point to, while the program is run)."""
+    nbytes = vla_program_bytes(stages)
+    if nbytes == 0:
+        raise VlaError(VLA_ERR_SHAPE, "compile_program")
+    buf = torch.zeros(nbytes + 256, dtype=torch.uint8, device=device)
+    off = (-buf.data_ptr()) % 256
+    prog = buf[off:off + nbytes]
+    vla_program_build(stages, prog, nbytes)
+    prog._vla_keep = buf
+    return prog
+
+
 def pack_weights(w_i8):
     """int8 [N,K] CUDA tensor -> uint8 packed tensor of vla_ternary_packed_bytes(N,K) bytes."""
     N, K = w_i8.shape

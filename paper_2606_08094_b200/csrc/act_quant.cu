@@ -6,37 +6,13 @@
 // over HBM.  Rows longer than the register window are re-read (they hit L1/L2).
 #include <cuda_bf16.h>
 #include "common.cuh"
+#include "quant.cuh"
 #include "kernels.h"
 
 namespace vla {
 
 constexpr int AQ_THREADS = 256;
 constexpr int AQ_VEC_PER_THREAD = 4;                    // 4 x 8 bf16 per thread in registers -> K <= 8192
-
-__device__ __forceinline__ float bf16lo(uint32_t u) { return __uint_as_float(u << 16); }
-__device__ __forceinline__ float bf16hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
-
-__device__ __forceinline__ float absmax8(uint4 v, float m) {
-    m = fmaxf(m, fabsf(bf16lo(v.x))); m = fmaxf(m, fabsf(bf16hi(v.x)));
-    m = fmaxf(m, fabsf(bf16lo(v.y))); m = fmaxf(m, fabsf(bf16hi(v.y)));
-    m = fmaxf(m, fabsf(bf16lo(v.z))); m = fmaxf(m, fabsf(bf16hi(v.z)));
-    m = fmaxf(m, fabsf(bf16lo(v.w))); m = fmaxf(m, fabsf(bf16hi(v.w)));
-    return m;
-}
-
-__device__ __forceinline__ uint32_t q1(float x, float alpha) {
-    float t = __fdiv_rn(x, alpha);
-    int r = __float2int_rn(t);                           // round-half-to-even
-    r = max(-127, min(127, r));
-    return (uint32_t)r & 0xFFu;
-}
-
-__device__ __forceinline__ uint2 quant8(uint4 v, float alpha) {
-    uint2 o;
-    o.x = q1(bf16lo(v.x), alpha) | (q1(bf16hi(v.x), alpha) << 8) | (q1(bf16lo(v.y), alpha) << 16) | (q1(bf16hi(v.y), alpha) << 24);
-    o.y = q1(bf16lo(v.z), alpha) | (q1(bf16hi(v.z), alpha) << 8) | (q1(bf16lo(v.w), alpha) << 16) | (q1(bf16hi(v.w), alpha) << 24);
-    return o;
-}
 
 __global__ void __launch_bounds__(AQ_THREADS) act_quant_kernel(const uint4* __restrict__ x, int K,
                                                                uint2* __restrict__ xq, float* __restrict__ x_scale) {
@@ -66,7 +42,7 @@ __global__ void __launch_bounds__(AQ_THREADS) act_quant_kernel(const uint4* __re
 #pragma unroll
     for (int i = 1; i < AQ_THREADS / 32; ++i) m = fmaxf(m, s_max[i]);
 
-    const float alpha = __fdiv_rn(fmaxf(m, 1e-5f), 127.0f);
+    const float alpha = alpha_of(m);
     if (threadIdx.x == 0) x_scale[row] = alpha;
     pdl_launch_dependents();
 #pragma unroll

@@ -66,7 +66,7 @@ const char* vla_status_string(vla_status s) {
         case VLA_ERR_NULL: return "VLA_ERR_NULL: a required pointer is NULL";
         case VLA_ERR_SHAPE: return "VLA_ERR_SHAPE: need M>=1, N%128==0, K%128==0, K<=65536, and M within the forced path's range";
         case VLA_ERR_ALIGN: return "VLA_ERR_ALIGN: pointers must be 16-byte aligned";
-        case VLA_ERR_VALUE: return "VLA_ERR_VALUE: weight element outside {-1,0,+1}";
+        case VLA_ERR_VALUE: return "VLA_ERR_VALUE: weight element outside {-1,0,+1}, or not a compiled program";
         case VLA_ERR_DTYPE: return "VLA_ERR_DTYPE: unknown vla_dtype or vla_path";
         case VLA_ERR_WORKSPACE: return "VLA_ERR_WORKSPACE: workspace missing or too small";
         case VLA_ERR_ARCH: return "VLA_ERR_ARCH: current device is not sm_100 (no fallback path exists)";

@@ -1,0 +1,164 @@
+// api_program.cu -- host side of the program API of include/vla_ternary.h: validation, compilation of the
+// descriptor tables into device memory, and the single launch.  Nothing here computes.
+#include "../../include/vla_ternary.h"
+#include <cstring>
+#include <mutex>
+#include <unordered_map>
+#include <vector>
+#include "kernels.h"
+#include "program.h"
+
+namespace {
+
+using vla::DevLin;
+using vla::DevProg;
+using vla::DevStage;
+
+struct ProgInfo { int grid; int n_stages; };
+std::mutex g_mu;
+std::unordered_map<const void*, ProgInfo> g_programs;
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline size_t round256(size_t b) { return (b + 255) / 256 * 256; }
+
+vla_status check_stages(const vla_prog_stage* st, int n) {
+    if (!st) return VLA_ERR_NULL;
+    if (n < 1 || n > 4096) return VLA_ERR_SHAPE;
+    for (int s = 0; s < n; ++s) {
+        const vla_prog_stage& a = st[s];
+        if (!a.x_bf16 || !a.linears) return VLA_ERR_NULL;
+        if (a.M < 1 || a.M > 16 || a.K < 128 || a.K % 128 != 0 || a.K > 8192) return VLA_ERR_SHAPE;
+        if (a.n_linears < 1 || a.n_linears > 16) return VLA_ERR_SHAPE;
+        if (a.depends != 0 && a.depends != 1) return VLA_ERR_SHAPE;
+        if (!aligned16(a.x_bf16) || (a.xq_opt && !aligned16(a.xq_opt)) || (a.x_scale_opt && !aligned16(a.x_scale_opt)))
+            return VLA_ERR_ALIGN;
+        for (int j = 0; j < a.n_linears; ++j) {
+            const vla_prog_linear& l = a.linears[j];
+            if (l.out_dtype < 0 || l.out_dtype > 2) return VLA_ERR_DTYPE;
+            if (!l.packed || !l.out || (l.out_dtype != VLA_I32 && !l.w_scale)) return VLA_ERR_NULL;
+            if (l.N < 128 || l.N % 128 != 0) return VLA_ERR_SHAPE;
+            if (!aligned16(l.packed) || !aligned16(l.out) || (reinterpret_cast<uintptr_t>(l.w_scale) & 3u)) return VLA_ERR_ALIGN;
+        }
+    }
+    return VLA_OK;
+}
+
+struct Layout {
+    size_t off_stages, off_lins, off_counters, off_act, total;
+    int n_lin;
+};
+
+Layout layout_of(const vla_prog_stage* st, int n) {
+    Layout L{};
+    L.n_lin = 0;
+    for (int s = 0; s < n; ++s) L.n_lin += st[s].n_linears;
+    size_t o = round256(sizeof(DevProg));
+    L.off_stages = o;   o += round256(sizeof(DevStage) * (size_t)n);
+    L.off_lins = o;     o += round256(sizeof(DevLin) * (size_t)L.n_lin);
+    L.off_counters = o; o += round256(sizeof(unsigned) * (2 * (size_t)n + 1));
+    L.off_act = o;
+    for (int s = 0; s < n; ++s) o += round256((size_t)st[s].M * st[s].K) + 256;      // int8 [M,K] + alpha [M]
+    L.total = o;
+    return L;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t vla_program_bytes(const vla_prog_stage* stages, int n_stages) {
+    if (check_stages(stages, n_stages) != VLA_OK) return 0;
+    return layout_of(stages, n_stages).total;
+}
+
+vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* prog_dev, size_t prog_bytes, void* stream) {
+    vla_status st = check_stages(stages, n_stages);
+    if (st != VLA_OK) return st;
+    if (!prog_dev) return VLA_ERR_NULL;
+    if (reinterpret_cast<uintptr_t>(prog_dev) & 255u) return VLA_ERR_ALIGN;
+    const Layout L = layout_of(stages, n_stages);
+    if (prog_bytes < L.total) return VLA_ERR_WORKSPACE;
+    int dev = 0, sms = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return VLA_ERR_ARCH;
+    }
+    if (major != 10) return VLA_ERR_ARCH;
+
+    uint8_t* base = reinterpret_cast<uint8_t*>(prog_dev);
+    std::vector<uint8_t> host(L.off_act, 0);
+    DevProg* P = reinterpret_cast<DevProg*>(host.data());
+    DevStage* S = reinterpret_cast<DevStage*>(host.data() + L.off_stages);
+    DevLin* Q = reinterpret_cast<DevLin*>(host.data() + L.off_lins);
+    P->magic = vla::PROG_MAGIC;
+    P->n_stages = n_stages;
+    P->n_lin = L.n_lin;
+    P->b1 = reinterpret_cast<unsigned*>(base + L.off_counters);
+    P->b2 = P->b1 + n_stages;
+    P->done = P->b2 + n_stages;
+    P->stages = reinterpret_cast<const DevStage*>(base + L.off_stages);
+    P->lins = reinterpret_cast<const DevLin*>(base + L.off_lins);
+    size_t act = L.off_act;
+    int li = 0, max_gran = 0;
+    for (int s = 0; s < n_stages; ++s) {
+        const vla_prog_stage& a = stages[s];
+        DevStage& d = S[s];
+        d.x = reinterpret_cast<const uint4*>(a.x_bf16);
+        const size_t qbytes = round256((size_t)a.M * a.K);
+        d.xq = reinterpret_cast<uint2*>(a.xq_opt ? (void*)a.xq_opt : (void*)(base + act));
+        d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + act + qbytes);
+        act += qbytes + 256;
+        d.M = a.M;
+        d.K = a.K;
+        d.depends = a.depends;
+        d.lin_begin = li;
+        d.n_lin = a.n_linears;
+        int gran = 0;
+        for (int j = 0; j < a.n_linears; ++j, ++li) {
+            const vla_prog_linear& l = a.linears[j];
+            Q[li].packed = reinterpret_cast<const uint8_t*>(l.packed);
+            Q[li].beta = l.w_scale;
+            Q[li].out = l.out;
+            Q[li].N = l.N;
+            Q[li].dtype = l.out_dtype;
+            Q[li].gran_begin = gran;
+            Q[li].pad = 0;
+            gran += l.N / 32;
+        }
+        d.granules = gran;
+        if (gran > max_gran) max_gran = gran;
+    }
+    int grid = max_gran < sms ? max_gran : sms;
+    if (grid < 16 && sms >= 16) grid = 16;                  // enough CTAs to own one activation row each
+
+    cudaStream_t cs = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(prog_dev, host.data(), host.size(), cudaMemcpyHostToDevice, cs);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
+    if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_programs[prog_dev] = ProgInfo{grid, n_stages};
+    return VLA_OK;
+}
+
+vla_status vla_program_run(const void* prog_dev, void* stream) {
+    if (!prog_dev) return VLA_ERR_NULL;
+    ProgInfo info;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        auto it = g_programs.find(prog_dev);
+        if (it == g_programs.end()) return VLA_ERR_VALUE;
+        info = it->second;
+    }
+    cudaError_t e = vla::launch_program(prog_dev, info.grid, (cudaStream_t)stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+    return VLA_OK;
+}
+
+vla_status vla_program_release(const void* prog_dev) {
+    if (!prog_dev) return VLA_ERR_NULL;
+    std::lock_guard<std::mutex> lk(g_mu);
+    return g_programs.erase(prog_dev) ? VLA_OK : VLA_ERR_VALUE;
+}
+
+}  // extern "C"

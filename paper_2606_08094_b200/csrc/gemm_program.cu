@@ -1,0 +1,299 @@
+// gemm_program.cu -- persistent "program" kernel for the small-M (M <= 16) regime: ONE launch runs a whole list
+// of ternary linears (Eq. 4), independent or chained, e.g. the 30-layer stack of
+// BASELINE.json configs[3].  PAPER.md line 56 removes dispatch overhead by persisting graphs; on B200 a launch
+// costs ~5000 cycles, more than ten times the HBM time of a 1.6 MB weight tensor, so the whole program is one
+// kernel and the only thing that ever waits is data.
+//
+// Grid: one CTA per SM, 17 warps.
+//   warp 16 (producer)   streams this CTA's share of the packed weights of EVERY stage, in program order, through
+//                        a 12 x 16 KiB shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
+//                        activations, so HBM stays busy across stage boundaries and grid barriers.
+//   warps 0-15 (consumers) per stage: hold the int8 activations as mma.m16n8k32 B fragments IN REGISTERS (warp w
+//                        owns the 64-wide k blocks kq = w mod 16), read packed words from the ring, decode them
+//                        in registers (2 ALU ops per 4 weights, common.cuh) into A fragments, accumulate int32,
+//                        reduce the 16 partial sums per output through shared memory, and run the dequant
+//                        epilogue  y = (float)acc * (alpha_m * beta).
+// Work unit: a GRANULE = 32 output channels x all of K of one linear (K/128 contiguous 1 KiB pieces of the packed
+// layout); granule gi of a stage goes to CTA gi mod gridDim.x.
+// Activation quant (Eq. 4 lines 1-2): row r of stage s is quantised by ONE owner CTA (absmax over the row, then
+// the true-division quantiser of quant.cuh) into global int8 + alpha; counters in global memory order the phases:
+//   b1[s] = CTAs that finished stage s   (a dependent stage's row owners wait for b1[s-1] == gridDim.x)
+//   b2[s] = rows of stage s quantised    (every CTA waits for b2[s] == M_s before it loads its B fragments)
+// Stages that do not depend on earlier ones are quantised up front.  int32 sums are exact in any order, so the
+// result is bit-identical to the per-call kernels and to the oracle.
+#include <cuda_bf16.h>
+#include "common.cuh"
+#include "kernels.h"
+#include "program.h"
+#include "quant.cuh"
+
+namespace vla {
+
+constexpr int PG_W = 16;                         // consumer warps
+constexpr int PG_CONSUMERS = PG_W * 32;          // 512 threads
+constexpr int PG_THREADS = PG_CONSUMERS + 32;
+constexpr int PG_SLOT_BYTES = 16384;             // 16 pieces of 1 KiB = 32 blocks of 32 ch x 64 k
+constexpr int PG_NSLOT = 12;
+constexpr int PG_NBMAX = 8;                      // k blocks per warp per granule  ->  K <= 8192
+constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 8448 ints = 33 792 B
+constexpr int PG_SMEM = PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + 2 * PG_NSLOT * 8 + 64 + 128;
+
+__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(PG_CONSUMERS) : "memory"); }
+
+__device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void spin_until(const unsigned* p, unsigned target) {
+    while (ld_acquire_gpu(p) < target) { }
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 r;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr) : "memory");
+    return r;
+}
+
+__device__ __forceinline__ int owner_of(int s, int r, int G) { return G - 1 - ((s * 16 + r) % G); }
+
+// ---------------------------------------------------------------- producer warp
+__device__ __forceinline__ void producer(const DevProg& P, int cta, int G, int lane, uint32_t ring, uint32_t bar_full,
+                                         uint32_t bar_empty) {
+    uint32_t slot = 0, round = 0;
+    for (int s = 0; s < P.n_stages; ++s) {
+        const DevStage st = P.stages[s];
+        const int KB = st.K / TILE_K;                       // 1 KiB pieces per granule
+        for (int gi = cta; gi < st.granules; gi += G) {
+            int l = st.lin_begin;
+            for (int j = 1; j < st.n_lin; ++j)
+                if (gi >= P.lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
+            const int n32 = gi - P.lins[l].gran_begin;
+            const uint8_t* src = P.lins[l].packed + ((size_t)(n32 >> 2) * KB * 8 + (size_t)(n32 & 3) * 2) * 512;
+            for (int p0 = 0; p0 < KB; p0 += 16) {
+                const int np = min(16, KB - p0);
+                if (round > 0) mbar_wait(bar_empty + 8u * slot, (round - 1) & 1);
+                if (lane == 0) mbar_arrive_expect_tx(bar_full + 8u * slot, (uint32_t)np * 1024u);
+                __syncwarp();
+                if (lane < np)
+                    tma_bulk_g2s(ring + slot * PG_SLOT_BYTES + lane * 1024, src + (size_t)(p0 + lane) * TILE_BYTES, 1024,
+                                 bar_full + 8u * slot);
+                if (++slot == PG_NSLOT) { slot = 0; ++round; }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- row-owner activation quant (Eq. 4 lines 1-2)
+// All 512 consumer threads of the owner CTA quantise row r of stage st: one pass, the row lives in registers.
+__device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, float* s_max) {
+    const int nvec = st.K / 8;                               // uint4 of 8 bf16; K <= 8192 -> nvec <= 1024
+    const uint4* xr = st.x + (size_t)r * nvec;
+    const uint4 z = make_uint4(0, 0, 0, 0);
+    const uint4 v0 = (tid < nvec) ? __ldcg(xr + tid) : z;
+    const uint4 v1 = (tid + PG_CONSUMERS < nvec) ? __ldcg(xr + tid + PG_CONSUMERS) : z;
+    float m = absmax8(v1, absmax8(v0, 0.0f));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+    if ((tid & 31) == 0) s_max[tid >> 5] = m;
+    consumer_bar();
+    m = s_max[0];
+#pragma unroll
+    for (int i = 1; i < PG_W; ++i) m = fmaxf(m, s_max[i]);
+    const float alpha = alpha_of(m);
+    if (tid == 0) st.xs[r] = alpha;
+    uint2* qr = st.xq + (size_t)r * nvec;
+    if (tid < nvec) qr[tid] = quant8(v0, alpha);
+    if (tid + PG_CONSUMERS < nvec) qr[tid + PG_CONSUMERS] = quant8(v1, alpha);
+    consumer_bar();                                          // s_max may be reused; stores precede thread 0's fence
+}
+
+__device__ __forceinline__ void quant_owned_rows(const DevProg& P, int s, const DevStage& st, int cta, int G, int tid,
+                                                 float* s_max) {
+    int owned = 0;
+    for (int r = 0; r < st.M; ++r) owned += (owner_of(s, r, G) == cta);
+    if (owned == 0) return;
+    if (st.depends && s > 0) {
+        if (tid == 0) spin_until(P.b1 + (s - 1), (unsigned)G);
+        consumer_bar();
+    }
+    for (int r = 0; r < st.M; ++r)
+        if (owner_of(s, r, G) == cta) quant_row(st, r, tid, s_max);
+    if (tid == 0) {
+        __threadfence();
+        atomicAdd(P.b2 + s, (unsigned)owned);
+    }
+}
+
+// ---------------------------------------------------------------- one stage's granules on the consumer warps
+template <int MT>
+__device__ __forceinline__ void stage_gemm(const DevProg& P, const DevStage& st, int cta, int G, int tid, uint32_t ring,
+                                           int* red, uint32_t bar_full, uint32_t bar_empty, uint32_t& slot,
+                                           uint32_t& phase, uint32_t& gcount) {
+    constexpr int MTOK = MT * 8;
+    const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int K = st.K, M = st.M, nblk = K / BLK_K, KB = K / TILE_K;
+    const int nchunks = (KB + 15) >> 4;
+
+    // int8 activations of this warp's k blocks, as B fragments, in registers for the whole stage
+    uint4 xv[PG_NBMAX][MT];
+    const int8_t* xq = reinterpret_cast<const int8_t*>(st.xq);
+#pragma unroll
+    for (int i = 0; i < PG_NBMAX; ++i)
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            const int kq = i * PG_W + w, tok = mt * 8 + g;
+            xv[i][mt] = (kq < nblk && tok < M)
+                            ? __ldcg(reinterpret_cast<const uint4*>(xq + (size_t)tok * K + kq * BLK_K + t * 16))
+                            : make_uint4(0, 0, 0, 0);
+        }
+    const int etok = tid >> 5, ech = tid & 31;               // epilogue role: one output per thread
+    const bool eactive = (etok < M) && (etok < MTOK);
+    const float alpha = eactive ? __ldcg(st.xs + etok) : 0.0f;
+    const uint32_t my_off = (uint32_t)((w >> 1) * 1024 + (w & 1) * 512 + lane * 16);
+
+    for (int gi = cta; gi < st.granules; gi += G) {
+        int l = st.lin_begin;
+        for (int j = 1; j < st.n_lin; ++j)
+            if (gi >= P.lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
+        const DevLin L = P.lins[l];
+        const int n32 = gi - L.gran_begin;
+
+        int acc[2][MT][4];
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) acc[c][mt][i] = 0;
+
+#pragma unroll
+        for (int ck = 0; ck < PG_NBMAX / 2; ++ck) {
+            if (ck < nchunks) {
+                mbar_wait(bar_full + 8u * slot, phase);
+#pragma unroll
+                for (int ii = 0; ii < 2; ++ii) {
+                    const int i = 2 * ck + ii;
+                    if (i * PG_W + w < nblk) {
+                        const uint4 wv = lds128(ring + slot * PG_SLOT_BYTES + ii * 8192 + my_off);
+                        const uint32_t w4[4] = {wv.x, wv.y, wv.z, wv.w};
+#pragma unroll
+                        for (int c = 0; c < 2; ++c) {
+                            const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];     // channels 16c+g and 16c+g+8
+                            const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
+                            const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
+#pragma unroll
+                            for (int mt = 0; mt < MT; ++mt) {
+                                mma_m16n8k32_s8(acc[c][mt], a0, a1, a2, a3, xv[i][mt].x, xv[i][mt].y);
+                                mma_m16n8k32_s8(acc[c][mt], e0, e1, e2, e3, xv[i][mt].z, xv[i][mt].w);
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty + 8u * slot);
+                if (++slot == PG_NSLOT) { slot = 0; phase ^= 1; }
+            }
+        }
+
+        // 16 per-warp partial sums -> shared memory -> one thread per output
+        int* rb = red + ((MT == 1) ? (int)(gcount & 1) * (PG_W * 8 * 33) : 0);
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                int* row0 = rb + (w * MTOK + mt * 8 + 2 * t) * 33 + 16 * c + g;
+                row0[0] = acc[c][mt][0];
+                row0[33] = acc[c][mt][1];
+                row0[8] = acc[c][mt][2];
+                row0[33 + 8] = acc[c][mt][3];
+            }
+        consumer_bar();
+        if (eactive) {
+            int sum = 0;
+#pragma unroll
+            for (int ww = 0; ww < PG_W; ++ww) sum += rb[(ww * MTOK + etok) * 33 + ech];
+            const int a = sum >> 6;                           // the decode's factor 64 leaves exactly
+            const size_t o = (size_t)etok * L.N + (size_t)n32 * BLK_N + ech;
+            if (L.dtype == 2) {
+                reinterpret_cast<int*>(L.out)[o] = a;
+            } else {
+                const float y = dequant(a, __fmul_rn(alpha, __ldcg(L.beta)));
+                if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
+                else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
+            }
+        }
+        if (MT == 2) consumer_bar();                          // single reduction buffer: wait for the readers
+        ++gcount;
+    }
+}
+
+// ---------------------------------------------------------------- the kernel
+__global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* __restrict__ prog) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
+    uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
+    const uint32_t ring = base;
+    int* red = reinterpret_cast<int*>(base_ptr + PG_NSLOT * PG_SLOT_BYTES);
+    const uint32_t bar_full = base + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4;
+    const uint32_t bar_empty = bar_full + 8u * PG_NSLOT;
+    float* s_max = reinterpret_cast<float*>(base_ptr + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + 16 * PG_NSLOT);
+
+    const int tid = threadIdx.x, cta = blockIdx.x, G = gridDim.x;
+    if (tid == 0) {
+        for (int s = 0; s < PG_NSLOT; ++s) {
+            mbar_init(bar_full + 8u * s, 1);
+            mbar_init(bar_empty + 8u * s, PG_W);
+        }
+        fence_barrier_init();
+    }
+    __syncthreads();
+    const DevProg P = *prog;
+
+    if (tid >= PG_CONSUMERS) {
+        producer(P, cta, G, tid & 31, ring, bar_full, bar_empty);
+        return;
+    }
+
+    // stages whose input comes from outside the program: quantise up front
+    for (int s = 0; s < P.n_stages; ++s) {
+        const DevStage st = P.stages[s];
+        if (!st.depends || s == 0) quant_owned_rows(P, s, st, cta, G, tid, s_max);
+    }
+    uint32_t slot = 0, phase = 0, gcount = 0;
+    for (int s = 0; s < P.n_stages; ++s) {
+        const DevStage st = P.stages[s];
+        if (st.depends && s > 0) quant_owned_rows(P, s, st, cta, G, tid, s_max);
+        if (tid == 0) spin_until(P.b2 + s, (unsigned)st.M);
+        consumer_bar();
+        if (st.M <= 8) stage_gemm<1>(P, st, cta, G, tid, ring, red, bar_full, bar_empty, slot, phase, gcount);
+        else           stage_gemm<2>(P, st, cta, G, tid, ring, red, bar_full, bar_empty, slot, phase, gcount);
+        consumer_bar();                                      // every output store of this CTA precedes the fence
+        if (tid == 0) {
+            __threadfence();
+            atomicAdd(P.b1 + s, 1u);
+        }
+    }
+    // the last CTA to finish re-zeroes the counters, so the next launch of the same program needs no memset
+    if (tid == 0) {
+        const unsigned prev = atomicAdd(P.done, 1u);
+        if (prev == (unsigned)G - 1u) {
+            for (int s = 0; s < P.n_stages; ++s) { P.b1[s] = 0u; P.b2[s] = 0u; }
+            *P.done = 0u;
+            __threadfence();
+        }
+    }
+}
+
+cudaError_t launch_program(const void* prog_dev, int grid, cudaStream_t s) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(program_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PG_SMEM);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    count_launch();
+    program_kernel<<<grid, PG_THREADS, PG_SMEM, s>>>(reinterpret_cast<const DevProg*>(prog_dev));
+    return cudaGetLastError();
+}
+
+}  // namespace vla

@@ -27,13 +27,6 @@ constexpr int SM_WARPS = 8;
 constexpr int SM_THREADS = SM_WARPS * 32;
 constexpr int SM_UNROLL = 2;
 
-__device__ __forceinline__ void mma_m16n8k32_s8(int (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
-                                                uint32_t b0, uint32_t b1) {
-    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
-                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
-}
-
 // MTOK: padded token count (multiple of 8 for the MMA variant).
 template <int MTOK, bool USE_MMA>
 __global__ void __launch_bounds__(SM_THREADS) gemm_small_kernel(

@@ -1,0 +1,44 @@
+// program.h -- device-side form of a compiled "program" of ternary linears (internal to libvlaternary.so).
+// A program is a list of STAGES; a stage is one bf16 activation matrix x [M,K] (M <= 16) and the
+// ternary linears that consume it (q|k|v share one input, gate|up share one input: the per-output-group
+// scales beta_g(n) of Eq. 4).  Stage s+1 may read what stage s wrote (depends = 1).
+#pragma once
+#include <cstdint>
+
+namespace vla {
+
+constexpr uint32_t PROG_MAGIC = 0x564C4150u;   // "VLAP"
+
+struct DevLin {
+    const uint8_t* packed;     // packed W [N,K]
+    const float* beta;         // one fp32
+    void* out;                 // [M,N]
+    int N;
+    int dtype;                 // vla_dtype
+    int gran_begin;            // first 32-channel granule of this linear within its stage
+    int pad;
+};
+
+struct DevStage {
+    const uint4* x;            // bf16 [M,K]
+    uint2* xq;                 // int8 [M,K]   (inside the program buffer unless the caller asked for it)
+    float* xs;                 // fp32 [M]
+    int M, K;
+    int depends;               // 1: x is written by earlier stages of this program
+    int lin_begin, n_lin;
+    int granules;              // sum over its linears of N/32
+};
+
+struct DevProg {
+    uint32_t magic;
+    int n_stages;
+    int n_lin;
+    int pad;
+    unsigned* b1;              // [n_stages] CTAs that finished stage s        (target gridDim.x)
+    unsigned* b2;              // [n_stages] rows of stage s that are quantised (target M_s)
+    unsigned* done;            // [1]        CTAs that finished the program; the last one re-zeroes the counters
+    const DevStage* stages;
+    const DevLin* lins;
+};
+
+}  // namespace vla

@@ -1,0 +1,84 @@
+"""The chained decoder-layer stack of BASELINE.json configs[3] as a list of program stages (plumbing only).
+
+Per layer (reading R12; attention, activation function, norm and residual are skipped):
+    q,k,v = lin(quant(h));  h2 = lin_o(quant(q));  g,u = lin(quant(h2));  h' = lin_down(quant(u))
+i.e. four stages per layer, all intermediates bf16: [q|k|v] <- h, [o] <- q, [gate|up] <- h2, [down] <- u.
+Nothing here computes: the stages are executed by vla_program_run (M <= 16, one persistent launch) or, for
+larger M, one vla_ternary_linear call per linear (`run_stack_calls`).
+"""
+import torch
+
+from . import binding as vla
+from . import synth
+
+STAGES = [("h", ["q", "k", "v"]), ("q", ["o"]), ("o", ["gate", "up"]), ("up", ["down"])]
+_DIMS = {name: (K, N) for (name, K, N) in synth.STACK_LINEARS}
+
+
+class Stack:
+    """Device-resident weights and activation buffers of `layers` decoder layers at M tokens."""
+
+    def __init__(self, layers, M, device="cuda", weights=None):
+        self.layers, self.M, self.device = layers, M, device
+        self.packed, self.beta = [], []
+        for layer in range(layers):
+            lw = weights[layer] if weights is not None else synth.stack_layer(layer)
+            p, b = {}, {}
+            for d in lw:
+                w = torch.from_numpy(d["w"]).to(device)
+                p[d["name"]] = vla.pack_weights(w)
+                b[d["name"]] = torch.tensor([float(d["beta"])], dtype=torch.float32, device=device)
+                del w
+            self.packed.append(p)
+            self.beta.append(b)
+        # per-layer outputs (kept, so that every intermediate can be compared with the oracle)
+        self.h0 = torch.zeros((M, 2560), dtype=torch.bfloat16, device=device)
+        self.out = [{name: torch.zeros((M, _DIMS[name][1]), dtype=torch.bfloat16, device=device)
+                     for name in _DIMS} for _ in range(layers)]
+        self.packed_bytes = sum(t.numel() for p in self.packed for t in p.values())
+
+    def set_input(self, x_bits_u16):
+        import numpy as np
+        t = torch.from_numpy(np.ascontiguousarray(x_bits_u16).view(np.int16)).to(self.device).view(torch.bfloat16)
+        self.h0.copy_(t)
+
+    def _input_of(self, layer, src):
+        if src == "h":
+            return self.h0 if layer == 0 else self.out[layer - 1]["down"]
+        return self.out[layer][src]
+
+    def stages(self):
+        """Stage descriptors for vla_program_build (M <= 16)."""
+        st = []
+        for layer in range(self.layers):
+            for (src, names) in STAGES:
+                st.append(dict(
+                    x=self._input_of(layer, src), M=self.M, K=_DIMS[names[0]][0],
+                    depends=0 if (layer == 0 and src == "h") else 1,
+                    linears=[dict(packed=self.packed[layer][n], w_scale=self.beta[layer][n], out=self.out[layer][n],
+                                  N=_DIMS[n][1], out_dtype=vla.VLA_BF16) for n in names]))
+        return st
+
+    def compile(self):
+        self.program = vla.compile_program(self.stages(), self.device)
+        return self.program
+
+    def run_program(self):
+        vla.vla_program_run(self.program)
+
+    def alloc_call_workspace(self):
+        M = self.M
+        self.xq = {K: torch.empty((M, K), dtype=torch.int8, device=self.device) for K in (2560, 6912)}
+        self.xs = torch.empty((M,), dtype=torch.float32, device=self.device)
+
+    def run_stack_calls(self):
+        """One activation quant per stage and one GEMM call per linear (any M; the large-M route)."""
+        M = self.M
+        for layer in range(self.layers):
+            for (src, names) in STAGES:
+                x = self._input_of(layer, src)
+                K = _DIMS[names[0]][0]
+                vla.vla_act_quant(x, M, K, self.xq[K], self.xs)
+                for n in names:
+                    vla.vla_ternary_gemm(self.packed[layer][n], self.beta[layer][n], self.xq[K], self.xs, M,
+                                         _DIMS[n][1], K, self.out[layer][n], vla.VLA_BF16, vla.VLA_PATH_AUTO, None, 0)

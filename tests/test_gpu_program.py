@@ -1,0 +1,175 @@
+"""GPU parity tests (-m gpu) of the persistent program kernel (vla_program_build / vla_program_run): lists of
+small-M ternary linears, independent and chained, against the CPU oracle.  Same bars as test_gpu_parity.py;
+because the canonical operation order is followed (R1, R6) every output is also bit-identical, which
+is what makes the free-running chained stack of BASELINE.json configs[3] checkable end to end.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_08094_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL_F32 = 1e-6
+
+
+@pytest.fixture(scope="module")
+def vla():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_2606_08094_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def dev_bf16(bits_u16):
+    return torch.from_numpy(np.ascontiguousarray(bits_u16).view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def bits(t):
+    return t.view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+_TDT = {0: torch.float32, 1: torch.bfloat16, 2: torch.int32}
+
+
+def make_point(vla, M, K, N, seed, dtype, p_zero=0.35, want_xq=False):
+    w = synth.ternary_weights(N, K, p_zero, seed)
+    x = synth.activations(M, K, seed + 1, outlier_frac=0.01)
+    beta = synth.weight_scale(seed + 2)
+    d = dict(M=M, K=K, N=N, w=w, x_bits=x, beta=beta, dtype=dtype, packed=vla.pack_weights(dev(w)),
+             beta_d=dev(np.array([beta], np.float32)), x=dev_bf16(x),
+             out=torch.full((M, N), -7, dtype=_TDT[dtype], device="cuda"))
+    if want_xq:
+        d["xq"] = torch.full((M, K), 99, dtype=torch.int8, device="cuda")
+        d["xs"] = torch.full((M,), -1.0, dtype=torch.float32, device="cuda")
+    return d
+
+
+def stage_of(p):
+    return dict(x=p["x"], M=p["M"], K=p["K"], depends=0, xq_opt=p.get("xq"), x_scale_opt=p.get("xs"),
+                linears=[dict(packed=p["packed"], w_scale=p["beta_d"], out=p["out"], N=p["N"], out_dtype=p["dtype"])])
+
+
+def check_point(vla, oracle, p):
+    ref = oracle.ternary_linear(p["x_bits"], p["w"], p["beta"])
+    if p["dtype"] == vla.VLA_I32:
+        got = p["out"].cpu().numpy()
+        bad = np.argwhere(got != ref["acc"])
+        assert bad.size == 0, "int32 differs at %d places, first %s" % (len(bad), bad[0])
+    elif p["dtype"] == vla.VLA_F32:
+        got = p["out"].cpu().numpy()
+        assert np.all(np.abs(got.astype(np.float64) - ref["y64"]) <= REL_TOL_F32 * np.abs(ref["y64"]))
+        assert np.array_equal(got.view(np.uint32), ref["y32"].view(np.uint32))
+    else:
+        assert np.array_equal(bits(p["out"]), ref["ybf16"])
+    if "xq" in p:
+        assert np.array_equal(p["xq"].cpu().numpy(), ref["a"])
+        assert np.array_equal(p["xs"].cpu().numpy().view(np.uint32), ref["alpha"].view(np.uint32))
+
+
+@pytest.mark.parametrize("M,K,N", [(1, 128, 128), (8, 256, 256), (3, 384, 128), (16, 2560, 640), (13, 4224, 256),
+                                   (8, 8192, 384), (16, 8192, 128), (5, 6912, 2560)])
+@pytest.mark.parametrize("dtype", [0, 1, 2])
+def test_single_stage_program(vla, oracle, M, K, N, dtype):
+    """one linear per program, every output type; shapes span 1..4 ring chunks, ragged piece counts, both M tiles"""
+    p = make_point(vla, M, K, N, 9000 + M + K + N, dtype, want_xq=True)
+    prog = vla.compile_program([stage_of(p)])
+    vla.vla_program_run(prog)
+    torch.cuda.synchronize()
+    check_point(vla, oracle, p)
+    vla.vla_program_release(prog)
+
+
+def test_configs1_as_one_program(vla, oracle):
+    """BASELINE.json configs[1]: the 12 decode points (4 shapes x M in {1,8,16}) as 12 independent stages of ONE
+    launch, at full size, in the launch configuration bench.py times; run twice (the counters reset themselves)
+    and once from a CUDA graph."""
+    pts = []
+    for M in synth.DECODE_M:
+        for si in range(len(synth.MODEL_SHAPES)):
+            c = synth.config1_point(si, M)
+            pts.append(dict(M=M, K=c["K"], N=c["N"], w=c["w"], x_bits=c["x"], beta=c["beta"], dtype=vla.VLA_BF16,
+                            packed=vla.pack_weights(dev(c["w"])), beta_d=dev(np.array([c["beta"]], np.float32)),
+                            x=dev_bf16(c["x"]), out=torch.zeros((M, c["N"]), dtype=torch.bfloat16, device="cuda")))
+    prog = vla.compile_program([stage_of(p) for p in pts])
+    for rep in range(2):
+        for p in pts:
+            p["out"].fill_(-3.0)
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        for p in pts:
+            check_point(vla, oracle, p)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        vla.vla_program_run(prog)
+        vla.vla_program_run(prog)
+    for p in pts:
+        p["out"].fill_(-3.0)
+    g.replay()
+    torch.cuda.synchronize()
+    for p in pts:
+        check_point(vla, oracle, p)
+
+
+def oracle_stack(oracle, weights, x_bits):
+    """The chain of DESIGN.md R12 on the oracle, free-running, all intermediates bf16.  Returns per layer the
+    bf16 bit patterns of q, k, v, o, gate, up, down."""
+    outs = []
+    h = x_bits
+    for lw in weights:
+        W = {d["name"]: d for d in lw}
+        o = {}
+        for n in ("q", "k", "v"):
+            o[n] = oracle.ternary_linear(h, W[n]["w"], W[n]["beta"], want_y64=False)["ybf16"]
+        o["o"] = oracle.ternary_linear(o["q"], W["o"]["w"], W["o"]["beta"], want_y64=False)["ybf16"]
+        for n in ("gate", "up"):
+            o[n] = oracle.ternary_linear(o["o"], W[n]["w"], W[n]["beta"], want_y64=False)["ybf16"]
+        o["down"] = oracle.ternary_linear(o["up"], W["down"]["w"], W["down"]["beta"], want_y64=False)["ybf16"]
+        outs.append(o)
+        h = o["down"]
+    return outs
+
+
+@pytest.mark.parametrize("M", [1, 8, 16])
+def test_chained_stack_free_running(vla, oracle, M):
+    """configs[3] layers (full shapes: hidden 2560, 5 KV heads x 128, FFN 6912), 3 layers = 12 dependent stages in
+    one launch; every intermediate of every layer must be bit-identical to the oracle's chain."""
+    from paper_2606_08094_b200.stack import Stack
+    layers = 3
+    weights = [synth.stack_layer(l) for l in range(layers)]
+    x = synth.stack_input(M)
+    st = Stack(layers, M, weights=weights)
+    st.set_input(x)
+    st.compile()
+    for rep in range(2):
+        st.run_program()
+        torch.cuda.synchronize()
+        ref = oracle_stack(oracle, weights, x)
+        for l in range(layers):
+            for n in ref[l]:
+                assert np.array_equal(bits(st.out[l][n]), ref[l][n]), "layer %d %s differs (rep %d)" % (l, n, rep)
+    # the per-call route (quant kernel + one GEMM launch per linear) must give the same bits
+    st2 = Stack(layers, M, weights=weights)
+    st2.set_input(x)
+    st2.alloc_call_workspace()
+    st2.run_stack_calls()
+    torch.cuda.synchronize()
+    for l in range(layers):
+        for n in ref[l]:
+            assert np.array_equal(bits(st2.out[l][n]), ref[l][n]), "per-call route: layer %d %s differs" % (l, n)
+
+
+def test_program_errors(vla):
+    p = make_point(vla, 8, 256, 256, 5, vla.VLA_BF16)
+    bad_m = dict(stage_of(p), M=17)
+    assert vla.vla_program_bytes([bad_m]) == 0
+    bad_k = dict(stage_of(p), K=8192 + 128)
+    assert vla.vla_program_bytes([bad_k]) == 0
+    with pytest.raises(vla.VlaError) as e:
+        vla.vla_program_run(p["out"])          # not a compiled program
+    assert e.value.status == vla.VLA_ERR_VALUE
