@@ -129,9 +129,10 @@ vla_status vla_ternary_linear_host(const void* packed, const float* w_scale, con
  * (1..16) ternary linears that all consume it, each with its own packed W [N,K], scale beta and output:
  * the per-output-group scales beta_g(n) of Eq. 4, e.g. q|k|v or gate|up.
  * Every stage runs Eq. 4 end to end: absmax int8 quant of x, int32 contraction, dequant to out_dtype.
- *   depends = 0   x is written before the launch (quantised up front)
- *   depends = 1   x is (part of) the output of EARLIER stages of this program: the stage starts only
- *                 after every earlier stage has completed on the whole grid
+ *   depends = 0   x does not depend on the stages since the last depends = 1 stage: the stage joins the
+ *                 current PHASE, whose stages run concurrently on disjoint groups of SMs
+ *   depends = 1   x is (part of) the output of EARLIER stages of this program: the stage opens a new
+ *                 phase, which starts only after every earlier phase has completed on the whole grid
  * All pointers inside the descriptors are DEVICE pointers, 16-byte aligned, and must stay valid for as
  * long as the program is run.  The descriptor arrays themselves are HOST memory.
  */

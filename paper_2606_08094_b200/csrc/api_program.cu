@@ -14,7 +14,7 @@ using vla::DevLin;
 using vla::DevProg;
 using vla::DevStage;
 
-struct ProgInfo { int grid; int n_stages; };
+struct ProgInfo { int grid; int n_stages; int max_m; };
 std::mutex g_mu;
 std::unordered_map<const void*, ProgInfo> g_programs;
 
@@ -40,6 +40,9 @@ vla_status check_stages(const vla_prog_stage* st, int n) {
             if (!aligned16(l.packed) || !aligned16(l.out) || (reinterpret_cast<uintptr_t>(l.w_scale) & 3u)) return VLA_ERR_ALIGN;
         }
     }
+    size_t n_lin = 0;
+    for (int s = 0; s < n; ++s) n_lin += (size_t)st[s].n_linears;
+    if (sizeof(DevStage) * (size_t)n + sizeof(DevLin) * n_lin > vla::program_desc_capacity()) return VLA_ERR_SHAPE;
     return VLA_OK;
 }
 
@@ -94,13 +97,13 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     P->magic = vla::PROG_MAGIC;
     P->n_stages = n_stages;
     P->n_lin = L.n_lin;
-    P->b1 = reinterpret_cast<unsigned*>(base + L.off_counters);
-    P->b2 = P->b1 + n_stages;
+    P->bp = reinterpret_cast<unsigned*>(base + L.off_counters);
+    P->b2 = P->bp + n_stages;
     P->done = P->b2 + n_stages;
     P->stages = reinterpret_cast<const DevStage*>(base + L.off_stages);
     P->lins = reinterpret_cast<const DevLin*>(base + L.off_lins);
     size_t act = L.off_act;
-    int li = 0, max_gran = 0;
+    int li = 0, max_m = 0, phase = 0, max_phase_gran = 0, phase_gran = 0;
     for (int s = 0; s < n_stages; ++s) {
         const vla_prog_stage& a = stages[s];
         DevStage& d = S[s];
@@ -109,11 +112,15 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
         d.xq = reinterpret_cast<uint2*>(a.xq_opt ? (void*)a.xq_opt : (void*)(base + act));
         d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + act + qbytes);
         act += qbytes + 256;
-        d.M = a.M;
+        d.M = (int16_t)a.M;
         d.K = a.K;
-        d.depends = a.depends;
+        d.depends = (int16_t)((s == 0) ? 0 : a.depends);    // nothing precedes the first stage
+        if (d.depends) { ++phase; phase_gran = 0; }          // a dependent stage opens a new phase
+        d.phase = phase;
+        d.publish = 0;
+        if (a.M > max_m) max_m = a.M;
         d.lin_begin = li;
-        d.n_lin = a.n_linears;
+        d.n_lin = (int16_t)a.n_linears;
         int gran = 0;
         for (int j = 0; j < a.n_linears; ++j, ++li) {
             const vla_prog_linear& l = a.linears[j];
@@ -127,17 +134,49 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
             gran += l.N / 32;
         }
         d.granules = gran;
-        if (gran > max_gran) max_gran = gran;
+        phase_gran += gran;
+        if (phase_gran > max_phase_gran) max_phase_gran = phase_gran;
     }
-    int grid = max_gran < sms ? max_gran : sms;
+    P->n_phases = phase + 1;
+    int grid = max_phase_gran < sms ? max_phase_gran : sms;
     if (grid < 16 && sms >= 16) grid = 16;                  // enough CTAs to own one activation row each
+    // Split the grid among the stages of each phase in proportion to their weight bytes (>= 1 CTA each).
+    for (int s0 = 0; s0 < n_stages;) {
+        int s1 = s0 + 1;
+        while (s1 < n_stages && S[s1].phase == S[s0].phase) ++s1;
+        const int ns = s1 - s0;
+        if (ns > grid) return VLA_ERR_SHAPE;                 // more independent stages in one phase than CTAs
+        double total = 0.0;
+        for (int s = s0; s < s1; ++s) total += (double)S[s].granules * S[s].K;
+        int given = 0;
+        for (int s = s0; s < s1; ++s) {
+            int c = (int)((double)grid * ((double)S[s].granules * S[s].K) / total);
+            if (c < 1) c = 1;
+            S[s].cta_count = c;
+            given += c;
+        }
+        while (given != grid) {                              // hand the remainder to / take the excess from the
+            int best = s0;                                   // stage with the most / least bytes per CTA
+            for (int s = s0; s < s1; ++s) {
+                const double ls = (double)S[s].granules * S[s].K / S[s].cta_count;
+                const double lb = (double)S[best].granules * S[best].K / S[best].cta_count;
+                if (given < grid ? ls > lb : (S[s].cta_count > 1 && (S[best].cta_count <= 1 || ls < lb))) best = s;
+            }
+            S[best].cta_count += (given < grid) ? 1 : -1;
+            given += (given < grid) ? 1 : -1;
+        }
+        int begin = 0;
+        for (int s = s0; s < s1; ++s) { S[s].cta_begin = begin; begin += S[s].cta_count; }
+        S[s1 - 1].publish = (int16_t)((s1 < n_stages) ? 1 : 0);   // the next phase opens with a dependent stage
+        s0 = s1;
+    }
 
     cudaStream_t cs = (cudaStream_t)stream;
     cudaError_t e = cudaMemcpyAsync(prog_dev, host.data(), host.size(), cudaMemcpyHostToDevice, cs);
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     std::lock_guard<std::mutex> lk(g_mu);
-    g_programs[prog_dev] = ProgInfo{grid, n_stages};
+    g_programs[prog_dev] = ProgInfo{grid, n_stages, max_m};
     return VLA_OK;
 }
 
@@ -150,7 +189,7 @@ vla_status vla_program_run(const void* prog_dev, void* stream) {
         if (it == g_programs.end()) return VLA_ERR_VALUE;
         info = it->second;
     }
-    cudaError_t e = vla::launch_program(prog_dev, info.grid, (cudaStream_t)stream);
+    cudaError_t e = vla::launch_program(prog_dev, info.grid, info.max_m, (cudaStream_t)stream);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     return VLA_OK;
 }

@@ -14,12 +14,14 @@
 //                        reduce the 16 partial sums per output through shared memory, and run the dequant
 //                        epilogue  y = (float)acc * (alpha_m * beta).
 // Work unit: a GRANULE = 32 output channels x all of K of one linear (K/128 contiguous 1 KiB pieces of the packed
-// layout); granule gi of a stage goes to CTA gi mod gridDim.x.
+// layout).  The stages of one PHASE are independent, so they run CONCURRENTLY on disjoint CTA groups sized by their
+// weight bytes (no serialisation between them, and each activation matrix is read by its own group only instead
+// of by all 148 SMs); granule gi of a stage goes to CTA (gi mod group size) of its group.
 // Activation quant (Eq. 4 lines 1-2): row r of stage s is quantised by ONE owner CTA (absmax over the row, then
 // the true-division quantiser of quant.cuh) into global int8 + alpha; counters in global memory order the phases:
-//   b1[s] = CTAs that finished stage s   (a dependent stage's row owners wait for b1[s-1] == gridDim.x)
-//   b2[s] = rows of stage s quantised    (every CTA waits for b2[s] == M_s before it loads its B fragments)
-// Stages that do not depend on earlier ones are quantised up front.  int32 sums are exact in any order, so the
+//   bp[p] = CTAs that finished phase p   (a dependent stage's row owners wait for bp[p-1] == gridDim.x)
+//   b2[s] = rows of stage s quantised    (the stage's group waits for b2[s] == M_s before it loads its B fragments)
+// int32 sums are exact in any order, so the
 // result is bit-identical to the per-call kernels and to the oracle.
 #include <cuda_bf16.h>
 #include "common.cuh"
@@ -33,10 +35,28 @@ constexpr int PG_W = 16;                         // consumer warps
 constexpr int PG_CONSUMERS = PG_W * 32;          // 512 threads
 constexpr int PG_THREADS = PG_CONSUMERS + 32;
 constexpr int PG_SLOT_BYTES = 16384;             // 16 pieces of 1 KiB = 32 blocks of 32 ch x 64 k
-constexpr int PG_NSLOT = 12;
+constexpr int PG_NSLOT = 11;
+constexpr int PG_DESC_BYTES = 15360;             // stage + linear descriptors cached in shared memory
 constexpr int PG_NBMAX = 8;                      // k blocks per warp per granule  ->  K <= 8192
 constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 8448 ints = 33 792 B
-constexpr int PG_SMEM = PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + 2 * PG_NSLOT * 8 + 64 + 128;
+constexpr int PG_SMEM = PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + 2 * PG_NSLOT * 8 + 64 + 128;
+
+#ifdef VLA_PROG_TRACE
+// debug-only (never defined in the product build): per-CTA globaltimer stamps, read back by vla_debug_read_trace
+__device__ unsigned long long g_trace[148 * 1024];
+__device__ __forceinline__ void trace(int cta, int& n, int tid) {
+    if (tid == 0 && n < 1024) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        g_trace[cta * 1024 + n++] = t;
+    }
+}
+#define TRACE() trace(cta, tr_n, tid)
+#define TRARG , tr_n
+#else
+#define TRACE()
+#define TRARG
+#endif
 
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(PG_CONSUMERS) : "memory"); }
 
@@ -54,21 +74,34 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return r;
 }
 
-__device__ __forceinline__ int owner_of(int s, int r, int G) { return G - 1 - ((s * 16 + r) % G); }
+// publish: every store this CTA made before the preceding consumer_bar() becomes visible before the count does
+__device__ __forceinline__ void red_release_gpu(unsigned* p, unsigned v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+
+// non-volatile form: the compiler may interleave it with the decode of the next block
+__device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                                   uint32_t b0, uint32_t b1) {
+    asm("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
 
 // ---------------------------------------------------------------- producer warp
-__device__ __forceinline__ void producer(const DevProg& P, int cta, int G, int lane, uint32_t ring, uint32_t bar_full,
-                                         uint32_t bar_empty) {
+__device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, int cta,
+                                         int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty) {
     uint32_t slot = 0, round = 0;
     for (int s = 0; s < P.n_stages; ++s) {
-        const DevStage st = P.stages[s];
+        const DevStage& st = stages[s];
+        const int rank = cta - st.cta_begin;
+        if (rank < 0 || rank >= st.cta_count) continue;      // another group's stage
         const int KB = st.K / TILE_K;                       // 1 KiB pieces per granule
-        for (int gi = cta; gi < st.granules; gi += G) {
+        for (int gi = rank; gi < st.granules; gi += st.cta_count) {
             int l = st.lin_begin;
             for (int j = 1; j < st.n_lin; ++j)
-                if (gi >= P.lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
-            const int n32 = gi - P.lins[l].gran_begin;
-            const uint8_t* src = P.lins[l].packed + ((size_t)(n32 >> 2) * KB * 8 + (size_t)(n32 & 3) * 2) * 512;
+                if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
+            const int n32 = gi - lins[l].gran_begin;
+            const uint8_t* src = lins[l].packed + ((size_t)(n32 >> 2) * KB * 8 + (size_t)(n32 & 3) * 2) * 512;
             for (int p0 = 0; p0 < KB; p0 += 16) {
                 const int np = min(16, KB - p0);
                 if (round > 0) mbar_wait(bar_empty + 8u * slot, (round - 1) & 1);
@@ -107,57 +140,68 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     consumer_bar();                                          // s_max may be reused; stores precede thread 0's fence
 }
 
-__device__ __forceinline__ void quant_owned_rows(const DevProg& P, int s, const DevStage& st, int cta, int G, int tid,
-                                                 float* s_max) {
-    int owned = 0;
-    for (int r = 0; r < st.M; ++r) owned += (owner_of(s, r, G) == cta);
-    if (owned == 0) return;
-    if (st.depends && s > 0) {
-        if (tid == 0) spin_until(P.b1 + (s - 1), (unsigned)G);
+// Row r of a stage is quantised by CTA (count - 1 - r mod count) of the stage's group.
+__device__ __forceinline__ void quant_owned_rows(const DevProg& P, int s, const DevStage& st, int rank, int count, int G,
+                                                 int tid, float* s_max) {
+    const int first = count - 1 - rank;                      // rows first, first + count, ...
+    if (first >= st.M) return;
+    if (st.depends) {
+        if (tid == 0) spin_until(P.bp + (st.phase - 1), (unsigned)G);
         consumer_bar();
     }
-    for (int r = 0; r < st.M; ++r)
-        if (owner_of(s, r, G) == cta) quant_row(st, r, tid, s_max);
-    if (tid == 0) {
-        __threadfence();
-        atomicAdd(P.b2 + s, (unsigned)owned);
-    }
+    int owned = 0;
+    for (int r = first; r < st.M; r += count, ++owned) quant_row(st, r, tid, s_max);
+    if (tid == 0) red_release_gpu(P.b2 + s, (unsigned)owned);
 }
 
 // ---------------------------------------------------------------- one stage's granules on the consumer warps
-template <int MT>
-__device__ __forceinline__ void stage_gemm(const DevProg& P, const DevStage& st, int cta, int G, int tid, uint32_t ring,
-                                           int* red, uint32_t bar_full, uint32_t bar_empty, uint32_t& slot,
-                                           uint32_t& phase, uint32_t& gcount) {
-    constexpr int MTOK = MT * 8;
+// int8 activations of this warp's k blocks (kq = 16 i + w), as mma B fragments, in registers for the whole stage
+template <int MAXMT>
+__device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)[PG_NBMAX][MAXMT]) {
     const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-    const int K = st.K, M = st.M, nblk = K / BLK_K, KB = K / TILE_K;
-    const int nchunks = (KB + 15) >> 4;
-
-    // int8 activations of this warp's k blocks, as B fragments, in registers for the whole stage
-    uint4 xv[PG_NBMAX][MT];
+    const int K = st.K, nblk = K / BLK_K;
     const int8_t* xq = reinterpret_cast<const int8_t*>(st.xq);
 #pragma unroll
     for (int i = 0; i < PG_NBMAX; ++i)
 #pragma unroll
-        for (int mt = 0; mt < MT; ++mt) {
+        for (int mt = 0; mt < MAXMT; ++mt) {
             const int kq = i * PG_W + w, tok = mt * 8 + g;
-            xv[i][mt] = (kq < nblk && tok < M)
+            xv[i][mt] = (kq < nblk && tok < st.M)
                             ? __ldcg(reinterpret_cast<const uint4*>(xq + (size_t)tok * K + kq * BLK_K + t * 16))
                             : make_uint4(0, 0, 0, 0);
         }
+}
+
+// cta / G: rank and size of the stage's CTA group
+template <int MT, int MAXMT>
+__device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& st, int cta, int G,
+                                           int tid, uint32_t ring, int* red, uint32_t bar_full, uint32_t bar_empty,
+                                           uint4 (&xv)[PG_NBMAX][MAXMT], uint32_t& slot, uint32_t& phase, uint32_t& gcount
+#ifdef VLA_PROG_TRACE
+                                           , int& tr_n
+#endif
+                                           ) {
+    constexpr int MTOK = MT * 8;
+    const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int M = st.M, nblk = st.K / BLK_K, KB = st.K / TILE_K;
+    const int nchunks = (KB + 15) >> 4;
     const int etok = tid >> 5, ech = tid & 31;               // epilogue role: one output per thread
     const bool eactive = (etok < M) && (etok < MTOK);
     const float alpha = eactive ? __ldcg(st.xs + etok) : 0.0f;
     const uint32_t my_off = (uint32_t)((w >> 1) * 1024 + (w & 1) * 512 + lane * 16);
 
     for (int gi = cta; gi < st.granules; gi += G) {
+        TRACE();
         int l = st.lin_begin;
         for (int j = 1; j < st.n_lin; ++j)
-            if (gi >= P.lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
-        const DevLin L = P.lins[l];
+            if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
+        const DevLin& L = lins[l];
         const int n32 = gi - L.gran_begin;
+        const float beta = (eactive && L.dtype != 2) ? __ldcg(L.beta) : 0.0f;     // needed only in the epilogue
 
+#ifdef VLA_PROG_TRACE
+        long long twait = 0;
+#endif
         int acc[2][MT][4];
 #pragma unroll
         for (int c = 0; c < 2; ++c)
@@ -169,13 +213,27 @@ __device__ __forceinline__ void stage_gemm(const DevProg& P, const DevStage& st,
 #pragma unroll
         for (int ck = 0; ck < PG_NBMAX / 2; ++ck) {
             if (ck < nchunks) {
+#ifdef VLA_PROG_TRACE
+                long long tw0 = clock64();
+#endif
                 mbar_wait(bar_full + 8u * slot, phase);
+#ifdef VLA_PROG_TRACE
+                twait += clock64() - tw0;
+#endif
+                // both blocks of this warp in the chunk -> registers, then hand the slot back at once
+                uint4 wv[2];
+#pragma unroll
+                for (int ii = 0; ii < 2; ++ii)
+                    wv[ii] = ((2 * ck + ii) * PG_W + w < nblk) ? lds128(ring + slot * PG_SLOT_BYTES + ii * 8192 + my_off)
+                                                               : make_uint4(0, 0, 0, 0);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty + 8u * slot);       // release: ordered after the loads above
+                if (++slot == PG_NSLOT) { slot = 0; phase ^= 1; }
 #pragma unroll
                 for (int ii = 0; ii < 2; ++ii) {
                     const int i = 2 * ck + ii;
                     if (i * PG_W + w < nblk) {
-                        const uint4 wv = lds128(ring + slot * PG_SLOT_BYTES + ii * 8192 + my_off);
-                        const uint32_t w4[4] = {wv.x, wv.y, wv.z, wv.w};
+                        const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
 #pragma unroll
                         for (int c = 0; c < 2; ++c) {
                             const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];     // channels 16c+g and 16c+g+8
@@ -183,18 +241,19 @@ __device__ __forceinline__ void stage_gemm(const DevProg& P, const DevStage& st,
                             const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
 #pragma unroll
                             for (int mt = 0; mt < MT; ++mt) {
-                                mma_m16n8k32_s8(acc[c][mt], a0, a1, a2, a3, xv[i][mt].x, xv[i][mt].y);
-                                mma_m16n8k32_s8(acc[c][mt], e0, e1, e2, e3, xv[i][mt].z, xv[i][mt].w);
+                                mma_m16n8k32_s8_nv(acc[c][mt], a0, a1, a2, a3, xv[i][mt].x, xv[i][mt].y);
+                                mma_m16n8k32_s8_nv(acc[c][mt], e0, e1, e2, e3, xv[i][mt].z, xv[i][mt].w);
                             }
                         }
                     }
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_empty + 8u * slot);
-                if (++slot == PG_NSLOT) { slot = 0; phase ^= 1; }
             }
         }
 
+#ifdef VLA_PROG_TRACE
+        if (tid == 0 && tr_n < 1024) g_trace[cta * 1024 + tr_n++] = (unsigned long long)twait;   // cycles, not a stamp
+#endif
+        TRACE();
         // 16 per-warp partial sums -> shared memory -> one thread per output
         int* rb = red + ((MT == 1) ? (int)(gcount & 1) * (PG_W * 8 * 33) : 0);
 #pragma unroll
@@ -208,6 +267,7 @@ __device__ __forceinline__ void stage_gemm(const DevProg& P, const DevStage& st,
                 row0[33 + 8] = acc[c][mt][3];
             }
         consumer_bar();
+        TRACE();
         if (eactive) {
             int sum = 0;
 #pragma unroll
@@ -217,26 +277,30 @@ __device__ __forceinline__ void stage_gemm(const DevProg& P, const DevStage& st,
             if (L.dtype == 2) {
                 reinterpret_cast<int*>(L.out)[o] = a;
             } else {
-                const float y = dequant(a, __fmul_rn(alpha, __ldcg(L.beta)));
+                const float y = dequant(a, __fmul_rn(alpha, beta));
                 if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
                 else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
             }
         }
         if (MT == 2) consumer_bar();                          // single reduction buffer: wait for the readers
+        TRACE();
         ++gcount;
     }
 }
 
 // ---------------------------------------------------------------- the kernel
+// MAXMT = 1: every stage has M <= 8 (32 registers of B fragments per thread, no spills);  MAXMT = 2: M <= 16.
+template <int MAXMT>
 __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* __restrict__ prog) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
     const uint32_t ring = base;
     int* red = reinterpret_cast<int*>(base_ptr + PG_NSLOT * PG_SLOT_BYTES);
-    const uint32_t bar_full = base + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4;
+    uint8_t* desc = base_ptr + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4;
+    const uint32_t bar_full = base + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES;
     const uint32_t bar_empty = bar_full + 8u * PG_NSLOT;
-    float* s_max = reinterpret_cast<float*>(base_ptr + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + 16 * PG_NSLOT);
+    float* s_max = reinterpret_cast<float*>(desc + PG_DESC_BYTES + 16 * PG_NSLOT);
 
     const int tid = threadIdx.x, cta = blockIdx.x, G = gridDim.x;
     if (tid == 0) {
@@ -246,54 +310,84 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
         }
         fence_barrier_init();
     }
-    __syncthreads();
     const DevProg P = *prog;
+    // descriptor tables -> shared memory (they are read on every granule by producer and consumers)
+    const int stage_words = P.n_stages * (int)(sizeof(DevStage) / 8), lin_words = P.n_lin * (int)(sizeof(DevLin) / 8);
+    {
+        const uint2* gs = reinterpret_cast<const uint2*>(P.stages);
+        const uint2* gl = reinterpret_cast<const uint2*>(P.lins);
+        uint2* d = reinterpret_cast<uint2*>(desc);
+        for (int i = tid; i < stage_words; i += PG_THREADS) d[i] = gs[i];
+        for (int i = tid; i < lin_words; i += PG_THREADS) d[stage_words + i] = gl[i];
+    }
+    __syncthreads();
+    const DevStage* stages = reinterpret_cast<const DevStage*>(desc);
+    const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
 
     if (tid >= PG_CONSUMERS) {
-        producer(P, cta, G, tid & 31, ring, bar_full, bar_empty);
+        producer(P, stages, lins, cta, tid & 31, ring, bar_full, bar_empty);
         return;
     }
-
-    // stages whose input comes from outside the program: quantise up front
-    for (int s = 0; s < P.n_stages; ++s) {
-        const DevStage st = P.stages[s];
-        if (!st.depends || s == 0) quant_owned_rows(P, s, st, cta, G, tid, s_max);
-    }
+#ifdef VLA_PROG_TRACE
+    int tr_n = 0;
+#endif
+    TRACE();
+    uint4 xv[PG_NBMAX][MAXMT];
     uint32_t slot = 0, phase = 0, gcount = 0;
     for (int s = 0; s < P.n_stages; ++s) {
-        const DevStage st = P.stages[s];
-        if (st.depends && s > 0) quant_owned_rows(P, s, st, cta, G, tid, s_max);
-        if (tid == 0) spin_until(P.b2 + s, (unsigned)st.M);
-        consumer_bar();
-        if (st.M <= 8) stage_gemm<1>(P, st, cta, G, tid, ring, red, bar_full, bar_empty, slot, phase, gcount);
-        else           stage_gemm<2>(P, st, cta, G, tid, ring, red, bar_full, bar_empty, slot, phase, gcount);
-        consumer_bar();                                      // every output store of this CTA precedes the fence
-        if (tid == 0) {
-            __threadfence();
-            atomicAdd(P.b1 + s, 1u);
+        const DevStage& st = stages[s];
+        const int rank = cta - st.cta_begin, count = st.cta_count;
+        if (rank >= 0 && rank < count) {                     // this CTA belongs to the stage's group
+            quant_owned_rows(P, s, st, rank, count, G, tid, s_max);
+            TRACE();
+            if (tid == 0) spin_until(P.b2 + s, (unsigned)st.M);
+            consumer_bar();
+            TRACE();
+            load_xv<MAXMT>(st, tid, xv);
+            if (MAXMT == 1 || st.M <= 8)
+                stage_gemm<1, MAXMT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, slot, phase, gcount TRARG);
+            else
+                stage_gemm<MAXMT, MAXMT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, slot, phase, gcount TRARG);
+            TRACE();
+        }
+        if (st.publish) {                                    // end of a phase that a later phase reads from
+            consumer_bar();                                  // every output store of this CTA precedes the release
+            if (tid == 0) red_release_gpu(P.bp + st.phase, 1u);
+            TRACE();
         }
     }
     // the last CTA to finish re-zeroes the counters, so the next launch of the same program needs no memset
     if (tid == 0) {
         const unsigned prev = atomicAdd(P.done, 1u);
         if (prev == (unsigned)G - 1u) {
-            for (int s = 0; s < P.n_stages; ++s) { P.b1[s] = 0u; P.b2[s] = 0u; }
+            for (int s = 0; s < P.n_stages; ++s) P.b2[s] = 0u;
+            for (int q = 0; q < P.n_phases; ++q) P.bp[q] = 0u;
             *P.done = 0u;
             __threadfence();
         }
     }
 }
 
-cudaError_t launch_program(const void* prog_dev, int grid, cudaStream_t s) {
+size_t program_desc_capacity() { return PG_DESC_BYTES; }
+
+cudaError_t launch_program(const void* prog_dev, int grid, int max_m, cudaStream_t s) {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(program_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PG_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(program_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, PG_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(program_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, PG_SMEM);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     count_launch();
-    program_kernel<<<grid, PG_THREADS, PG_SMEM, s>>>(reinterpret_cast<const DevProg*>(prog_dev));
+    if (max_m <= 8) program_kernel<1><<<grid, PG_THREADS, PG_SMEM, s>>>(reinterpret_cast<const DevProg*>(prog_dev));
+    else            program_kernel<2><<<grid, PG_THREADS, PG_SMEM, s>>>(reinterpret_cast<const DevProg*>(prog_dev));
     return cudaGetLastError();
 }
+
+#ifdef VLA_PROG_TRACE
+extern "C" int vla_debug_read_trace(unsigned long long* host, size_t n) {
+    return (int)cudaMemcpyFromSymbol(host, g_trace, n * sizeof(unsigned long long));
+}
+#endif
 
 }  // namespace vla

@@ -1,7 +1,8 @@
 // program.h -- device-side form of a compiled "program" of ternary linears (internal to libvlaternary.so).
 // A program is a list of STAGES; a stage is one bf16 activation matrix x [M,K] (M <= 16) and the
 // ternary linears that consume it (q|k|v share one input, gate|up share one input: the per-output-group
-// scales beta_g(n) of Eq. 4).  Stage s+1 may read what stage s wrote (depends = 1).
+// scales beta_g(n) of Eq. 4).  A stage with depends = 1 opens a new PHASE and may read what earlier
+// phases wrote; the stages of one phase are independent of each other.
 #pragma once
 #include <cstdint>
 
@@ -23,19 +24,24 @@ struct DevStage {
     const uint4* x;            // bf16 [M,K]
     uint2* xq;                 // int8 [M,K]   (inside the program buffer unless the caller asked for it)
     float* xs;                 // fp32 [M]
-    int M, K;
-    int depends;               // 1: x is written by earlier stages of this program
-    int lin_begin, n_lin;
+    int16_t M;
+    int16_t n_lin;
+    int16_t depends;           // 1: x is written by earlier phases of this program
+    int16_t publish;           // 1: last stage of its phase AND the next phase has a dependent stage -> count in bp
+    int K;
+    int lin_begin;
     int granules;              // sum over its linears of N/32
+    int phase;                 // stages of one phase are independent and run concurrently on disjoint CTA groups
+    int cta_begin, cta_count;  // the CTA group of this stage: [cta_begin, cta_begin + cta_count)
 };
 
 struct DevProg {
     uint32_t magic;
     int n_stages;
     int n_lin;
-    int pad;
-    unsigned* b1;              // [n_stages] CTAs that finished stage s        (target gridDim.x)
-    unsigned* b2;              // [n_stages] rows of stage s that are quantised (target M_s)
+    int n_phases;
+    unsigned* bp;              // [n_phases] CTAs that finished phase p             (target gridDim.x)
+    unsigned* b2;              // [n_stages] rows of stage s that are quantised      (target M_s)
     unsigned* done;            // [1]        CTAs that finished the program; the last one re-zeroes the counters
     const DevStage* stages;
     const DevLin* lins;
