@@ -168,6 +168,18 @@ vla_status vla_program_build(const vla_prog_stage* stages /*host*/, int n_stages
  * Runs of the same program must not overlap in time (they share its counters and activations). */
 vla_status vla_program_run(const void* prog_dev, void* stream);
 
+/* Host-buffer form of vla_program_run (the end-to-end call of a serving process): copies every `in` entry
+ * host->device, runs the program, copies every `out` entry device->host, all on `stream`, then SYNCHRONISES
+ * `stream`.  `host` pointers are HOST memory (pinned for asynchronous copies), `dev` pointers the device
+ * buffers the program's stages read / write.  The arrays themselves are HOST memory. */
+typedef struct {
+    void* host;
+    void* dev;
+    size_t bytes;
+} vla_copy;
+vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in /*host*/, int n_in,
+                                const vla_copy* out /*host*/, int n_out, void* stream);
+
 /* Forgets a compiled program (the caller then frees prog_dev). */
 vla_status vla_program_release(const void* prog_dev);
 

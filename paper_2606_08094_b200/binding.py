@@ -26,8 +26,12 @@ EXPORTS = [
     "vla_act_quant", "vla_ternary_gemm", "vla_ternary_linear", "vla_ternary_linear_host",
     "vla_ternary_host_workspace_bytes",
     "vla_ternary_auto_path", "vla_i8_mma_issue_probe", "vla_status_string", "vla_launch_count",
-    "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_release",
+    "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_run_host", "vla_program_release",
 ]
+
+
+class vla_copy(ctypes.Structure):
+    _fields_ = [("host", ctypes.c_void_p), ("dev", ctypes.c_void_p), ("bytes", ctypes.c_size_t)]
 
 
 class vla_prog_linear(ctypes.Structure):
@@ -86,6 +90,8 @@ def _load():
     lib.vla_program_build.argtypes = [ps, i, vp, sz, vp]
     lib.vla_program_run.restype = st
     lib.vla_program_run.argtypes = [vp, vp]
+    lib.vla_program_run_host.restype = st
+    lib.vla_program_run_host.argtypes = [vp, ctypes.POINTER(vla_copy), i, ctypes.POINTER(vla_copy), i, vp]
     lib.vla_program_release.restype = st
     lib.vla_program_release.argtypes = [vp]
     return lib
@@ -213,6 +219,20 @@ def vla_program_build(stages, prog_dev, prog_bytes=None, stream=None):
 
 def vla_program_run(prog_dev, stream=None):
     _check(_lib.vla_program_run(_ptr(prog_dev), _stream(stream)), "vla_program_run")
+
+
+def make_copies(pairs):
+    """[(host tensor, device tensor)] -> ctypes array of vla_copy (marshalled once, reusable across calls)."""
+    arr = (vla_copy * len(pairs))()
+    for k, (h, d) in enumerate(pairs):
+        arr[k] = vla_copy(_ptr(h), _ptr(d), h.numel() * h.element_size())
+    return arr
+
+
+def vla_program_run_host(prog_dev, copies_in, copies_out, stream=None):
+    """copies_in / copies_out: ctypes arrays from make_copies.  Synchronises the stream."""
+    _check(_lib.vla_program_run_host(_ptr(prog_dev), copies_in, len(copies_in), copies_out, len(copies_out),
+                                     _stream(stream)), "vla_program_run_host")
 
 
 def vla_program_release(prog_dev):

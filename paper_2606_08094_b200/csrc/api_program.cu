@@ -194,6 +194,29 @@ vla_status vla_program_run(const void* prog_dev, void* stream) {
     return VLA_OK;
 }
 
+vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in, int n_in, const vla_copy* out, int n_out,
+                                void* stream) {
+    if (!prog_dev || (n_in > 0 && !in) || (n_out > 0 && !out)) return VLA_ERR_NULL;
+    if (n_in < 0 || n_out < 0) return VLA_ERR_SHAPE;
+    for (int i = 0; i < n_in; ++i) if (!in[i].host || !in[i].dev) return VLA_ERR_NULL;
+    for (int i = 0; i < n_out; ++i) if (!out[i].host || !out[i].dev) return VLA_ERR_NULL;
+    cudaStream_t cs = (cudaStream_t)stream;
+    for (int i = 0; i < n_in; ++i)
+        if (cudaMemcpyAsync(in[i].dev, in[i].host, in[i].bytes, cudaMemcpyHostToDevice, cs) != cudaSuccess) {
+            cudaGetLastError();
+            return VLA_ERR_CUDA;
+        }
+    vla_status st = vla_program_run(prog_dev, stream);
+    if (st != VLA_OK) return st;
+    for (int i = 0; i < n_out; ++i)
+        if (cudaMemcpyAsync(out[i].host, out[i].dev, out[i].bytes, cudaMemcpyDeviceToHost, cs) != cudaSuccess) {
+            cudaGetLastError();
+            return VLA_ERR_CUDA;
+        }
+    if (cudaStreamSynchronize(cs) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+    return VLA_OK;
+}
+
 vla_status vla_program_release(const void* prog_dev) {
     if (!prog_dev) return VLA_ERR_NULL;
     std::lock_guard<std::mutex> lk(g_mu);
