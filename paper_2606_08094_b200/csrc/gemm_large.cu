@@ -2,178 +2,278 @@
 // ("Packed weight tiles are decoded in shared memory; activation tiles are
 // reused across outputs.  Products accumulate in 32-bit integers ...").
 //
-// One CTA computes a 128(channels) x TN(tokens) output tile:
-//   MMA operand A = decoded weights  [128 ch  x 128 k] int8, K-major, SWIZZLE_128B  (written by decode warps)
+// Persistent kernel: one CTA per SM walks the output tiles  t = blockIdx.x, += gridDim.x.
+// A tile is 128 (channels) x TN (tokens, multiple of 16, <= 256):
+//   MMA operand A = decoded weights  [128 ch  x 128 k] int8, K-major, SWIZZLE_128B  (written by the decode warps)
 //   MMA operand B = int8 activations [TN tok  x 128 k] int8, K-major, SWIZZLE_128B  (written by TMA)
-//   D (TMEM)      = int32 [128 lanes = channels] x [TN columns = tokens]
-// Warp roles (192 threads):
-//   warp 0      TMA producer: cp.async.bulk of the 4 KiB packed weight tile + tensor-map load of the X tile
-//   warp 1      TMEM allocator; one lane issues tcgen05.mma.cta_group::1.kind::i8 (4 x K=32 per k-block)
-//   warps 2-5   decode: packed words (smem) -> int8 (64*q) -> swizzled A tile; fence.proxy.async; then,
-//               after the last k-block, the epilogue: tcgen05.ld -> >>6 -> (float)acc*(alpha_m*beta) -> store
-// Pipelines: full_w (TMA->decode), full_x (TMA->MMA), decoded (decode->MMA), empty (MMA commit->TMA).
+//   D (TMEM)      = int32 [128 lanes = channels] x [TN columns = tokens], TWO buffers (columns 0.. and 256..)
+// Warp roles (15 warps):
+//   warp 0       W producer: cp.async.bulk of the 4 KiB packed weight tile per k block, 8-deep ring (weights never
+//                depend on the previous kernel, so this starts before griddepcontrol.wait)
+//   warp 1       X producer: tensor-map (TMA) load of the [TN x 128] activation tile per k block, 4-deep ring
+//   warp 2       TMEM allocator; one lane issues tcgen05.mma.cta_group::1.kind::i8 (4 x K=32 per k block)
+//   warps 3-10   decode: packed words (smem) -> int8 (64*q) -> swizzled A tile (3-deep ring); fence.proxy.async
+//   warps 11-14  epilogue: tcgen05.ld -> >>6 -> (float)acc*(alpha_m*beta) -> store, overlapped with the next
+//                tile's main loop through the second TMEM buffer
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cstdlib>
 #include "common.cuh"
 #include "kernels.h"
 
 namespace vla {
 
-constexpr int LG_THREADS = 192;
-constexpr int LG_STAGES = 4;
+#ifdef VLA_LG_DEBUG
+// debug-only (never defined in the product build): switch pipeline pieces off to find the per-k-block bottleneck
+__device__ int g_lg_dbg = 0;
+__device__ long long g_lg_trace[4][512];
+#define LG_DBG(bit) (g_lg_dbg & (bit))
+#define LG_STAMP(role, n) do { if (blockIdx.x == 0 && (n) < 512) g_lg_trace[role][(n)] = clock64(); } while (0)
+#else
+#define LG_DBG(bit) 0
+#define LG_STAMP(role, n) do { } while (0)
+#endif
+
+constexpr int LG_THREADS = 15 * 32;
+constexpr int LG_SW = 6;                                // packed-weight stages (4 KiB each)
+constexpr int LG_NS_MAX = 8;                            // {decoded A, X} stages
 constexpr int LG_A_BYTES = TILE_N * TILE_K;             // 16384 decoded int8
-constexpr int LG_X_BYTES = 256 * TILE_K;                // 32768 (TN <= 256)
 constexpr int LG_W_BYTES = TILE_BYTES;                  // 4096 packed
-constexpr int LG_SMEM = LG_STAGES * (LG_A_BYTES + LG_X_BYTES + LG_W_BYTES) + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int LG_STAGE_REGION = 192 * 1024;             // 4 stages at TN = 256, 6 at TN = 96
+constexpr int LG_SCALE_BYTES = 4 * 256 * 4;             // per epilogue warp: alpha_m * beta of the tile's tokens
+constexpr int LG_NBAR = 2 * LG_SW + 2 * LG_NS_MAX + 4;
+constexpr int LG_FIXED_SMEM = LG_SW * LG_W_BYTES + LG_SCALE_BYTES + 1024 /*align*/ + 8 * LG_NBAR + 16;
+
+__host__ __device__ inline uint32_t lg_stage_stride(int TN) { return LG_A_BYTES + (((uint32_t)TN * TILE_K + 1023u) & ~1023u); }
+
+__device__ __forceinline__ uint4 lds128_nv(uint32_t addr) {
+    uint4 r;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+    return r;
+}
 
 __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     const __grid_constant__ CUtensorMap tmap_x, const uint8_t* __restrict__ packed,
-    const float* __restrict__ w_scale, const float* x_scale, void* out,
-    int M, int N, int K, int TN, int tmem_cols, int out_dtype) {
+    const float* __restrict__ w_scale, const float* __restrict__ x_scale, void* __restrict__ out,
+    int M, int N, int K, int TN, int NS, int out_dtype) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
-    const uint32_t sA = base;                                           // [STAGES][16384]
-    const uint32_t sX = sA + LG_STAGES * LG_A_BYTES;                    // [STAGES][32768]
-    const uint32_t sW = sX + LG_STAGES * LG_X_BYTES;                    // [STAGES][4096]
-    const uint32_t sBar = sW + LG_STAGES * LG_W_BYTES;
-    uint8_t* pW = base_ptr + LG_STAGES * (LG_A_BYTES + LG_X_BYTES);
-    uint8_t* pA = base_ptr;
-    auto bar_full_w = [&](int s) { return sBar + 8u * s; };
-    auto bar_full_x = [&](int s) { return sBar + 8u * (LG_STAGES + s); };
-    auto bar_decoded = [&](int s) { return sBar + 8u * (2 * LG_STAGES + s); };
-    auto bar_empty = [&](int s) { return sBar + 8u * (3 * LG_STAGES + s); };
-    const uint32_t bar_acc = sBar + 8u * (4 * LG_STAGES);
-    const uint32_t tmem_slot = sBar + 8u * (4 * LG_STAGES + 1);
+    const uint32_t stride = lg_stage_stride(TN);
+    const uint32_t sS = base;                                           // [NS]{A 16384 | X TN*128}
+    const uint32_t sW = sS + (uint32_t)NS * stride;                     // [SW][4096]
+    const uint32_t sBar = sW + LG_SW * LG_W_BYTES + LG_SCALE_BYTES;
+    uint8_t* pS = base_ptr;
+    uint8_t* pW = base_ptr + (size_t)NS * stride;
+    float* pScale = reinterpret_cast<float*>(pW + LG_SW * LG_W_BYTES);
+    auto bar_full_w = [&](uint32_t s) { return sBar + 8u * s; };
+    auto bar_empty_w = [&](uint32_t s) { return sBar + 8u * (LG_SW + s); };
+    auto bar_full = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + s); };                  // A decoded + X landed
+    auto bar_empty = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + LG_NS_MAX + s); };     // MMAs of the stage done
+    auto bar_acc_full = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + 2 * LG_NS_MAX + s); };
+    auto bar_acc_empty = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + 2 * LG_NS_MAX + 2 + s); };
+    const uint32_t tmem_slot = sBar + 8u * LG_NBAR;
     volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(base_ptr + (tmem_slot - base));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nb = blockIdx.x;                    // 128-channel tile
-    const int m0 = blockIdx.y * TN;               // first token of this tile
     const int num_kb = K / TILE_K;
+    const int tiles_n = N / TILE_N, tiles_m = (M + TN - 1) / TN;
+    const int ntiles = tiles_n * tiles_m;
+    const uint32_t ns = (uint32_t)NS;
 
-    if (warp == 0 && lane == 0) {
+    if (threadIdx.x == 0) {
         tma_prefetch_desc(&tmap_x);
-        for (int s = 0; s < LG_STAGES; ++s) {
-            mbar_init(bar_full_w(s), 1);
-            mbar_init(bar_full_x(s), 1);
-            mbar_init(bar_decoded(s), 4);          // one arrive per decode warp
-            mbar_init(bar_empty(s), 1);
-        }
-        mbar_init(bar_acc, 1);
+        for (int s = 0; s < LG_SW; ++s) { mbar_init(bar_full_w(s), 1); mbar_init(bar_empty_w(s), 4); }
+        for (int s = 0; s < LG_NS_MAX; ++s) { mbar_init(bar_full(s), 5); mbar_init(bar_empty(s), 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(bar_acc_full(s), 1); mbar_init(bar_acc_empty(s), 4); }
         fence_barrier_init();
     }
-    if (warp == 1) tmem_alloc(tmem_slot, (uint32_t)tmem_cols);
+    if (warp == 2) tmem_alloc(tmem_slot, 512u);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     if (warp == 0) {
+        // ---------------- W producer ----------------
         if (lane == 0) {
-            const uint8_t* wsrc = packed + (size_t)nb * num_kb * TILE_BYTES;
-            // weights do not depend on the previous kernel: prefetch the first stages before the PDL wait
-            int pre = min(num_kb, LG_STAGES);
-            for (int kb = 0; kb < pre; ++kb) {
-                mbar_arrive_expect_tx(bar_full_w(kb), LG_W_BYTES);
-                tma_bulk_g2s(sW + kb * LG_W_BYTES, wsrc + (size_t)kb * TILE_BYTES, LG_W_BYTES, bar_full_w(kb));
-            }
-            pdl_wait();
-            for (int kb = 0; kb < num_kb; ++kb) {
-                const int s = kb % LG_STAGES;
-                const uint32_t ph = (kb / LG_STAGES) & 1;
-                if (kb >= LG_STAGES) {
-                    mbar_wait(bar_empty(s), ph ^ 1);
+            uint32_t it = 0;
+            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                const int nb = tile % tiles_n;
+                const uint8_t* wsrc = packed + (size_t)nb * num_kb * TILE_BYTES;
+                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                    const uint32_t s = it % LG_SW;
+                    if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar_full_w(s), LG_W_BYTES);
                     tma_bulk_g2s(sW + s * LG_W_BYTES, wsrc + (size_t)kb * TILE_BYTES, LG_W_BYTES, bar_full_w(s));
                 }
-                mbar_arrive_expect_tx(bar_full_x(s), (uint32_t)TN * TILE_K);
-                tma_tensor2d_g2s(sX + s * LG_X_BYTES, &tmap_x, kb * TILE_K, m0, bar_full_x(s));
             }
         }
     } else if (warp == 1) {
+        // ---------------- X producer ----------------
         if (lane == 0) {
-            const uint32_t idesc = umma_idesc_i8(TILE_N, TN);
-            for (int kb = 0; kb < num_kb; ++kb) {
-                const int s = kb % LG_STAGES;
-                const uint32_t ph = (kb / LG_STAGES) & 1;
-                mbar_wait(bar_decoded(s), ph);
-                mbar_wait(bar_full_x(s), ph);
-                tc_fence_after();
-                const uint64_t a_desc = umma_desc_k_sw128(sA + s * LG_A_BYTES);
-                const uint64_t b_desc = umma_desc_k_sw128(sX + s * LG_X_BYTES);
-#pragma unroll
-                for (int k = 0; k < TILE_K / 32; ++k)
-                    mma_i8_ss(tmem_base, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0);
-                mma_commit(bar_empty(s));
-            }
-            mma_commit(bar_acc);
-        }
-    } else {
-        // ---------------- decode warps ----------------
-        const int d = threadIdx.x - 64;
-        const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
-        const int g = 2 * q + p;
-        for (int kb = 0; kb < num_kb; ++kb) {
-            const int s = kb % LG_STAGES;
-            const uint32_t ph = (kb / LG_STAGES) & 1;
-            mbar_wait(bar_full_w(s), ph);
-            const uint8_t* wst = pW + s * LG_W_BYTES;
-            uint8_t* ast = pA + s * LG_A_BYTES;
-#pragma unroll
-            for (int it = 0; it < 2; ++it) {
-                const int h = p ^ it;
-                const uint4 wv = *reinterpret_cast<const uint4*>(wst + ((i32 * 2 + h) * 32 + g * 4 + t) * 16);
-                const uint32_t w4[4] = {wv.x, wv.y, wv.z, wv.w};
-                const int pos = (4 * h + t) ^ g;              // SWIZZLE_128B: 16-byte chunk index ^ (row & 7)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    uint4 o = make_uint4(decode64<0>(w4[j]), decode64<1>(w4[j]), decode64<2>(w4[j]), decode64<3>(w4[j]));
-                    *reinterpret_cast<uint4*>(ast + (i32 * 4 + j) * 1024 + g * 128 + pos * 16) = o;
+            pdl_wait();                                       // activations come from the previous kernel
+            uint32_t it = 0;
+            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                const int m0 = (tile / tiles_n) * TN;
+                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                    const uint32_t s = it % ns;
+                    if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
+                    mbar_arrive_expect_tx(bar_full(s), (uint32_t)TN * TILE_K);
+                    tma_tensor2d_g2s(sS + s * stride + LG_A_BYTES, &tmap_x, kb * TILE_K, m0, bar_full(s));
                 }
             }
-            fence_proxy_async_smem();                         // generic-proxy stores -> visible to the tensor core
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_decoded(s));
         }
-        // ---------------- epilogue ----------------
-        mbar_wait(bar_acc, 0);
-        tc_fence_after();
-        const int lq = warp & 3;                              // TMEM lane quarter this warp may read
-        const int ch = nb * TILE_N + lq * 32 + lane;
-        const float beta = (out_dtype == 2) ? 0.0f : *w_scale;
-        for (int c0 = 0; c0 < TN; c0 += 16) {
-            if (m0 + c0 >= M) break;
-            uint32_t r[16];
-            tmem_ld_32x32b_x16(tmem_base + ((uint32_t)(lq * 32) << 16) + (uint32_t)c0, r);
-            tmem_ld_wait();
+    } else if (warp == 2) {
+        // ---------------- MMA issuer: one wait, four MMAs, one commit per k block ----------------
+        if (lane == 0) {
+            const uint32_t idesc = umma_idesc_i8(TILE_N, TN);
+            uint32_t it = 0, ti = 0;
+            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++ti) {
+                const uint32_t ab = ti & 1;
+                if (ti >= 2) mbar_wait(bar_acc_empty(ab), ((ti >> 1) & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + ab * 256u;
+                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                    const uint32_t s = it % ns;
+                    mbar_wait(bar_full(s), (it / ns) & 1);
+                    tc_fence_after();
+                    LG_STAMP(0, it);
+                    const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride);
+                    const uint64_t b_desc = umma_desc_k_sw128(sS + s * stride + LG_A_BYTES);
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                const int m = m0 + c0 + i;
-                if (m < M) {
-                    const int a = (int)r[i] >> 6;
-                    const size_t o = (size_t)m * N + ch;
-                    if (out_dtype == 2) {
-                        reinterpret_cast<int*>(out)[o] = a;
+                    for (int k = 0; k < TILE_K / 32; ++k)
+                        mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0);
+                    mma_commit(bar_empty(s));
+                }
+                mma_commit(bar_acc_full(ab));
+            }
+        }
+    } else if (warp <= 10) {
+        // ---------------- decode warps: two groups of four warps take alternate k blocks ----------------
+        const int dgrp = (warp - 3) >> 2;
+        const int d = (threadIdx.x - 96) & 127;
+        const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
+        const int g = 2 * q + p;
+        uint32_t it = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                if ((int)(it & 1u) != dgrp) continue;
+                const uint32_t sw = it % LG_SW, s = it % ns;
+                mbar_wait(bar_full_w(sw), (it / LG_SW) & 1);
+                const uint8_t* wst = pW + sw * LG_W_BYTES;
+                uint4 wv[2];
+#pragma unroll
+                for (int itx = 0; itx < 2; ++itx)
+                    wv[itx] = *reinterpret_cast<const uint4*>(wst + ((i32 * 2 + (p ^ itx)) * 32 + g * 4 + t) * 16);
+                if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
+                if (threadIdx.x == 96) LG_STAMP(1, it);
+                uint8_t* ast = pS + s * stride;
+#pragma unroll
+                for (int itx = 0; itx < 2; ++itx) {
+                    const int h = p ^ itx;
+                    const uint32_t w4[4] = {wv[itx].x, wv[itx].y, wv[itx].z, wv[itx].w};
+                    const int pos = (4 * h + t) ^ g;          // SWIZZLE_128B: 16-byte chunk index ^ (row & 7)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        uint4 o = make_uint4(decode64<0>(w4[j]), decode64<1>(w4[j]), decode64<2>(w4[j]), decode64<3>(w4[j]));
+                        *reinterpret_cast<uint4*>(ast + (i32 * 4 + j) * 1024 + g * 128 + pos * 16) = o;
+                    }
+                }
+                fence_proxy_async_smem();                     // generic-proxy stores -> visible to the tensor core
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(bar_empty_w(sw));
+                    mbar_arrive(bar_full(s));
+                }
+                if (threadIdx.x == 96) LG_STAMP(2, it);
+            }
+        }
+    } else {
+        // ---------------- epilogue warps ----------------
+        const int lq = warp & 3;                              // TMEM lane quarter this warp may read
+        const float beta = (out_dtype == 2) ? 0.0f : *w_scale;
+        float* sc = pScale + lq * 256;                        // this warp's alpha_m * beta of the tile's tokens
+        const uint32_t sc_addr = sW + LG_SW * LG_W_BYTES + (uint32_t)lq * 1024u;
+        pdl_wait();                                           // x_scale comes from the previous kernel
+        uint32_t ti = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++ti) {
+            const int nb = tile % tiles_n, m0 = (tile / tiles_n) * TN;
+            const uint32_t ab = ti & 1;
+            const int ch = nb * TILE_N + lq * 32 + lane;
+            if (out_dtype != 2)
+                for (int i = lane; i < TN; i += 32) sc[i] = (m0 + i < M) ? __fmul_rn(x_scale[m0 + i], beta) : 0.0f;
+            __syncwarp();
+            mbar_wait(bar_acc_full(ab), (ti >> 1) & 1);
+            tc_fence_after();
+            if (threadIdx.x == 11 * 32) LG_STAMP(3, 2 * ti);
+            const uint32_t t_addr = tmem_base + ab * 256u + ((uint32_t)(lq * 32) << 16);
+            for (int c0 = 0; c0 < TN; c0 += 16) {
+                if (m0 + c0 >= M) break;
+                uint32_t r[16];
+                if (threadIdx.x == 11 * 32) LG_STAMP(3, 8 + 2 * (c0 >> 4));
+                tmem_ld_32x32b_x16(t_addr + (uint32_t)c0, r);
+                tmem_ld_wait();
+                if (threadIdx.x == 11 * 32) LG_STAMP(3, 9 + 2 * (c0 >> 4));
+                const int nrow = min(16, M - m0 - c0);
+                float sv[16];                                 // explicit ld.shared: cannot alias the stores below
+#pragma unroll
+                for (int i4 = 0; i4 < 4; ++i4) {
+                    const uint4 q4 = lds128_nv(sc_addr + (uint32_t)(c0 + 4 * i4) * 4u);
+                    sv[4 * i4] = __uint_as_float(q4.x); sv[4 * i4 + 1] = __uint_as_float(q4.y);
+                    sv[4 * i4 + 2] = __uint_as_float(q4.z); sv[4 * i4 + 3] = __uint_as_float(q4.w);
+                }
+                int acc[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) acc[i] = (int)r[i] >> 6;       // the decode's factor 64 leaves exactly
+                const size_t o0 = (size_t)(m0 + c0) * N + ch;
+                if (nrow == 16) {                              // full chunk: branch-free, 16 independent stores
+                    if (out_dtype == 0) {
+                        float* o = reinterpret_cast<float*>(out) + o0;
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) o[(size_t)i * N] = dequant(acc[i], sv[i]);
+                    } else if (out_dtype == 1) {
+                        __nv_bfloat16* o = reinterpret_cast<__nv_bfloat16*>(out) + o0;
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) o[(size_t)i * N] = __float2bfloat16_rn(dequant(acc[i], sv[i]));
                     } else {
-                        const float y = dequant(a, __fmul_rn(x_scale[m], beta));
-                        if (out_dtype == 0) reinterpret_cast<float*>(out)[o] = y;
-                        else reinterpret_cast<__nv_bfloat16*>(out)[o] = __float2bfloat16_rn(y);
+                        int* o = reinterpret_cast<int*>(out) + o0;
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) o[(size_t)i * N] = acc[i];
+                    }
+                } else {                                       // ragged tail of M
+                    for (int i = 0; i < nrow; ++i) {
+                        const size_t o = o0 + (size_t)i * N;
+                        int a = 0; float sc_i = 0.0f;
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) if (j == i) { a = acc[j]; sc_i = sv[j]; }
+                        if (out_dtype == 0) reinterpret_cast<float*>(out)[o] = dequant(a, sc_i);
+                        else if (out_dtype == 1) reinterpret_cast<__nv_bfloat16*>(out)[o] = __float2bfloat16_rn(dequant(a, sc_i));
+                        else reinterpret_cast<int*>(out)[o] = a;
                     }
                 }
             }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_acc_empty(ab));    // this TMEM buffer may be overwritten
+            if (threadIdx.x == 11 * 32) LG_STAMP(3, 2 * ti + 1);
         }
     }
     pdl_launch_dependents();
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem_base, (uint32_t)tmem_cols);
+    if (warp == 2) tmem_dealloc(tmem_base, 512u);
 }
 
 // ---------------------------------------------------------------- host side
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static int env_tn() {
+    const char* v = std::getenv("VLA_TUNE_TN");                 // tuning aid: force the token-tile width
+    return v ? std::atoi(v) : 0;
+}
 
 static EncodeTiledFn get_encode() {
     static EncodeTiledFn fn = nullptr;
@@ -187,19 +287,37 @@ static EncodeTiledFn get_encode() {
     return fn;
 }
 
-static int pick_tn(int M) {
-    int tiles = (M + 255) / 256;
-    int tn = ((M + tiles - 1) / tiles + 15) / 16 * 16;
-    return tn < 16 ? 16 : tn;
+// Token-tile width TN (multiple of 16, <= 256) for a persistent grid of `sms` CTAs: minimise
+//   waves * max(MMA cycles per k block = 2*TN, decode cycles per k block ~ 220)
+// where waves = ceil(tiles / sms); ties go to the wider tile (fewer re-decodes of the same weights).
+static int pick_tn(int M, int N, int sms) {
+    int best = 16;
+    double best_cost = 1e30;
+    for (int tn = 16; tn <= 256; tn += 16) {
+        const int tiles_m = (M + tn - 1) / tn;
+        if (tn > 16 && (tiles_m * (tn - 16) >= M)) continue;          // a narrower tile covers M with the same count
+        const long tiles = (long)tiles_m * (N / TILE_N);
+        const long waves = (tiles + sms - 1) / sms;
+        const double per_kb = (2.0 * tn > 220.0) ? 2.0 * tn : 220.0;
+        const double cost = (double)waves * per_kb;
+        if (cost <= best_cost) { best_cost = cost; best = tn; }
+    }
+    return best;
 }
 
 cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
                               int M, int N, int K, void* out, int out_dtype, cudaStream_t s) {
     EncodeTiledFn enc = get_encode();
     if (!enc) return cudaErrorNotSupported;
-    const int TN = pick_tn(M);
-    int cols = 32;
-    while (cols < TN) cols *= 2;
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (sms <= 0) sms = 148;
+    }
+    static const int tune_tn = env_tn();
+    const int TN = tune_tn > 0 ? tune_tn : pick_tn(M, N, sms);
 
     CUtensorMap tm;
     cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)M};
@@ -213,14 +331,18 @@ cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const in
 
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
+    const int ntiles = (N / TILE_N) * ((M + TN - 1) / TN);
+    int NS = LG_STAGE_REGION / (int)lg_stage_stride(TN);
+    if (NS > LG_NS_MAX) NS = LG_NS_MAX;
+    const int smem = NS * (int)lg_stage_stride(TN) + LG_FIXED_SMEM;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(N / TILE_N), (unsigned)((M + TN - 1) / TN));
+    cfg.gridDim = dim3((unsigned)(ntiles < sms ? ntiles : sms));
     cfg.blockDim = dim3(LG_THREADS);
-    cfg.dynamicSmemBytes = LG_SMEM;
+    cfg.dynamicSmemBytes = (size_t)smem;
     cfg.stream = s;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -229,7 +351,7 @@ cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const in
     cfg.numAttrs = 1;
     count_launch();
     return cudaLaunchKernelEx(&cfg, gemm_large_kernel, tm, (const uint8_t*)packed, w_scale, x_scale, out,
-                              M, N, K, TN, cols, out_dtype);
+                              M, N, K, TN, NS, out_dtype);
 }
 
 // ---------------------------------------------------------------- INT8 tensor-pipe issue-rate probe
@@ -278,5 +400,10 @@ cudaError_t run_i8_mma_probe(int ctas, int mmas_per_cta, float* ms_out) {
     cudaEventDestroy(b);
     return e;
 }
+
+#ifdef VLA_LG_DEBUG
+extern "C" int vla_debug_set_lg(int v) { return (int)cudaMemcpyToSymbol(g_lg_dbg, &v, sizeof(int)); }
+extern "C" int vla_debug_get_lg_trace(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_lg_trace, sizeof(g_lg_trace)); }
+#endif
 
 }  // namespace vla
