@@ -1,0 +1,58 @@
+"""Host-side validation of the program API (no GPU needed): vla_program_bytes / vla_program_build answer from the
+host before any launch, and there is no CPU fallback behind vla_program_run."""
+import pytest
+
+
+@pytest.fixture(scope="module")
+def vla():
+    from paper_2606_08094_b200 import binding
+    return binding
+
+
+FAKE = 0x10000   # 256-byte aligned non-NULL "pointer"; never dereferenced because validation comes first
+
+
+def stage(M=8, K=2560, N=2560, depends=0, n=1, dtype=1):
+    return dict(x=FAKE, M=M, K=K, depends=depends,
+                linears=[dict(packed=FAKE, w_scale=FAKE, out=FAKE, N=N, out_dtype=dtype) for _ in range(n)])
+
+
+def test_program_bytes_counts_tables_counters_and_quantised_activations(vla):
+    one = vla.vla_program_bytes([stage()])
+    assert one % 256 == 0 and one >= 8 * 2560 + 8 * 4
+    two = vla.vla_program_bytes([stage(), stage(M=16, K=6912, depends=1)])
+    assert two >= one + 16 * 6912
+
+
+@pytest.mark.parametrize("bad", [dict(M=0), dict(M=17), dict(K=100), dict(K=8192 + 128), dict(N=100), dict(N=0),
+                                 dict(depends=2), dict(n=0), dict(n=17), dict(dtype=3)])
+def test_invalid_stage_gives_zero_bytes(vla, bad):
+    assert vla.vla_program_bytes([stage(**bad)]) == 0
+
+
+def test_descriptor_capacity_is_enforced(vla):
+    # 30 layers x 4 stages with 7 linears fit (BASELINE.json configs[3]); ten times that does not
+    layer = [stage(n=3), stage(depends=1), stage(n=2, depends=1), stage(K=6912, depends=1)]
+    assert vla.vla_program_bytes(layer * 30) > 0
+    assert vla.vla_program_bytes(layer * 300) == 0
+
+
+def test_build_and_run_validate_on_the_host(vla):
+    arr, _keep = vla._marshal_stages([stage()])
+    L = vla._lib
+    assert L.vla_program_build(arr, 1, None, 1 << 20, None) == vla.VLA_ERR_NULL
+    assert L.vla_program_build(arr, 1, FAKE + 16, 1 << 20, None) == vla.VLA_ERR_ALIGN
+    assert L.vla_program_build(arr, 1, FAKE, 16, None) == vla.VLA_ERR_WORKSPACE
+    assert L.vla_program_build(None, 1, FAKE, 1 << 20, None) == vla.VLA_ERR_NULL
+    assert L.vla_program_run(None, None) == vla.VLA_ERR_NULL
+    assert L.vla_program_run(FAKE, None) == vla.VLA_ERR_VALUE          # never compiled
+    assert L.vla_program_release(FAKE) == vla.VLA_ERR_VALUE
+    assert L.vla_program_run_host(FAKE, None, 1, None, 0, None) == vla.VLA_ERR_NULL
+
+
+def test_no_gpu_means_arch_error(vla):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    arr, _keep = vla._marshal_stages([stage()])
+    assert vla._lib.vla_program_build(arr, 1, FAKE, 1 << 20, None) == vla.VLA_ERR_ARCH
