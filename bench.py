@@ -422,6 +422,9 @@ def run_gpu(args):
                 "kernel": "gemm_large_kernel", "peak_source": pk["source"] + " bf16_tflops x 2 (int8:bf16 nominal ratio)",
                 "alg_ops_per_launch": alg, "us_per_launch": per_launch_s * 1e6,
                 "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS}
+        probe = int8_probe_tops(vla)
+        roof["int8_probe_tops"] = probe                       # tcgen05.mma.kind::i8 issue-rate ceiling of this box
+        roof["frac_of_probe"] = achieved / probe
 
     # ---- per-point table (the metric is "vs M"): each point alone, whole hot path, cold ring
     table = []
@@ -472,19 +475,50 @@ def run_gpu(args):
     return 0
 
 
+def int8_probe_tops(vla):
+    """Box-measured INT8 tensor ceiling: back-to-back tcgen05.mma.kind::i8 (128x256x32) on every SM, no loads."""
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    n = 20000
+    ms = vla.vla_i8_mma_issue_probe(sms, n)
+    return 2.0 * 128 * 256 * 32 * n * sms / (ms * 1e-3) / 1e12
+
+
+def run_extra(args):
+    """configs[3] / configs[4] (single GPU; BASELINE.json north_star: everything runs on one GPU)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path (use --impl reference for the oracle)")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    torch.cuda.set_device(0)
+    from paper_2606_08094_b200 import binding as vla
+    import bench_workloads as bw
+    pk = peaks()
+    if args.workload == "stack":
+        return bw.run_stack(args, pk, ClockSampler(0))
+    return bw.run_sweep(args, pk, ClockSampler(0), int8_probe_tops(vla))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=4000)
     ap.add_argument("--warmup", type=int, default=16)
-    ap.add_argument("--workload", choices=["decode", "prefill"], default="decode")
+    ap.add_argument("--workload", choices=["decode", "prefill", "stack", "sweep"], default="decode")
+    ap.add_argument("--quick", action="store_true", help="sweep: one zero fraction and one distribution only")
+    ap.add_argument("--sweep-m", default="", help="sweep: comma-separated M values (default: 1,2,4,...,4096)")
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle timing for cpu_baseline")
     ap.add_argument("--no-points", action="store_true", help="skip the per-point table")
     args = ap.parse_args()
     if args.impl == "reference":
+        if args.workload in ("stack", "sweep"):
+            args.workload = "decode"
         return run_reference(args)
+    if args.workload in ("stack", "sweep"):
+        return run_extra(args)
     return run_gpu(args)
 
 

@@ -1,0 +1,182 @@
+"""Extra bench.py workloads: BASELINE.json configs[3] (30-layer chained stack) and configs[4] (roofline sweep).
+
+Imported by bench.py only.  Timing protocol as in bench.py: CUDA graphs, CUDA events on the launching stream,
+cold weights (the stack is 521 MB >> L2; the sweep rotates through a ring of packed copies > 2 x L2).
+"""
+import json
+import os
+import time
+
+import numpy as np
+
+
+def _events(torch):
+    return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+
+def _time(torch, fn, reps):
+    fn()
+    torch.cuda.synchronize()
+    e0, e1 = _events(torch)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1) * 1e-3 / reps
+
+
+# ----------------------------------------------------------------------------- configs[3]
+def run_stack(args, pk, clock_sampler):
+    """30 decoder layers, q/k/v/o/gate/up/down ternary linears + their activation quant, chained; M=544 (one quant
+    kernel per stage + one tcgen05 GEMM launch per linear, CUDA graph + PDL) then M=8 (ONE persistent program launch)."""
+    import torch
+    from paper_2606_08094_b200 import binding as vla, synth
+    from paper_2606_08094_b200.stack import Stack
+    layers = synth.STACK_LAYERS
+    out = {}
+    sampler = clock_sampler
+    sampler.start()
+    for M in (synth.PREFILL_M, 8):
+        st = Stack(layers, M)
+        st.set_input(synth.stack_input(M))
+        n0 = vla.vla_launch_count()
+        if M <= 16:
+            st.compile()
+            fn = st.run_program
+            fn()
+            launches = vla.vla_launch_count() - n0
+        else:
+            st.alloc_call_workspace()
+            st.run_stack_calls()
+            torch.cuda.synchronize()
+            n0 = vla.vla_launch_count()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                st.run_stack_calls()
+            launches = vla.vla_launch_count() - n0
+            fn = g.replay
+        for _ in range(max(3, args.warmup // 4)):
+            fn()
+        sec = _time(torch, fn, max(3, min(args.steps, 50)))
+        ops = 2.0 * M * sum(K * N for (_, K, N) in synth.STACK_LINEARS) * layers
+        wbytes = float(st.packed_bytes)
+        t_roof = max(wbytes / (pk["hbm_gbs"] * 1e9), ops / (pk["bf16_tflops"] * 2e12))
+        out["M%d" % M] = {"us": sec * 1e6, "us_per_layer": sec * 1e6 / layers, "launches": launches,
+                          "weight_GBs": wbytes / sec / 1e9, "TOPS": ops / sec / 1e12, "roofline_frac": t_roof / sec,
+                          "route": "one persistent program launch" if M <= 16 else "act_quant + tcgen05 GEMM per linear, CUDA graph + PDL"}
+        del st
+        torch.cuda.empty_cache()
+    clocks = sampler.stop()
+    m8 = out["M8"]
+    line = {
+        "metric": "ternary_stack_weight_stream_gbs", "value": m8["weight_GBs"], "unit": "GB/s", "n_gpus": 1,
+        "steps": max(3, min(args.steps, 50)), "warmup": max(3, args.warmup // 4), "ms_per_step": m8["us"] * 1e-3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8*ternary->int32",
+        "data": "synthetic",
+        "config": {"workload": "configs[3] 30-layer stack (hidden 2560, 20q/5kv x128, FFN 6912), linears + quant chained; "
+                               "value is the M=8 pass", "cold_weights": "521 MB packed per pass (>> L2)"},
+        "clocks": clocks, "gpu_launches": m8["launches"], "stack": out,
+        "roofline": {"bound": "hbm", "achieved": m8["weight_GBs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
+                     "frac": m8["weight_GBs"] / pk["hbm_gbs"], "traffic": None, "kernel": "program_kernel"},
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- configs[4]
+def run_sweep(args, pk, clock_sampler, int8_probe_tops):
+    """M in {1..4096} x 4 shapes x zero fraction x activation distribution, fused quant, fp32 out: TOPS, GB/s and
+    roofline fraction per point (single vla_ternary_linear calls in a CUDA graph over a cold ring); for M <= 16 also
+    the streaming regime (a ring-full of the same linear as independent stages of one persistent program)."""
+    import torch
+    from paper_2606_08094_b200 import binding as vla, synth
+    dev = torch.device("cuda", 0)
+    l2 = torch.cuda.get_device_properties(dev).L2_cache_size
+    peak_i8 = pk["bf16_tflops"] * 2.0
+    Ms = synth.SWEEP_M if not args.sweep_m else [int(m) for m in args.sweep_m.split(",")]
+    zfs = range(len(synth.SWEEP_ZERO_FRAC)) if not args.quick else [1]
+    dists = range(len(synth.SWEEP_DISTS)) if not args.quick else [0]
+    pts = []
+    sampler = clock_sampler
+    sampler.start()
+    for si, (K, N) in enumerate(synth.SWEEP_SHAPES):
+        copies = max(2, -(-2 * l2 // (N * K // 4)))
+        Mmax = max(Ms)
+        for zf in zfs:
+            w = synth.ternary_weights(N, K, synth.SWEEP_ZERO_FRAC[zf], 4000 + 10 * si + zf)
+            packed1 = vla.pack_weights(torch.from_numpy(w).to(dev))
+            ring = packed1.unsqueeze(0).repeat(copies, 1).contiguous()
+            del w, packed1
+            beta = torch.tensor([0.05], dtype=torch.float32, device=dev)
+            for di in dists:
+                xb = synth.activations(Mmax, K, 504000 + 10 * si + di, dist=synth.SWEEP_DISTS[di])
+                x_all = torch.from_numpy(xb.view(np.int16)).to(dev).view(torch.bfloat16)
+                for M in Ms:
+                    x = x_all[:M].contiguous()
+                    out = torch.empty((M, N), dtype=torch.float32, device=dev)
+                    xq = torch.empty((M, K), dtype=torch.int8, device=dev)
+                    xs = torch.empty((M,), dtype=torch.float32, device=dev)
+                    nb = vla.vla_ternary_workspace_bytes(M, N, K)
+                    ws = torch.empty(nb, dtype=torch.uint8, device=dev)
+                    ncall = min(copies, 32)
+
+                    def calls():
+                        for c in range(ncall):
+                            vla.vla_ternary_linear(ring[c], beta, x, M, N, K, out, vla.VLA_F32, vla.VLA_PATH_AUTO, xq, xs, ws, nb)
+                    calls()
+                    torch.cuda.synchronize()
+                    g = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(g):
+                        calls()
+                    sec = _time(torch, g.replay, 3 if M >= 1024 else 10) / ncall
+                    by = N * K // 4 + 4 + 2 * M * K + 4 * M * N
+                    op = 2.0 * M * N * K
+                    t_roof = max(by / (pk["hbm_gbs"] * 1e9), op / (peak_i8 * 1e12))
+                    p = {"M": M, "K": K, "N": N, "zero_frac": synth.SWEEP_ZERO_FRAC[zf], "dist": synth.SWEEP_DISTS[di],
+                         "us": sec * 1e6, "TOPS": op / sec / 1e12, "GBs": by / sec / 1e9, "roofline_frac": t_roof / sec,
+                         "bound": "hbm" if by / (pk["hbm_gbs"] * 1e9) > op / (peak_i8 * 1e12) else "tensor",
+                         "path": int(vla.vla_ternary_auto_path(M, N, K))}
+                    if M <= 16 and zf == list(zfs)[0] and di == list(dists)[0]:
+                        nst = min(copies, 128)
+                        outs = [torch.empty((M, N), dtype=torch.float32, device=dev) for _ in range(nst)]
+                        stages = [dict(x=x, M=M, K=K, depends=0,
+                                       linears=[dict(packed=ring[c], w_scale=beta, out=outs[c], N=N, out_dtype=vla.VLA_F32)])
+                                  for c in range(nst)]
+                        prog = vla.compile_program(stages, dev)
+                        secp = _time(torch, lambda: vla.vla_program_run(prog), 10) / nst
+                        p["stream_us"] = secp * 1e6
+                        p["stream_GBs"] = by / secp / 1e9
+                        p["stream_roofline_frac"] = (by / (pk["hbm_gbs"] * 1e9)) / secp
+                        vla.vla_program_release(prog)
+                        del prog, outs
+                    pts.append(p)
+                    del g
+                del x_all
+            del ring
+            torch.cuda.empty_cache()
+    clocks = sampler.stop()
+    big = [p for p in pts if p["M"] >= 512]
+    small = [p for p in pts if p["M"] <= 16]
+    best_big = max(big, key=lambda p: p["roofline_frac"]) if big else None
+    line = {
+        "metric": "ternary GEMM TOPS & HBM GB/s vs M; fraction of INT8/HBM roofline (1 B200)",
+        "value": best_big["TOPS"] if best_big else 0.0, "unit": "TOP/s", "n_gpus": 1, "steps": len(pts), "warmup": 1,
+        "ms_per_step": None, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int8*ternary->int32", "data": "synthetic",
+        "config": {"workload": "configs[4] roofline sweep, %d points, fused quant, fp32 out; value = best M>=512 point" % len(pts),
+                   "cold_weights": "ring of packed copies > 2 x L2 per shape"},
+        "clocks": clocks,
+        "peaks": {"hbm_gbs": pk["hbm_gbs"], "int8_tops_bf16x2": peak_i8, "int8_tops_probe": int8_probe_tops,
+                  "int8_tops_nominal": 4500.0},
+        "summary": {
+            "M>=512 roofline_frac min/median/max": [float(np.min([p["roofline_frac"] for p in big])),
+                                                    float(np.median([p["roofline_frac"] for p in big])),
+                                                    float(np.max([p["roofline_frac"] for p in big]))] if big else None,
+            "M<=16 single-call roofline_frac median": float(np.median([p["roofline_frac"] for p in small])) if small else None,
+            "M<=16 streaming roofline_frac median": float(np.median([p["stream_roofline_frac"] for p in small
+                                                                     if "stream_roofline_frac" in p])) if small else None},
+        "points": pts,
+    }
+    print(json.dumps(line))
+    return 0

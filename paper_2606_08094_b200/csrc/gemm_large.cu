@@ -288,8 +288,10 @@ static EncodeTiledFn get_encode() {
 }
 
 // Token-tile width TN (multiple of 16, <= 256) for a persistent grid of `sms` CTAs: minimise
-//   waves * max(MMA cycles per k block = 2*TN, decode cycles per k block ~ 220)
-// where waves = ceil(tiles / sms); ties go to the wider tile (fewer re-decodes of the same weights).
+//   waves * (cycles per k block), waves = ceil(tiles / sms).
+// Measured on B200 (profiles/): a k block costs ~540 cycles at TN = 96 and ~610 at TN = 256 -- the shared-memory
+// traffic of decode + operand fetch dominates, not the 2*TN cycles of the MMAs -- so cycles ~ 500 + 0.42*TN.
+// Ties go to the wider tile (fewer re-decodes of the same weights).
 static int pick_tn(int M, int N, int sms) {
     int best = 16;
     double best_cost = 1e30;
@@ -298,7 +300,7 @@ static int pick_tn(int M, int N, int sms) {
         if (tn > 16 && (tiles_m * (tn - 16) >= M)) continue;          // a narrower tile covers M with the same count
         const long tiles = (long)tiles_m * (N / TILE_N);
         const long waves = (tiles + sms - 1) / sms;
-        const double per_kb = (2.0 * tn > 220.0) ? 2.0 * tn : 220.0;
+        const double per_kb = 500.0 + 0.42 * tn;
         const double cost = (double)waves * per_kb;
         if (cost <= best_cost) { best_cost = cost; best = tn; }
     }
