@@ -6,11 +6,14 @@
 //   bits [8b+2i+1 : 8b+2i], so that   (word << (6-2i)) & 0xC0C0C0C0   is four int8 lanes equal to
 //   64*q for k_local = 4i..4i+3 (2 ALU ops per 4 weights, already signed; the factor 64 is removed
 //   exactly by an arithmetic shift of the int32 accumulator).
-//   Words are ordered [N/128][K/128][i32:4][h:2][lane:32][j:4] with
-//       n = 128*nb + 32*i32 + 8*j + g,   k = 128*kb + 64*h + 16*t + k_local,   lane = 4*g + t.
-//   -> a 128(n) x 128(k) tile is 4 KiB contiguous (one TMA bulk copy for the tcgen05 path);
+//   Words are ordered [N/32][K/128][h:2][lane:32][j:4] with
+//       n = 32*n32 + 8*j + g,   k = 128*kb + 64*h + 16*t + k_local,   lane = 4*g + t.
 //   -> a 32(n) x 64(k) block is 512 B contiguous, one 128-bit load per lane, and the four words a
-//      lane gets are exactly the A fragments of mma.m16n8k32 for two 16-channel tiles.
+//      lane gets are exactly the A fragments of mma.m16n8k32 for two 16-channel tiles;
+//   -> a GRANULE (32 channels x all of K) is ONE contiguous run of 8*K bytes, so the persistent kernel streams it
+//      with bulk copies of up to 16 KiB (measured on B200: 1 KiB cp.async.bulk copies cap the chip at 3.7 TB/s,
+//      >= 4 KiB copies reach 6.2-6.7 TB/s);
+//   -> a 128(n) x 128(k) tile of the tcgen05 path is four 1 KiB pieces, 8*K bytes apart.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -25,8 +28,7 @@ constexpr int TILE_BYTES = TILE_N * TILE_K / 4;   // 4096
 
 // byte offset of the 512-byte block holding channels [32*n32, +32) and k in [64*k64, +64)
 __host__ __device__ inline size_t block_offset(int n32, int k64, int K) {
-    int nb = n32 >> 2, i32 = n32 & 3, kb = k64 >> 1, h = k64 & 1;
-    return ((size_t)(nb * (K / TILE_K) + kb) * 8 + (i32 * 2 + h)) * 512;
+    return ((size_t)n32 * (K / BLK_K) + k64) * 512;
 }
 
 // four int8 lanes of 64*q for k_local = 4i .. 4i+3

@@ -8,7 +8,7 @@
 //   MMA operand B = int8 activations [TN tok  x 128 k] int8, K-major, SWIZZLE_128B  (written by TMA)
 //   D (TMEM)      = int32 [128 lanes = channels] x [TN columns = tokens], TWO buffers (columns 0.. and 256..)
 // Warp roles (15 warps):
-//   warp 0       W producer: cp.async.bulk of the 4 KiB packed weight tile per k block, 8-deep ring (weights never
+//   warp 0       W producer: cp.async.bulk of the four 1 KiB pieces of the packed weight tile per k block, 6-deep ring (weights never
 //                depend on the previous kernel, so this starts before griddepcontrol.wait)
 //   warp 1       X producer: tensor-map (TMA) load of the [TN x 128] activation tile per k block, 4-deep ring
 //   warp 2       TMEM allocator; one lane issues tcgen05.mma.cta_group::1.kind::i8 (4 x K=32 per k block)
@@ -96,16 +96,18 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
 
     if (warp == 0) {
         // ---------------- W producer ----------------
-        if (lane == 0) {
+        // a 128 x 128 tile is four 1 KiB pieces (one per 32-channel group), 8*K bytes apart: lanes 0-3 copy one each
+        if (lane < 4) {
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const int nb = tile % tiles_n;
-                const uint8_t* wsrc = packed + (size_t)nb * num_kb * TILE_BYTES;
+                const uint8_t* wsrc = packed + (size_t)(nb * 4 + lane) * num_kb * 1024;
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
                     const uint32_t s = it % LG_SW;
                     if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
-                    mbar_arrive_expect_tx(bar_full_w(s), LG_W_BYTES);
-                    tma_bulk_g2s(sW + s * LG_W_BYTES, wsrc + (size_t)kb * TILE_BYTES, LG_W_BYTES, bar_full_w(s));
+                    if (lane == 0) mbar_arrive_expect_tx(bar_full_w(s), LG_W_BYTES);
+                    __syncwarp(0xF);
+                    tma_bulk_g2s(sW + s * LG_W_BYTES + lane * 1024, wsrc + (size_t)kb * 1024, 1024, bar_full_w(s));
                 }
             }
         }

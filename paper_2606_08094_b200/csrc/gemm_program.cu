@@ -35,11 +35,15 @@ constexpr int PG_W = 16;                         // consumer warps
 constexpr int PG_CONSUMERS = PG_W * 32;          // 512 threads
 constexpr int PG_THREADS = PG_CONSUMERS + 32;
 constexpr int PG_SLOT_BYTES = 16384;             // 16 pieces of 1 KiB = 32 blocks of 32 ch x 64 k
-constexpr int PG_NSLOT = 11;
+constexpr int PG_XHI_BYTES = 65536;              // M <= 16 variant: B fragments of tokens 8-15 (8 * K bytes, K <= 8192)
+__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 11 : 7; }
 constexpr int PG_DESC_BYTES = 15360;             // stage + linear descriptors cached in shared memory
 constexpr int PG_NBMAX = 8;                      // k blocks per warp per granule  ->  K <= 8192
 constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 8448 ints = 33 792 B
-constexpr int PG_SMEM = PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + 2 * PG_NSLOT * 8 + 64 + 128;
+__host__ __device__ constexpr int pg_smem(int maxmt) {
+    return pg_nslot(maxmt) * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + (maxmt == 1 ? 0 : PG_XHI_BYTES) +
+           2 * pg_nslot(maxmt) * 8 + 64 + 128;
+}
 
 #ifdef VLA_PROG_TRACE
 // debug-only (never defined in the product build): per-CTA globaltimer stamps, read back by vla_debug_read_trace
@@ -88,6 +92,7 @@ __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uin
 }
 
 // ---------------------------------------------------------------- producer warp
+template <int NSLOT>
 __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, int cta,
                                          int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty) {
     uint32_t slot = 0, round = 0;
@@ -101,16 +106,16 @@ __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stage
             for (int j = 1; j < st.n_lin; ++j)
                 if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
             const int n32 = gi - lins[l].gran_begin;
-            const uint8_t* src = lins[l].packed + ((size_t)(n32 >> 2) * KB * 8 + (size_t)(n32 & 3) * 2) * 512;
+            const uint8_t* src = lins[l].packed + (size_t)n32 * KB * 1024;      // the granule is one contiguous run
             for (int p0 = 0; p0 < KB; p0 += 16) {
                 const int np = min(16, KB - p0);
                 if (round > 0) mbar_wait(bar_empty + 8u * slot, (round - 1) & 1);
-                if (lane == 0) mbar_arrive_expect_tx(bar_full + 8u * slot, (uint32_t)np * 1024u);
-                __syncwarp();
-                if (lane < np)
-                    tma_bulk_g2s(ring + slot * PG_SLOT_BYTES + lane * 1024, src + (size_t)(p0 + lane) * TILE_BYTES, 1024,
+                if (lane == 0) {                              // one bulk copy of up to 16 KiB per chunk
+                    mbar_arrive_expect_tx(bar_full + 8u * slot, (uint32_t)np * 1024u);
+                    tma_bulk_g2s(ring + slot * PG_SLOT_BYTES, src + (size_t)p0 * 1024, (uint32_t)np * 1024u,
                                  bar_full + 8u * slot);
-                if (++slot == PG_NSLOT) { slot = 0; ++round; }
+                }
+                if (++slot == NSLOT) { slot = 0; ++round; }
             }
         }
     }
@@ -156,8 +161,14 @@ __device__ __forceinline__ void quant_owned_rows(const DevProg& P, int s, const 
 
 // ---------------------------------------------------------------- one stage's granules on the consumer warps
 // int8 activations of this warp's k blocks (kq = 16 i + w), as mma B fragments, in registers for the whole stage
+// Tokens 0-7 stay in registers (xv); in the M <= 16 variant the fragments of tokens 8-15 go to this thread's private
+// 16-byte slots of the shared-memory region xhi (64 registers of fragments would spill, and with 227 KB of shared
+// memory there is no L1 left to catch spills).
+__device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 template <int MAXMT>
-__device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)[PG_NBMAX][MAXMT]) {
+__device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)[PG_NBMAX], uint32_t xhi) {
     const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int K = st.K, nblk = K / BLK_K;
     const int8_t* xq = reinterpret_cast<const int8_t*>(st.xq);
@@ -166,17 +177,19 @@ __device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)
 #pragma unroll
         for (int mt = 0; mt < MAXMT; ++mt) {
             const int kq = i * PG_W + w, tok = mt * 8 + g;
-            xv[i][mt] = (kq < nblk && tok < st.M)
-                            ? __ldcg(reinterpret_cast<const uint4*>(xq + (size_t)tok * K + kq * BLK_K + t * 16))
-                            : make_uint4(0, 0, 0, 0);
+            const uint4 v = (kq < nblk && tok < st.M)
+                                ? __ldcg(reinterpret_cast<const uint4*>(xq + (size_t)tok * K + kq * BLK_K + t * 16))
+                                : make_uint4(0, 0, 0, 0);
+            if (mt == 0) xv[i] = v;
+            else if (kq < nblk) sts128(xhi + (uint32_t)(kq * 32 + lane) * 16u, v);
         }
 }
 
 // cta / G: rank and size of the stage's CTA group
-template <int MT, int MAXMT>
+template <int MT, int NSLOT>
 __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& st, int cta, int G,
                                            int tid, uint32_t ring, int* red, uint32_t bar_full, uint32_t bar_empty,
-                                           uint4 (&xv)[PG_NBMAX][MAXMT], uint32_t& slot, uint32_t& phase, uint32_t& gcount
+                                           uint4 (&xv)[PG_NBMAX], uint32_t xhi, uint32_t& slot, uint32_t& phase, uint32_t& gcount
 #ifdef VLA_PROG_TRACE
                                            , int& tr_n
 #endif
@@ -228,21 +241,24 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
                                                                : make_uint4(0, 0, 0, 0);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_empty + 8u * slot);       // release: ordered after the loads above
-                if (++slot == PG_NSLOT) { slot = 0; phase ^= 1; }
+                if (++slot == NSLOT) { slot = 0; phase ^= 1; }
 #pragma unroll
                 for (int ii = 0; ii < 2; ++ii) {
                     const int i = 2 * ck + ii;
                     if (i * PG_W + w < nblk) {
                         const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
+                        uint4 xh = make_uint4(0, 0, 0, 0);    // tokens 8-15 of this block (M <= 16 variant)
+                        if (MT == 2) xh = lds128(xhi + (uint32_t)((i * PG_W + w) * 32 + lane) * 16u);
 #pragma unroll
                         for (int c = 0; c < 2; ++c) {
                             const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];     // channels 16c+g and 16c+g+8
                             const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
                             const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
-#pragma unroll
-                            for (int mt = 0; mt < MT; ++mt) {
-                                mma_m16n8k32_s8_nv(acc[c][mt], a0, a1, a2, a3, xv[i][mt].x, xv[i][mt].y);
-                                mma_m16n8k32_s8_nv(acc[c][mt], e0, e1, e2, e3, xv[i][mt].z, xv[i][mt].w);
+                            mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xv[i].x, xv[i].y);
+                            mma_m16n8k32_s8_nv(acc[c][0], e0, e1, e2, e3, xv[i].z, xv[i].w);
+                            if (MT == 2) {
+                                mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh.x, xh.y);
+                                mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh.z, xh.w);
                             }
                         }
                     }
@@ -296,15 +312,18 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
     const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
     const uint32_t ring = base;
-    int* red = reinterpret_cast<int*>(base_ptr + PG_NSLOT * PG_SLOT_BYTES);
-    uint8_t* desc = base_ptr + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4;
-    const uint32_t bar_full = base + PG_NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES;
-    const uint32_t bar_empty = bar_full + 8u * PG_NSLOT;
-    float* s_max = reinterpret_cast<float*>(desc + PG_DESC_BYTES + 16 * PG_NSLOT);
+    constexpr int NSLOT = pg_nslot(MAXMT);
+    constexpr int XHI = (MAXMT == 1) ? 0 : PG_XHI_BYTES;
+    int* red = reinterpret_cast<int*>(base_ptr + NSLOT * PG_SLOT_BYTES);
+    uint8_t* desc = base_ptr + NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4;
+    const uint32_t xhi = base + NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES;
+    const uint32_t bar_full = xhi + XHI;
+    const uint32_t bar_empty = bar_full + 8u * NSLOT;
+    float* s_max = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT);
 
     const int tid = threadIdx.x, cta = blockIdx.x, G = gridDim.x;
     if (tid == 0) {
-        for (int s = 0; s < PG_NSLOT; ++s) {
+        for (int s = 0; s < NSLOT; ++s) {
             mbar_init(bar_full + 8u * s, 1);
             mbar_init(bar_empty + 8u * s, PG_W);
         }
@@ -325,14 +344,14 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
     const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
 
     if (tid >= PG_CONSUMERS) {
-        producer(P, stages, lins, cta, tid & 31, ring, bar_full, bar_empty);
+        producer<NSLOT>(P, stages, lins, cta, tid & 31, ring, bar_full, bar_empty);
         return;
     }
 #ifdef VLA_PROG_TRACE
     int tr_n = 0;
 #endif
     TRACE();
-    uint4 xv[PG_NBMAX][MAXMT];
+    uint4 xv[PG_NBMAX];
     uint32_t slot = 0, phase = 0, gcount = 0;
     for (int s = 0; s < P.n_stages; ++s) {
         const DevStage& st = stages[s];
@@ -343,11 +362,11 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
             if (tid == 0) spin_until(P.b2 + s, (unsigned)st.M);
             consumer_bar();
             TRACE();
-            load_xv<MAXMT>(st, tid, xv);
+            load_xv<MAXMT>(st, tid, xv, xhi);
             if (MAXMT == 1 || st.M <= 8)
-                stage_gemm<1, MAXMT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, slot, phase, gcount TRARG);
+                stage_gemm<1, NSLOT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
             else
-                stage_gemm<MAXMT, MAXMT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, slot, phase, gcount TRARG);
+                stage_gemm<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
             TRACE();
         }
         if (st.publish) {                                    // end of a phase that a later phase reads from
@@ -373,14 +392,14 @@ size_t program_desc_capacity() { return PG_DESC_BYTES; }
 cudaError_t launch_program(const void* prog_dev, int grid, int max_m, cudaStream_t s) {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(program_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, PG_SMEM);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(program_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, PG_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(program_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg_smem(1));
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(program_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg_smem(2));
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     count_launch();
-    if (max_m <= 8) program_kernel<1><<<grid, PG_THREADS, PG_SMEM, s>>>(reinterpret_cast<const DevProg*>(prog_dev));
-    else            program_kernel<2><<<grid, PG_THREADS, PG_SMEM, s>>>(reinterpret_cast<const DevProg*>(prog_dev));
+    if (max_m <= 8) program_kernel<1><<<grid, PG_THREADS, pg_smem(1), s>>>(reinterpret_cast<const DevProg*>(prog_dev));
+    else            program_kernel<2><<<grid, PG_THREADS, pg_smem(2), s>>>(reinterpret_cast<const DevProg*>(prog_dev));
     return cudaGetLastError();
 }
 

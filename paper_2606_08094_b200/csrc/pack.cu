@@ -9,13 +9,12 @@ namespace vla {
 __device__ __forceinline__ void word_coords(size_t word, int K, int& n, int& k0) {
     int j = (int)(word & 3);
     int lane = (int)((word >> 2) & 31);
-    int blk = (int)((word >> 7) & 7);
-    size_t tile = word >> 10;
-    int tiles_k = K / TILE_K;
-    int nb = (int)(tile / tiles_k), kb = (int)(tile % tiles_k);
-    int g = lane >> 2, t = lane & 3, i32 = blk >> 1, h = blk & 1;
-    n = nb * TILE_N + i32 * 32 + j * 8 + g;
-    k0 = kb * TILE_K + h * 64 + t * 16;
+    size_t blk = word >> 7;                         // 512-byte block index = n32 * (K/64) + k64
+    int blocks_k = K / BLK_K;
+    int n32 = (int)(blk / blocks_k), k64 = (int)(blk % blocks_k);
+    int g = lane >> 2, t = lane & 3;
+    n = n32 * BLK_N + j * 8 + g;
+    k0 = k64 * BLK_K + t * 16;
 }
 
 __global__ void pack_kernel(const int8_t* __restrict__ w, int N, int K, uint32_t* __restrict__ packed, int* __restrict__ bad) {
