@@ -72,9 +72,12 @@ def peaks():
 
 def ncu_traffic(kernel_key):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    p = os.path.join(ROOT, "profiles", "traffic.csv")      # kernel,dram_bytes_per_launch,capture
     if os.path.exists(p):
-        return json.load(open(p)).get(kernel_key)
+        for line in open(p).read().splitlines()[1:]:
+            f = line.split(",")
+            if len(f) >= 2 and f[0] == kernel_key:
+                return float(f[1])
     return None
 
 
@@ -345,7 +348,8 @@ def run_gpu(args):
     # warm-up, eager (also sets function attributes outside any capture)
     for s in range(max(args.warmup, 3)):
         wl.launch_step(s)
-        wl.launch_step(s, "gemm")
+        if args.workload != "decode":
+            wl.launch_step(s, "gemm")
     torch.cuda.synchronize()
 
     g_rev, n_rev = wl.capture(list(range(rev)))
@@ -394,11 +398,12 @@ def run_gpu(args):
 
     # ---- roofline of the dominant kernel (the GEMM), timed alone on pre-quantised activations, cold ring
     pk = peaks()
-    g_gemm, n_gemm = wl.capture(list(range(rev)), "gemm")
-    time_replays(torch, [g_gemm] * 2)
-    reps_g = max(3, min(200, int(2e5 / max(1, n_gemm))))
-    gemm_ms = time_replays(torch, [g_gemm] * reps_g) / reps_g
-    per_launch_s = gemm_ms * 1e-3 / n_gemm
+    if args.workload != "decode":
+        g_gemm, n_gemm = wl.capture(list(range(rev)), "gemm")
+        time_replays(torch, [g_gemm] * 2)
+        reps_g = max(3, min(200, int(2e5 / max(1, n_gemm))))
+        gemm_ms = time_replays(torch, [g_gemm] * reps_g) / reps_g
+        per_launch_s = gemm_ms * 1e-3 / n_gemm
     if args.workload == "decode":
         # the dominant (only) kernel of the step is the persistent program kernel: one launch = one step
         g_one, n_one = wl.capture(list(range(rev)))
@@ -411,8 +416,7 @@ def run_gpu(args):
                 "frac": achieved / pk["hbm_gbs"], "traffic": ncu_traffic("program_kernel"),
                 "kernel": "program_kernel", "peak_source": pk["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
                 "alg_bytes_per_launch": alg, "us_per_launch": per_launch_s * 1e6,
-                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                "single_call_gemm_us": gemm_ms * 1e3 / n_gemm}
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
     else:
         alg = wl.step_ops / len(wl.buf)
         achieved = alg / per_launch_s / 1e12
@@ -438,7 +442,8 @@ def run_gpu(args):
             t_roof = max(by / (pk["hbm_gbs"] * 1e9), op / (pk["bf16_tflops"] * 2e12))
             table.append({"M": b["M"], "K": b["K"], "N": b["N"], "us": t * 1e6, "GBs": by / t / 1e9,
                           "TOPS": op / t / 1e12, "roofline_frac": t_roof / t,
-                          "path": int(vla.vla_ternary_auto_path(b["M"], b["N"], b["K"]))})
+                          "path": int(vla.vla_ternary_auto_path(b["M"], b["N"], b["K"])),
+                          "route": "single vla_ternary_linear call (quant kernel + GEMM kernel)"})
             del g
 
     # ---- the oracle on this box's host cores, bounded sample
