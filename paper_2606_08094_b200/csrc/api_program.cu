@@ -140,17 +140,19 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     P->n_phases = phase + 1;
     int grid = max_phase_gran < sms ? max_phase_gran : sms;
     if (grid < 16 && sms >= 16) grid = 16;                  // enough CTAs to own one activation row each
-    // Split the grid among the stages of each phase in proportion to their weight bytes (>= 1 CTA each).
+    // Split the grid among the stages of each phase in proportion to their cost (>= 1 CTA each): weight bytes,
+    // times 1.6 for M > 8 (two token tiles: twice the IMMAs per decoded fragment; measured ratio).
+    auto cost = [&](int s) { return (double)S[s].granules * S[s].K * (S[s].M > 8 ? 1.6 : 1.0); };
     for (int s0 = 0; s0 < n_stages;) {
         int s1 = s0 + 1;
         while (s1 < n_stages && S[s1].phase == S[s0].phase) ++s1;
         const int ns = s1 - s0;
         if (ns > grid) return VLA_ERR_SHAPE;                 // more independent stages in one phase than CTAs
         double total = 0.0;
-        for (int s = s0; s < s1; ++s) total += (double)S[s].granules * S[s].K;
+        for (int s = s0; s < s1; ++s) total += cost(s);
         int given = 0;
         for (int s = s0; s < s1; ++s) {
-            int c = (int)((double)grid * ((double)S[s].granules * S[s].K) / total);
+            int c = (int)((double)grid * cost(s) / total);
             if (c < 1) c = 1;
             S[s].cta_count = c;
             given += c;
@@ -158,8 +160,8 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
         while (given != grid) {                              // hand the remainder to / take the excess from the
             int best = s0;                                   // stage with the most / least bytes per CTA
             for (int s = s0; s < s1; ++s) {
-                const double ls = (double)S[s].granules * S[s].K / S[s].cta_count;
-                const double lb = (double)S[best].granules * S[best].K / S[best].cta_count;
+                const double ls = cost(s) / S[s].cta_count;
+                const double lb = cost(best) / S[best].cta_count;
                 if (given < grid ? ls > lb : (S[s].cta_count > 1 && (S[best].cta_count <= 1 || ls < lb))) best = s;
             }
             S[best].cta_count += (given < grid) ? 1 : -1;

@@ -4,14 +4,14 @@
 // costs ~5000 cycles, more than ten times the HBM time of a 1.6 MB weight tensor, so the whole program is one
 // kernel and the only thing that ever waits is data.
 //
-// Grid: one CTA per SM, 17 warps.
-//   warp 16 (producer)   streams this CTA's share of the packed weights of EVERY stage, in program order, through
-//                        a 12 x 16 KiB shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
+// Grid: one CTA per SM, 16 warps.
+//   warp 15 (producer)   streams this CTA's share of the packed weights of EVERY stage, in program order, through
+//                        a 12 x 15 KiB shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
 //                        activations, so HBM stays busy across stage boundaries and grid barriers.
-//   warps 0-15 (consumers) per stage: hold the int8 activations as mma.m16n8k32 B fragments IN REGISTERS (warp w
-//                        owns the 64-wide k blocks kq = w mod 16), read packed words from the ring, decode them
+//   warps 0-14 (consumers) per stage: hold the int8 activations as mma.m16n8k32 B fragments IN REGISTERS (warp w
+//                        owns the 64-wide k blocks kq = w mod 15), read packed words from the ring, decode them
 //                        in registers (2 ALU ops per 4 weights, common.cuh) into A fragments, accumulate int32,
-//                        reduce the 16 partial sums per output through shared memory, and run the dequant
+//                        reduce the 15 partial sums per output through shared memory, and run the dequant
 //                        epilogue  y = (float)acc * (alpha_m * beta).
 // Work unit: a GRANULE = 32 output channels x all of K of one linear (K/128 contiguous 1 KiB pieces of the packed
 // layout).  The stages of one PHASE are independent, so they run CONCURRENTLY on disjoint CTA groups sized by their
@@ -31,18 +31,22 @@
 
 namespace vla {
 
-constexpr int PG_W = 16;                         // consumer warps
-constexpr int PG_CONSUMERS = PG_W * 32;          // 512 threads
-constexpr int PG_THREADS = PG_CONSUMERS + 32;
-constexpr int PG_SLOT_BYTES = 16384;             // 16 pieces of 1 KiB = 32 blocks of 32 ch x 64 k
+// 15 consumer warps + 1 producer = 16 warps = 4 per SM sub-partition -> 128 registers per thread.  (A 17th warp puts
+// five warps on one sub-partition and caps every thread at 96 registers: the B fragments then spill, and with 227 KB
+// of shared memory there is no L1 to catch the spills.)
+constexpr int PG_W = 15;                         // consumer warps
+constexpr int PG_CONSUMERS = PG_W * 32;          // 480 threads
+constexpr int PG_THREADS = PG_CONSUMERS + 32;    // 512
+constexpr int PG_CHUNK_PIECES = PG_W;            // 15 pieces of 1 KiB = 30 blocks of 32 ch x 64 k: two per warp
+constexpr int PG_SLOT_BYTES = PG_CHUNK_PIECES * 1024;
 constexpr int PG_XHI_BYTES = 65536;              // M <= 16 variant: B fragments of tokens 8-15 (8 * K bytes, K <= 8192)
-__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 11 : 7; }
+__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 12 : 7; }
 constexpr int PG_DESC_BYTES = 15360;             // stage + linear descriptors cached in shared memory
-constexpr int PG_NBMAX = 8;                      // k blocks per warp per granule  ->  K <= 8192
-constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 8448 ints = 33 792 B
+constexpr int PG_NBMAX = 10;                     // k blocks per warp per granule (5 chunks x 2)  ->  K <= 8192
+constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 7920 ints = 31 680 B
 __host__ __device__ constexpr int pg_smem(int maxmt) {
     return pg_nslot(maxmt) * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + (maxmt == 1 ? 0 : PG_XHI_BYTES) +
-           2 * pg_nslot(maxmt) * 8 + 64 + 128;
+           2 * pg_nslot(maxmt) * 8 + 64 + 16 + 128;
 }
 
 #ifdef VLA_PROG_TRACE
@@ -94,8 +98,11 @@ __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uin
 // ---------------------------------------------------------------- producer warp
 template <int NSLOT>
 __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, int cta,
-                                         int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty) {
-    uint32_t slot = 0, round = 0;
+                                         int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty, uint32_t bar_go) {
+    // The first two chunks go out at once; the rest of the ring is filled only after this CTA's consumers have seen
+    // their first quantised activations: otherwise 148 rings (26 MB) are requested in the first microsecond and the
+    // few KB of activation rows the quant owners need queue behind them (measured: 2.5-10 us before the first MMA).
+    uint32_t slot = 0, round = 0, issued = 0;
     for (int s = 0; s < P.n_stages; ++s) {
         const DevStage& st = stages[s];
         const int rank = cta - st.cta_begin;
@@ -107,10 +114,12 @@ __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stage
                 if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
             const int n32 = gi - lins[l].gran_begin;
             const uint8_t* src = lins[l].packed + (size_t)n32 * KB * 1024;      // the granule is one contiguous run
-            for (int p0 = 0; p0 < KB; p0 += 16) {
-                const int np = min(16, KB - p0);
+            for (int p0 = 0; p0 < KB; p0 += PG_CHUNK_PIECES) {
+                const int np = min(PG_CHUNK_PIECES, KB - p0);
+                if (issued == 2) mbar_wait(bar_go, 0);
+                ++issued;
                 if (round > 0) mbar_wait(bar_empty + 8u * slot, (round - 1) & 1);
-                if (lane == 0) {                              // one bulk copy of up to 16 KiB per chunk
+                if (lane == 0) {                              // one bulk copy of up to 15 KiB per chunk
                     mbar_arrive_expect_tx(bar_full + 8u * slot, (uint32_t)np * 1024u);
                     tma_bulk_g2s(ring + slot * PG_SLOT_BYTES, src + (size_t)p0 * 1024, (uint32_t)np * 1024u,
                                  bar_full + 8u * slot);
@@ -129,7 +138,8 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     const uint4 z = make_uint4(0, 0, 0, 0);
     const uint4 v0 = (tid < nvec) ? __ldcg(xr + tid) : z;
     const uint4 v1 = (tid + PG_CONSUMERS < nvec) ? __ldcg(xr + tid + PG_CONSUMERS) : z;
-    float m = absmax8(v1, absmax8(v0, 0.0f));
+    const uint4 v2 = (tid + 2 * PG_CONSUMERS < nvec) ? __ldcg(xr + tid + 2 * PG_CONSUMERS) : z;
+    float m = absmax8(v2, absmax8(v1, absmax8(v0, 0.0f)));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
     if ((tid & 31) == 0) s_max[tid >> 5] = m;
@@ -142,6 +152,7 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     uint2* qr = st.xq + (size_t)r * nvec;
     if (tid < nvec) qr[tid] = quant8(v0, alpha);
     if (tid + PG_CONSUMERS < nvec) qr[tid + PG_CONSUMERS] = quant8(v1, alpha);
+    if (tid + 2 * PG_CONSUMERS < nvec) qr[tid + 2 * PG_CONSUMERS] = quant8(v2, alpha);
     consumer_bar();                                          // s_max may be reused; stores precede thread 0's fence
 }
 
@@ -197,11 +208,14 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
     constexpr int MTOK = MT * 8;
     const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int M = st.M, nblk = st.K / BLK_K, KB = st.K / TILE_K;
-    const int nchunks = (KB + 15) >> 4;
-    const int etok = tid >> 5, ech = tid & 31;               // epilogue role: one output per thread
+    const int nchunks = (KB + PG_CHUNK_PIECES - 1) / PG_CHUNK_PIECES;
+    // epilogue role: output (token tid/32, channel tid%32); the 32 threads of warp 0 also take token 15
+    const int etok = tid >> 5, ech = tid & 31;
     const bool eactive = (etok < M) && (etok < MTOK);
+    const bool eactive2 = (MT == 2) && (tid < 32) && (M == 16);
     const float alpha = eactive ? __ldcg(st.xs + etok) : 0.0f;
-    const uint32_t my_off = (uint32_t)((w >> 1) * 1024 + (w & 1) * 512 + lane * 16);
+    const float alpha2 = eactive2 ? __ldcg(st.xs + 15) : 0.0f;
+    const uint32_t my_off = (uint32_t)(w * 512 + lane * 16);  // block b = ii*15 + w of the chunk
 
     for (int gi = cta; gi < st.granules; gi += G) {
         TRACE();
@@ -210,7 +224,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
             if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
         const DevLin& L = lins[l];
         const int n32 = gi - L.gran_begin;
-        const float beta = (eactive && L.dtype != 2) ? __ldcg(L.beta) : 0.0f;     // needed only in the epilogue
+        const float beta = ((eactive || eactive2) && L.dtype != 2) ? __ldcg(L.beta) : 0.0f;   // for the epilogue
 
 #ifdef VLA_PROG_TRACE
         long long twait = 0;
@@ -224,7 +238,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
                 for (int i = 0; i < 4; ++i) acc[c][mt][i] = 0;
 
 #pragma unroll
-        for (int ck = 0; ck < PG_NBMAX / 2; ++ck) {
+        for (int ck = 0; ck < PG_NBMAX / 2; ++ck) {           // 5 chunks of 15 KiB cover K <= 8192
             if (ck < nchunks) {
 #ifdef VLA_PROG_TRACE
                 long long tw0 = clock64();
@@ -237,7 +251,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
                 uint4 wv[2];
 #pragma unroll
                 for (int ii = 0; ii < 2; ++ii)
-                    wv[ii] = ((2 * ck + ii) * PG_W + w < nblk) ? lds128(ring + slot * PG_SLOT_BYTES + ii * 8192 + my_off)
+                    wv[ii] = ((2 * ck + ii) * PG_W + w < nblk) ? lds128(ring + slot * PG_SLOT_BYTES + ii * (PG_W * 512) + my_off)
                                                                : make_uint4(0, 0, 0, 0);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_empty + 8u * slot);       // release: ordered after the loads above
@@ -270,7 +284,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
         if (tid == 0 && tr_n < 1024) g_trace[cta * 1024 + tr_n++] = (unsigned long long)twait;   // cycles, not a stamp
 #endif
         TRACE();
-        // 16 per-warp partial sums -> shared memory -> one thread per output
+        // 15 per-warp partial sums -> shared memory -> one thread per output
         int* rb = red + ((MT == 1) ? (int)(gcount & 1) * (PG_W * 8 * 33) : 0);
 #pragma unroll
         for (int c = 0; c < 2; ++c)
@@ -284,18 +298,23 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
             }
         consumer_bar();
         TRACE();
-        if (eactive) {
-            int sum = 0;
 #pragma unroll
-            for (int ww = 0; ww < PG_W; ++ww) sum += rb[(ww * MTOK + etok) * 33 + ech];
-            const int a = sum >> 6;                           // the decode's factor 64 leaves exactly
-            const size_t o = (size_t)etok * L.N + (size_t)n32 * BLK_N + ech;
-            if (L.dtype == 2) {
-                reinterpret_cast<int*>(L.out)[o] = a;
-            } else {
-                const float y = dequant(a, __fmul_rn(alpha, beta));
-                if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
-                else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
+        for (int rep = 0; rep < MT; ++rep) {
+            const bool act = rep == 0 ? eactive : eactive2;
+            const int tok = rep == 0 ? etok : 15;
+            if (act) {
+                int sum = 0;
+#pragma unroll
+                for (int ww = 0; ww < PG_W; ++ww) sum += rb[(ww * MTOK + tok) * 33 + ech];
+                const int a = sum >> 6;                       // the decode's factor 64 leaves exactly
+                const size_t o = (size_t)tok * L.N + (size_t)n32 * BLK_N + ech;
+                if (L.dtype == 2) {
+                    reinterpret_cast<int*>(L.out)[o] = a;
+                } else {
+                    const float y = dequant(a, __fmul_rn(rep == 0 ? alpha : alpha2, beta));
+                    if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
+                    else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
+                }
             }
         }
         if (MT == 2) consumer_bar();                          // single reduction buffer: wait for the readers
@@ -319,6 +338,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
     const uint32_t xhi = base + NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES;
     const uint32_t bar_full = xhi + XHI;
     const uint32_t bar_empty = bar_full + 8u * NSLOT;
+    const uint32_t bar_go = bar_empty + 8u * NSLOT + 64u;    // after s_max (64 B)
     float* s_max = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT);
 
     const int tid = threadIdx.x, cta = blockIdx.x, G = gridDim.x;
@@ -327,6 +347,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
             mbar_init(bar_full + 8u * s, 1);
             mbar_init(bar_empty + 8u * s, PG_W);
         }
+        mbar_init(bar_go, 1);
         fence_barrier_init();
     }
     const DevProg P = *prog;
@@ -344,7 +365,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
     const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
 
     if (tid >= PG_CONSUMERS) {
-        producer<NSLOT>(P, stages, lins, cta, tid & 31, ring, bar_full, bar_empty);
+        producer<NSLOT>(P, stages, lins, cta, tid & 31, ring, bar_full, bar_empty, bar_go);
         return;
     }
 #ifdef VLA_PROG_TRACE
@@ -352,6 +373,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
 #endif
     TRACE();
     uint4 xv[PG_NBMAX];
+    bool go_sent = false;
     uint32_t slot = 0, phase = 0, gcount = 0;
     for (int s = 0; s < P.n_stages; ++s) {
         const DevStage& st = stages[s];
@@ -359,7 +381,11 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
         if (rank >= 0 && rank < count) {                     // this CTA belongs to the stage's group
             quant_owned_rows(P, s, st, rank, count, G, tid, s_max);
             TRACE();
-            if (tid == 0) spin_until(P.b2 + s, (unsigned)st.M);
+            if (tid == 0) {
+                spin_until(P.b2 + s, (unsigned)st.M);
+                if (!go_sent) mbar_arrive(bar_go);            // let the producer fill the rest of the ring
+            }
+            go_sent = true;
             consumer_bar();
             TRACE();
             load_xv<MAXMT>(st, tid, xv, xhi);
