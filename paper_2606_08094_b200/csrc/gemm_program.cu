@@ -206,7 +206,9 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
 #endif
                                            ) {
     constexpr int MTOK = MT * 8;
-    const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    // w through a shuffle: the compiler then knows it is warp-uniform and the per-block range checks below become
+    // uniform branches (no BSSY/BSYNC reconvergence around every block)
+    const int w = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0), lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int M = st.M, nblk = st.K / BLK_K, KB = st.K / TILE_K;
     const int nchunks = (KB + PG_CHUNK_PIECES - 1) / PG_CHUNK_PIECES;
     // epilogue role: output (token tid/32, channel tid%32); the 32 threads of warp 0 also take token 15
@@ -229,13 +231,16 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
 #ifdef VLA_PROG_TRACE
         long long twait = 0;
 #endif
-        int acc[2][MT][4];
+        int acc[2][MT][4], acc2[2][4];                        // acc2: second IMMA chain of token tile 0 (ILP)
 #pragma unroll
-        for (int c = 0; c < 2; ++c)
+        for (int c = 0; c < 2; ++c) {
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
                 for (int i = 0; i < 4; ++i) acc[c][mt][i] = 0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc2[c][i] = 0;
+        }
 
 #pragma unroll
         for (int ck = 0; ck < PG_NBMAX / 2; ++ck) {           // 5 chunks of 15 KiB cover K <= 8192
@@ -269,7 +274,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
                             const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
                             const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
                             mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xv[i].x, xv[i].y);
-                            mma_m16n8k32_s8_nv(acc[c][0], e0, e1, e2, e3, xv[i].z, xv[i].w);
+                            mma_m16n8k32_s8_nv(acc2[c], e0, e1, e2, e3, xv[i].z, xv[i].w);
                             if (MT == 2) {
                                 mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh.x, xh.y);
                                 mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh.z, xh.w);
@@ -284,6 +289,10 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
         if (tid == 0 && tr_n < 1024) g_trace[cta * 1024 + tr_n++] = (unsigned long long)twait;   // cycles, not a stamp
 #endif
         TRACE();
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc[c][0][i] += acc2[c][i];
         // 15 per-warp partial sums -> shared memory -> one thread per output
         int* rb = red + ((MT == 1) ? (int)(gcount & 1) * (PG_W * 8 * 33) : 0);
 #pragma unroll
