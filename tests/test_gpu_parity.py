@@ -319,3 +319,36 @@ def test_library_is_the_loaded_native_code(vla):
     """the in-tree .so is what the process mapped (no silent eager fallback exists)"""
     maps = open("/proc/self/maps").read()
     assert os.path.basename(vla.LIB_PATH) in maps
+
+
+# ---------------------------------------------------------------- full-size shapes, sampled output channels
+@pytest.mark.parametrize("M,K,N", [(4096, 8192, 8192), (1024, 6912, 2560), (2048, 2560, 6912)])
+def test_full_size_large_m_sampled_channels(vla, oracle, M, K, N):
+    """BASELINE.json configs[4] sizes in the launch configuration bench.py --workload sweep times (fused quant, fp32
+    out, VLA_PATH_AUTO).  The oracle cannot do 2.7e11 MACs in seconds, so it computes 64 sampled output channels
+    (all M tokens, all of K) one by one; every activation row is checked in full."""
+    rng = np.random.Generator(np.random.PCG64(M + K + N))
+    w = synth.ternary_weights(N, K, 0.33, 77 + N)
+    x_bits = synth.activations(M, K, 78 + K, dist="student_t3")
+    beta = np.float32(0.05)
+    cols = np.sort(rng.choice(N, size=64, replace=False))
+    ref = oracle.ternary_linear(x_bits, np.ascontiguousarray(w[cols]), beta)
+    packed = vla.pack_weights(dev(w))
+    x = dev_bf16(x_bits)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    nb = vla.vla_ternary_workspace_bytes(M, N, K)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    beta_d = dev(np.array([beta], np.float32))
+    for dtype, key in ((vla.VLA_I32, "acc"), (vla.VLA_F32, "y32")):
+        out = vla.empty_out(M, N, dtype)
+        vla.vla_ternary_linear(packed, beta_d, x, M, N, K, out, dtype, vla.VLA_PATH_AUTO, xq, xs, ws, nb)
+        torch.cuda.synchronize()
+        got = out[:, torch.from_numpy(cols).cuda()].cpu().numpy()
+        if key == "acc":
+            assert np.array_equal(got, ref["acc"])
+        else:
+            assert np.array_equal(got.view(np.uint32), ref["y32"].view(np.uint32))
+            assert np.all(np.abs(got.astype(np.float64) - ref["y64"]) <= REL_TOL_F32 * np.abs(ref["y64"]))
+    assert np.array_equal(xq.cpu().numpy(), ref["a"])
+    assert np.array_equal(xs.cpu().numpy().view(np.uint32), ref["alpha"].view(np.uint32))
