@@ -14,7 +14,7 @@ using vla::DevLin;
 using vla::DevProg;
 using vla::DevStage;
 
-struct ProgInfo { int grid; int n_stages; int max_m; };
+struct ProgInfo { int grid; int n_stages; int max_m; DevProg header; };
 std::mutex g_mu;
 std::unordered_map<const void*, ProgInfo> g_programs;
 
@@ -103,7 +103,7 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     P->stages = reinterpret_cast<const DevStage*>(base + L.off_stages);
     P->lins = reinterpret_cast<const DevLin*>(base + L.off_lins);
     size_t act = L.off_act;
-    int li = 0, max_m = 0, phase = 0, max_phase_gran = 0, phase_gran = 0;
+    int li = 0, max_m = 0, phase = 0, max_phase_gran = 0, phase_gran = 0, rows = 0;
     for (int s = 0; s < n_stages; ++s) {
         const vla_prog_stage& a = stages[s];
         DevStage& d = S[s];
@@ -113,11 +113,12 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
         d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + act + qbytes);
         act += qbytes + 256;
         d.M = (int16_t)a.M;
-        d.K = a.K;
-        d.depends = (int16_t)((s == 0) ? 0 : a.depends);    // nothing precedes the first stage
-        if (d.depends) { ++phase; phase_gran = 0; }          // a dependent stage opens a new phase
+        d.K = (int16_t)a.K;
+        d.flags = (int16_t)((s == 0) ? 0 : a.depends);      // nothing precedes the first stage
+        if (d.flags & 1) { ++phase; phase_gran = 0; }        // a dependent stage opens a new phase
         d.phase = phase;
-        d.publish = 0;
+        d.row_begin = rows;
+        rows += a.M;
         if (a.M > max_m) max_m = a.M;
         d.lin_begin = li;
         d.n_lin = (int16_t)a.n_linears;
@@ -140,9 +141,13 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     P->n_phases = phase + 1;
     int grid = max_phase_gran < sms ? max_phase_gran : sms;
     if (grid < 16 && sms >= 16) grid = 16;                  // enough CTAs to own one activation row each
-    // Split the grid among the stages of each phase in proportion to their cost (>= 1 CTA each): weight bytes,
-    // times 1.6 for M > 8 (two token tiles: twice the IMMAs per decoded fragment; measured ratio).
-    auto cost = [&](int s) { return (double)S[s].granules * S[s].K * (S[s].M > 8 ? 1.6 : 1.0); };
+    // Split the grid among the stages of each phase in proportion to their cost (>= 1 CTA each).  Measured per
+    // granule on B200: ~0.65 us fixed (reduction barrier + epilogue) + 0.5 us per 15 KiB chunk of
+    // its K, the chunk part times 1.6 for M > 8 (two token tiles: twice the IMMAs per decoded fragment).
+    auto cost = [&](int s) {
+        const int chunks = (S[s].K / 128 + 14) / 15;
+        return (double)S[s].granules * (0.65 + 0.5 * chunks * (S[s].M > 8 ? 1.6 : 1.0));
+    };
     for (int s0 = 0; s0 < n_stages;) {
         int s1 = s0 + 1;
         while (s1 < n_stages && S[s1].phase == S[s0].phase) ++s1;
@@ -169,7 +174,7 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
         }
         int begin = 0;
         for (int s = s0; s < s1; ++s) { S[s].cta_begin = begin; begin += S[s].cta_count; }
-        S[s1 - 1].publish = (int16_t)((s1 < n_stages) ? 1 : 0);   // the next phase opens with a dependent stage
+        if (s1 < n_stages) S[s1 - 1].flags |= 2;             // publish: the next phase opens with a dependent stage
         s0 = s1;
     }
 
@@ -178,7 +183,7 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     std::lock_guard<std::mutex> lk(g_mu);
-    g_programs[prog_dev] = ProgInfo{grid, n_stages, max_m};
+    g_programs[prog_dev] = ProgInfo{grid, n_stages, max_m, *P};
     return VLA_OK;
 }
 
@@ -191,7 +196,7 @@ vla_status vla_program_run(const void* prog_dev, void* stream) {
         if (it == g_programs.end()) return VLA_ERR_VALUE;
         info = it->second;
     }
-    cudaError_t e = vla::launch_program(prog_dev, info.grid, info.max_m, (cudaStream_t)stream);
+    cudaError_t e = vla::launch_program(info.header, info.grid, info.max_m, (cudaStream_t)stream);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     return VLA_OK;
 }

@@ -59,10 +59,12 @@ __device__ __forceinline__ void trace(int cta, int& n, int tid) {
         g_trace[cta * 1024 + n++] = t;
     }
 }
+#define QTRACE(k) do { if (threadIdx.x == 0 && g_trace[blockIdx.x * 1024 + 900 + (k)] == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_trace[blockIdx.x * 1024 + 900 + (k)] = t_; } } while (0)
 #define TRACE() trace(cta, tr_n, tid)
 #define TRARG , tr_n
 #else
 #define TRACE()
+#define QTRACE(k) do { } while (0)
 #define TRARG
 #endif
 
@@ -136,6 +138,7 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     const int nvec = st.K / 8;                               // uint4 of 8 bf16; K <= 8192 -> nvec <= 1024
     const uint4* xr = st.x + (size_t)r * nvec;
     const uint4 z = make_uint4(0, 0, 0, 0);
+    QTRACE(0);
     const uint4 v0 = (tid < nvec) ? __ldcg(xr + tid) : z;
     const uint4 v1 = (tid + PG_CONSUMERS < nvec) ? __ldcg(xr + tid + PG_CONSUMERS) : z;
     const uint4 v2 = (tid + 2 * PG_CONSUMERS < nvec) ? __ldcg(xr + tid + 2 * PG_CONSUMERS) : z;
@@ -143,7 +146,9 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
     if ((tid & 31) == 0) s_max[tid >> 5] = m;
+    QTRACE(1);
     consumer_bar();
+    QTRACE(2);
     m = s_max[0];
 #pragma unroll
     for (int i = 1; i < PG_W; ++i) m = fmaxf(m, s_max[i]);
@@ -153,21 +158,32 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     if (tid < nvec) qr[tid] = quant8(v0, alpha);
     if (tid + PG_CONSUMERS < nvec) qr[tid + PG_CONSUMERS] = quant8(v1, alpha);
     if (tid + 2 * PG_CONSUMERS < nvec) qr[tid + 2 * PG_CONSUMERS] = quant8(v2, alpha);
+    QTRACE(3);
     consumer_bar();                                          // s_max may be reused; stores precede thread 0's fence
+    QTRACE(4);
 }
 
-// Row r of a stage is quantised by CTA (count - 1 - r mod count) of the stage's group.
-__device__ __forceinline__ void quant_owned_rows(const DevProg& P, int s, const DevStage& st, int rank, int count, int G,
-                                                 int tid, float* s_max) {
-    const int first = count - 1 - rank;                      // rows first, first + count, ...
-    if (first >= st.M) return;
-    if (st.depends) {
-        if (tid == 0) spin_until(P.bp + (st.phase - 1), (unsigned)G);
-        consumer_bar();
+// Row r of stage s is quantised by CTA (row_begin_s + r) mod gridDim.x -- any CTA, not only the stage's group, so that
+// the rows of all stages of a phase are spread over the whole grid (a 2-CTA group would otherwise quantise 8 rows
+// one after the other).  Called by every CTA at the start of a phase, for all stages [s0, s1) of the phase.
+__device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStage* stages, int s0, int cta, int G, int tid,
+                                                 float* s_max) {
+    const int phase = stages[s0].phase;
+    bool waited = false;
+    for (int s = s0; s < P.n_stages && stages[s].phase == phase; ++s) {
+        const DevStage& st = stages[s];
+        int r = cta - st.row_begin % G;                       // first row with (row_begin + r) % G == cta
+        if (r < 0) r += G;
+        for (; r < st.M; r += G) {
+            if ((st.flags & 1) && !waited) {                  // x is written by the previous phase
+                if (tid == 0) spin_until(P.bp + (phase - 1), (unsigned)G);
+                consumer_bar();
+                waited = true;
+            }
+            quant_row(st, r, tid, s_max);
+            if (tid == 0) red_release_gpu(P.b2 + s, 1u);
+        }
     }
-    int owned = 0;
-    for (int r = first; r < st.M; r += count, ++owned) quant_row(st, r, tid, s_max);
-    if (tid == 0) red_release_gpu(P.b2 + s, (unsigned)owned);
 }
 
 // ---------------------------------------------------------------- one stage's granules on the consumer warps
@@ -335,7 +351,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
 // ---------------------------------------------------------------- the kernel
 // MAXMT = 1: every stage has M <= 8 (32 registers of B fragments per thread, no spills);  MAXMT = 2: M <= 16.
 template <int MAXMT>
-__global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* __restrict__ prog) {
+__global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_constant__ DevProg P) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
@@ -359,7 +375,6 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
         mbar_init(bar_go, 1);
         fence_barrier_init();
     }
-    const DevProg P = *prog;
     // descriptor tables -> shared memory (they are read on every granule by producer and consumers)
     const int stage_words = P.n_stages * (int)(sizeof(DevStage) / 8), lin_words = P.n_lin * (int)(sizeof(DevLin) / 8);
     {
@@ -384,11 +399,15 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
     uint4 xv[PG_NBMAX];
     bool go_sent = false;
     uint32_t slot = 0, phase = 0, gcount = 0;
+    int cur_phase = -1;
     for (int s = 0; s < P.n_stages; ++s) {
         const DevStage& st = stages[s];
+        if (st.phase != cur_phase) {                         // a new phase: quantise the rows this CTA owns
+            cur_phase = st.phase;
+            quant_phase_rows(P, stages, s, cta, G, tid, s_max);
+        }
         const int rank = cta - st.cta_begin, count = st.cta_count;
         if (rank >= 0 && rank < count) {                     // this CTA belongs to the stage's group
-            quant_owned_rows(P, s, st, rank, count, G, tid, s_max);
             TRACE();
             if (tid == 0) {
                 spin_until(P.b2 + s, (unsigned)st.M);
@@ -404,7 +423,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
                 stage_gemm<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
             TRACE();
         }
-        if (st.publish) {                                    // end of a phase that a later phase reads from
+        if (st.flags & 2) {                                  // end of a phase that a later phase reads from
             consumer_bar();                                  // every output store of this CTA precedes the release
             if (tid == 0) red_release_gpu(P.bp + st.phase, 1u);
             TRACE();
@@ -424,7 +443,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const DevProg* _
 
 size_t program_desc_capacity() { return PG_DESC_BYTES; }
 
-cudaError_t launch_program(const void* prog_dev, int grid, int max_m, cudaStream_t s) {
+cudaError_t launch_program(const DevProg& prog, int grid, int max_m, cudaStream_t s) {
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(program_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg_smem(1));
@@ -433,8 +452,8 @@ cudaError_t launch_program(const void* prog_dev, int grid, int max_m, cudaStream
         attr_set = true;
     }
     count_launch();
-    if (max_m <= 8) program_kernel<1><<<grid, PG_THREADS, pg_smem(1), s>>>(reinterpret_cast<const DevProg*>(prog_dev));
-    else            program_kernel<2><<<grid, PG_THREADS, pg_smem(2), s>>>(reinterpret_cast<const DevProg*>(prog_dev));
+    if (max_m <= 8) program_kernel<1><<<grid, PG_THREADS, pg_smem(1), s>>>(prog);
+    else            program_kernel<2><<<grid, PG_THREADS, pg_smem(2), s>>>(prog);
     return cudaGetLastError();
 }
 

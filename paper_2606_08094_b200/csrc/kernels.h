@@ -19,8 +19,9 @@ cudaError_t launch_gemm_small(bool use_mma, const void* packed, const float* w_s
                               const float* x_scale, int M, int N, int K, void* out, int out_dtype, cudaStream_t s);
 cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
                               int M, int N, int K, void* out, int out_dtype, cudaStream_t s);
-// persistent program kernel (gemm_program.cu); prog_dev holds a DevProg (program.h)
-cudaError_t launch_program(const void* prog_dev, int grid, int max_m, cudaStream_t s);
+// persistent program kernel (gemm_program.cu); the program header travels as a kernel parameter
+struct DevProg;
+cudaError_t launch_program(const DevProg& prog, int grid, int max_m, cudaStream_t s);
 size_t program_desc_capacity();      // bytes of stage + linear descriptors a program may hold
 cudaError_t run_i8_mma_probe(int ctas, int mmas_per_cta, float* ms_out);
 

@@ -26,13 +26,14 @@ struct DevStage {
     float* xs;                 // fp32 [M]
     int16_t M;
     int16_t n_lin;
-    int16_t depends;           // 1: x is written by earlier phases of this program
-    int16_t publish;           // 1: last stage of its phase AND the next phase has a dependent stage -> count in bp
-    int K;
+    int16_t flags;             // bit 0 "depends": x is written by earlier phases of this program
+                               // bit 1 "publish": last stage of its phase AND the next phase depends -> count in bp
+    int16_t K;
     int lin_begin;
     int granules;              // sum over its linears of N/32
     int phase;                 // stages of one phase are independent and run concurrently on disjoint CTA groups
     int cta_begin, cta_count;  // the CTA group of this stage: [cta_begin, cta_begin + cta_count)
+    int row_begin;             // running sum of M over all earlier stages: row r is quantised by CTA (row_begin + r) % grid
 };
 
 struct DevProg {
