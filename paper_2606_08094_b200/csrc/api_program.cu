@@ -175,6 +175,13 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
         int begin = 0;
         for (int s = s0; s < s1; ++s) { S[s].cta_begin = begin; begin += S[s].cta_count; }
         if (s1 < n_stages) S[s1 - 1].flags |= 2;             // publish: the next phase opens with a dependent stage
+        // Activation rows: spread over the whole grid (<= 2 rows per CTA) unless the phase has so many rows that
+        // every CTA is busy quantising anyway; then each stage's own group quantises its rows (no cross-group wait).
+        int phase_rows = 0;
+        for (int s = s0; s < s1; ++s) phase_rows += S[s].M;
+        if (phase_rows > 2 * grid)
+            for (int s = s0; s < s1; ++s) S[s].flags |= 4;
+        for (int s = s0; s < s1; ++s) S[s].row_begin %= grid;
         s0 = s1;
     }
 

@@ -46,7 +46,7 @@ constexpr int PG_NBMAX = 10;                     // k blocks per warp per granul
 constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 7920 ints = 31 680 B
 __host__ __device__ constexpr int pg_smem(int maxmt) {
     return pg_nslot(maxmt) * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + (maxmt == 1 ? 0 : PG_XHI_BYTES) +
-           2 * pg_nslot(maxmt) * 8 + 64 + 16 + 128;
+           2 * pg_nslot(maxmt) * 8 + 64 + 16 + 64 + 128;
 }
 
 #ifdef VLA_PROG_TRACE
@@ -163,26 +163,38 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     QTRACE(4);
 }
 
-// Row r of stage s is quantised by CTA (row_begin_s + r) mod gridDim.x -- any CTA, not only the stage's group, so that
+// Row r of stage s is quantised by CTA (row_begin_s + r) mod gridDim.x (row_begin_s is stored reduced mod gridDim.x) -- any CTA, not only the stage's group, so that
 // the rows of all stages of a phase are spread over the whole grid (a 2-CTA group would otherwise quantise 8 rows
 // one after the other).  Called by every CTA at the start of a phase, for all stages [s0, s1) of the phase.
+// own_stage = true: only stage s0, and only if its rows stay inside its group (flag bit 2).
 __device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStage* stages, int s0, int cta, int G, int tid,
-                                                 float* s_max) {
+                                                 float* s_max, bool own_stage) {
     const int phase = stages[s0].phase;
     bool waited = false;
-    for (int s = s0; s < P.n_stages && stages[s].phase == phase; ++s) {
+    for (int s = s0; s < (own_stage ? s0 + 1 : P.n_stages) && stages[s].phase == phase; ++s) {
         const DevStage& st = stages[s];
-        int r = cta - st.row_begin % G;                       // first row with (row_begin + r) % G == cta
-        if (r < 0) r += G;
-        for (; r < st.M; r += G) {
+        int r, step;
+        if (st.flags & 4) {                                   // rows stay inside the stage's own CTA group
+            if (!own_stage) continue;                         // (quantised when the group reaches the stage)
+            r = cta - st.cta_begin;
+            step = st.cta_count;
+            if (r < 0 || r >= step) continue;
+        } else {                                              // first row with (row_begin + r) % G == cta
+            if (own_stage) continue;
+            r = cta - st.row_begin;                           // row_begin is already reduced mod gridDim.x
+            if (r < 0) r += G;
+            step = G;
+        }
+        unsigned done_rows = 0;
+        for (; r < st.M; r += step, ++done_rows) {
             if ((st.flags & 1) && !waited) {                  // x is written by the previous phase
                 if (tid == 0) spin_until(P.bp + (phase - 1), (unsigned)G);
                 consumer_bar();
                 waited = true;
             }
             quant_row(st, r, tid, s_max);
-            if (tid == 0) red_release_gpu(P.b2 + s, 1u);
         }
+        if (done_rows != 0 && tid == 0) red_release_gpu(P.b2 + s, done_rows);    // one release per stage
     }
 }
 
@@ -215,7 +227,7 @@ __device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)
 // cta / G: rank and size of the stage's CTA group
 template <int MT, int NSLOT>
 __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& st, int cta, int G,
-                                           int tid, uint32_t ring, int* red, uint32_t bar_full, uint32_t bar_empty,
+                                           int tid, uint32_t ring, int* red, const float* s_beta, uint32_t bar_full, uint32_t bar_empty,
                                            uint4 (&xv)[PG_NBMAX], uint32_t xhi, uint32_t& slot, uint32_t& phase, uint32_t& gcount
 #ifdef VLA_PROG_TRACE
                                            , int& tr_n
@@ -242,7 +254,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
             if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
         const DevLin& L = lins[l];
         const int n32 = gi - L.gran_begin;
-        const float beta = ((eactive || eactive2) && L.dtype != 2) ? __ldcg(L.beta) : 0.0f;   // for the epilogue
+        const float beta = s_beta[l - st.lin_begin];          // staged once per stage
 
 #ifdef VLA_PROG_TRACE
         long long twait = 0;
@@ -364,6 +376,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
     const uint32_t bar_full = xhi + XHI;
     const uint32_t bar_empty = bar_full + 8u * NSLOT;
     const uint32_t bar_go = bar_empty + 8u * NSLOT + 64u;    // after s_max (64 B)
+    float* s_beta = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT + 64 + 16);   // 16 floats
     float* s_max = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT);
 
     const int tid = threadIdx.x, cta = blockIdx.x, G = gridDim.x;
@@ -404,23 +417,29 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         const DevStage& st = stages[s];
         if (st.phase != cur_phase) {                         // a new phase: quantise the rows this CTA owns
             cur_phase = st.phase;
-            quant_phase_rows(P, stages, s, cta, G, tid, s_max);
+            quant_phase_rows(P, stages, s, cta, G, tid, s_max, false);
         }
         const int rank = cta - st.cta_begin, count = st.cta_count;
         if (rank >= 0 && rank < count) {                     // this CTA belongs to the stage's group
+            if (st.flags & 4) quant_phase_rows(P, stages, s, cta, G, tid, s_max, true);
             TRACE();
             if (tid == 0) {
                 spin_until(P.b2 + s, (unsigned)st.M);
                 if (!go_sent) mbar_arrive(bar_go);            // let the producer fill the rest of the ring
             }
             go_sent = true;
+            // the stage's scales beta -> shared memory (one L2 round trip per stage instead of one per granule)
+            if (tid >= 32 && tid < 32 + st.n_lin) {
+                const DevLin& L = lins[st.lin_begin + tid - 32];
+                s_beta[tid - 32] = (L.dtype != 2) ? __ldcg(L.beta) : 0.0f;
+            }
             consumer_bar();
             TRACE();
             load_xv<MAXMT>(st, tid, xv, xhi);
             if (MAXMT == 1 || st.M <= 8)
-                stage_gemm<1, NSLOT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
+                stage_gemm<1, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
             else
-                stage_gemm<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
+                stage_gemm<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
             TRACE();
         }
         if (st.flags & 2) {                                  // end of a phase that a later phase reads from

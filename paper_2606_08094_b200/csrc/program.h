@@ -28,12 +28,13 @@ struct DevStage {
     int16_t n_lin;
     int16_t flags;             // bit 0 "depends": x is written by earlier phases of this program
                                // bit 1 "publish": last stage of its phase AND the next phase depends -> count in bp
+                               // bit 2 "rows in group": the stage's own CTA group quantises its rows (else the whole grid)
     int16_t K;
     int lin_begin;
     int granules;              // sum over its linears of N/32
     int phase;                 // stages of one phase are independent and run concurrently on disjoint CTA groups
     int cta_begin, cta_count;  // the CTA group of this stage: [cta_begin, cta_begin + cta_count)
-    int row_begin;             // running sum of M over all earlier stages: row r is quantised by CTA (row_begin + r) % grid
+    int row_begin;             // (running sum of M over all earlier stages) % grid: row r is quantised by CTA (row_begin + r) % grid
 };
 
 struct DevProg {
