@@ -255,15 +255,33 @@ class GpuWorkload:
             xs_full[si] = c["x"]
             del w
         self.buf = []
+        # All activation inputs of a step live in ONE device arena (and one pinned host arena), all outputs in another:
+        # the host-buffer call then moves a step's inputs with one copy and its outputs with one copy.
+        dt = torch.bfloat16 if self.out_dtype == vla.VLA_BF16 else torch.float32
+        esz = 2 if dt == torch.bfloat16 else 4
+        al = lambda n: -(-n // 256) * 256
+        x_off, o_off, xo, oo = [], [], 0, 0
         for (M, si) in self.points:
             K, N = synth.MODEL_SHAPES[si]
+            x_off.append(xo); xo += al(2 * M * K)
+            o_off.append(oo); oo += al(esz * M * N)
+        self.x_arena = torch.empty(xo, dtype=torch.uint8, device=device)
+        self.x_arena_host = torch.empty(xo, dtype=torch.uint8).pin_memory()
+        self.o_arena = torch.empty(oo, dtype=torch.uint8, device=device)
+        self.o_arena_host = torch.empty(oo, dtype=torch.uint8).pin_memory()
+        for pi, (M, si) in enumerate(self.points):
+            K, N = synth.MODEL_SHAPES[si]
             xb = np.ascontiguousarray(xs_full[si][:M])
-            x_host = torch.from_numpy(xb.view(np.int16)).view(torch.bfloat16).pin_memory()
-            dt = torch.bfloat16 if self.out_dtype == vla.VLA_BF16 else torch.float32
+            x_host = self.x_arena_host[x_off[pi]:x_off[pi] + 2 * M * K].view(torch.bfloat16).view(M, K)
+            x_host.copy_(torch.from_numpy(xb.view(np.int16)).view(torch.bfloat16))
+            x_dev = self.x_arena[x_off[pi]:x_off[pi] + 2 * M * K].view(torch.bfloat16).view(M, K)
+            x_dev.copy_(x_host)
+            out_dev = self.o_arena[o_off[pi]:o_off[pi] + esz * M * N].view(dt).view(M, N)
+            out_host = self.o_arena_host[o_off[pi]:o_off[pi] + esz * M * N].view(dt).view(M, N)
             ws_bytes = vla.vla_ternary_host_workspace_bytes(M, N, K, self.out_dtype)
             self.buf.append(dict(
-                M=M, K=K, N=N, si=si, x=x_host.to(device), x_host=x_host,
-                out=torch.empty((M, N), dtype=dt, device=device), out_host=torch.empty((M, N), dtype=dt).pin_memory(),
+                M=M, K=K, N=N, si=si, x=x_dev, x_host=x_host,
+                out=out_dev, out_host=out_host,
                 xq=torch.empty((M, K), dtype=torch.int8, device=device),
                 xs=torch.empty((M,), dtype=torch.float32, device=device),
                 ws=torch.empty(ws_bytes, dtype=torch.uint8, device=device), ws_bytes=ws_bytes))
@@ -276,8 +294,8 @@ class GpuWorkload:
                                              out=b["out"], N=b["N"], out_dtype=self.out_dtype)])
                           for pi, b in enumerate(self.buf)]
                 self.programs.append(vla.compile_program(stages, device))
-            self.copies_in = vla.make_copies([(b["x_host"], b["x"]) for b in self.buf])
-            self.copies_out = vla.make_copies([(b["out_host"], b["out"]) for b in self.buf])
+            self.copies_in = vla.make_copies([(self.x_arena_host, self.x_arena)])
+            self.copies_out = vla.make_copies([(self.o_arena_host, self.o_arena)])
         self.step_bytes = sum(point_bytes(b["M"], b["K"], b["N"], self.out_bytes) for b in self.buf)
         self.step_ops = sum(point_ops(b["M"], b["K"], b["N"]) for b in self.buf)
         self.gemm_bytes = sum(point_bytes(b["M"], b["K"], b["N"], self.out_bytes, fused_quant=False) for b in self.buf)
