@@ -398,6 +398,9 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         for (int i = tid; i < lin_words; i += PG_THREADS) d[stage_words + i] = gl[i];
     }
     __syncthreads();
+    // Programmatic dependent launch: everything above (barrier init, the static descriptor tables) may overlap the
+    // tail of the previous kernel on this stream; counters, activations, weights-in-flight and outputs come after.
+    pdl_wait();
     const DevStage* stages = reinterpret_cast<const DevStage*>(desc);
     const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
 
@@ -448,6 +451,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
             TRACE();
         }
     }
+    pdl_launch_dependents();
     // the last CTA to finish re-zeroes the counters, so the next launch of the same program needs no memset
     if (tid == 0) {
         const unsigned prev = atomicAdd(P.done, 1u);
@@ -471,9 +475,18 @@ cudaError_t launch_program(const DevProg& prog, int grid, int max_m, cudaStream_
         attr_set = true;
     }
     count_launch();
-    if (max_m <= 8) program_kernel<1><<<grid, PG_THREADS, pg_smem(1), s>>>(prog);
-    else            program_kernel<2><<<grid, PG_THREADS, pg_smem(2), s>>>(prog);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(PG_THREADS);
+    cfg.dynamicSmemBytes = (size_t)pg_smem(max_m <= 8 ? 1 : 2);
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    if (max_m <= 8) return cudaLaunchKernelEx(&cfg, program_kernel<1>, prog);
+    return cudaLaunchKernelEx(&cfg, program_kernel<2>, prog);
 }
 
 #ifdef VLA_PROG_TRACE
