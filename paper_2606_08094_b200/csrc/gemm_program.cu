@@ -84,6 +84,15 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return r;
 }
 
+__device__ __forceinline__ int lds32(uint32_t addr) {
+    int r;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(r) : "r"(addr));
+    return r;
+}
+__device__ __forceinline__ void sts32(uint32_t addr, int v) {
+    asm volatile("st.shared.s32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
+}
+
 // publish: every store this CTA made before the preceding consumer_bar() becomes visible before the count does
 __device__ __forceinline__ void red_release_gpu(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
@@ -322,16 +331,17 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
 #pragma unroll
             for (int i = 0; i < 4; ++i) acc[c][0][i] += acc2[c][i];
         // 15 per-warp partial sums -> shared memory -> one thread per output
-        int* rb = red + ((MT == 1) ? (int)(gcount & 1) * (PG_W * 8 * 33) : 0);
+        // explicit shared-space accesses (a generic int* would compile to 64-bit generic LD/ST)
+        const uint32_t rb = smem_u32(red) + ((MT == 1) ? (uint32_t)(gcount & 1) * (PG_W * 8 * 33 * 4) : 0u);
 #pragma unroll
         for (int c = 0; c < 2; ++c)
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) {
-                int* row0 = rb + (w * MTOK + mt * 8 + 2 * t) * 33 + 16 * c + g;
-                row0[0] = acc[c][mt][0];
-                row0[33] = acc[c][mt][1];
-                row0[8] = acc[c][mt][2];
-                row0[33 + 8] = acc[c][mt][3];
+                const uint32_t row0 = rb + (uint32_t)((w * MTOK + mt * 8 + 2 * t) * 33 + 16 * c + g) * 4u;
+                sts32(row0, acc[c][mt][0]);
+                sts32(row0 + 33 * 4, acc[c][mt][1]);
+                sts32(row0 + 8 * 4, acc[c][mt][2]);
+                sts32(row0 + (33 + 8) * 4, acc[c][mt][3]);
             }
         consumer_bar();
         TRACE();
@@ -342,7 +352,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
             if (act) {
                 int sum = 0;
 #pragma unroll
-                for (int ww = 0; ww < PG_W; ++ww) sum += rb[(ww * MTOK + tok) * 33 + ech];
+                for (int ww = 0; ww < PG_W; ++ww) sum += lds32(rb + (uint32_t)((ww * MTOK + tok) * 33 + ech) * 4u);
                 const int a = sum >> 6;                       // the decode's factor 64 leaves exactly
                 const size_t o = (size_t)tok * L.N + (size_t)n32 * BLK_N + ech;
                 if (L.dtype == 2) {
