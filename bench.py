@@ -47,6 +47,13 @@ def workload_points(name):
     raise ValueError(name)
 
 
+def workload_name(workload):
+    """`config.workload` of the JSON line -- the same string for the B200 arm and the reference arm."""
+    if workload == "decode":
+        return "configs[1] decode: 4 BitNet-2B linears x M in {1,8,16}, fused quant, bf16 out (B200 arm: one persistent program launch per step)"
+    return "configs[2] prefill: 4 BitNet-2B linears at M=544, fused quant, fp32 out"
+
+
 def out_elem_bytes(workload):
     return 2 if workload == "decode" else 4       # configs[1]: bf16 output; configs[2]: fp32 output
 
@@ -186,7 +193,7 @@ def run_reference(args):
         "n_gpus": args.gpus, "steps": done, "warmup": min(args.warmup, 1), "ms_per_step": sec / done * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8*ternary->int32",
         "data": "synthetic", "tops": nops / sec / 1e12,
-        "config": {"workload": "configs[1] decode" if args.workload == "decode" else "configs[2] prefill M=544"},
+        "config": {"workload": workload_name(args.workload), "sample": sample},
         "cpu_baseline": {"value": val, "unit": "GB/s", "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
@@ -482,9 +489,7 @@ def run_gpu(args):
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int8*ternary->int32", "data": "synthetic",
         "tops": total_ops / (ms * 1e-3) / 1e12,
-        "config": {"workload": "configs[1] decode: 4 BitNet-2B linears x M in {1,8,16}, fused quant, bf16 out, "
-                               "one persistent program launch per step"
-                   if args.workload == "decode" else "configs[2] prefill: 4 BitNet-2B linears at M=544, fused quant, fp32 out",
+        "config": {"workload": workload_name(args.workload),
                    "cold_weights": "ring of %d packed copies per shape (%.0f MB > 2 x L2 %.0f MB), next slot every use"
                    % (wl.copies, wl.copies * sum(r.shape[1] for r in wl.ring) / 1e6, wl.l2 / 1e6),
                    "launch": ("CUDA graphs of %d program launches" if args.workload == "decode" else "CUDA graphs of %d steps + PDL") % rev, "parallelism": "replicas" if world > 1 else "single"},
