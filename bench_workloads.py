@@ -29,7 +29,7 @@ def _time(torch, fn, reps):
 # ----------------------------------------------------------------------------- configs[3]
 def run_stack(args, pk, clock_sampler):
     """30 decoder layers, q/k/v/o/gate/up/down ternary linears + their activation quant, chained; M=544 (one quant
-    kernel per stage + one tcgen05 GEMM launch per linear, CUDA graph + PDL) then M=8 (ONE persistent program launch)."""
+    kernel + one grouped tcgen05 GEMM launch per stage, CUDA graph + PDL) then M=8 (ONE persistent program launch)."""
     import torch
     from paper_2606_08094_b200 import binding as vla, synth
     from paper_2606_08094_b200.stack import Stack
@@ -64,7 +64,7 @@ def run_stack(args, pk, clock_sampler):
         t_roof = max(wbytes / (pk["hbm_gbs"] * 1e9), ops / (pk["bf16_tflops"] * 2e12))
         out["M%d" % M] = {"us": sec * 1e6, "us_per_layer": sec * 1e6 / layers, "launches": launches,
                           "weight_GBs": wbytes / sec / 1e9, "TOPS": ops / sec / 1e12, "roofline_frac": t_roof / sec,
-                          "route": "one persistent program launch" if M <= 16 else "act_quant + tcgen05 GEMM per linear, CUDA graph + PDL"}
+                          "route": "one persistent program launch" if M <= 16 else "act_quant + one grouped tcgen05 launch per stage, CUDA graph + PDL"}
         del st
         torch.cuda.empty_cache()
     clocks = sampler.stop()

@@ -26,7 +26,7 @@ EXPORTS = [
     "vla_act_quant", "vla_ternary_gemm", "vla_ternary_linear", "vla_ternary_linear_host",
     "vla_ternary_host_workspace_bytes",
     "vla_ternary_auto_path", "vla_i8_mma_issue_probe", "vla_status_string", "vla_launch_count",
-    "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_run_host", "vla_program_release",
+    "vla_ternary_gemm_grouped", "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_run_host", "vla_program_release",
 ]
 
 
@@ -90,6 +90,8 @@ def _load():
     lib.vla_program_build.argtypes = [ps, i, vp, sz, vp]
     lib.vla_program_run.restype = st
     lib.vla_program_run.argtypes = [vp, vp]
+    lib.vla_ternary_gemm_grouped.restype = st
+    lib.vla_ternary_gemm_grouped.argtypes = [ctypes.POINTER(vla_prog_linear), i, vp, vp, i, i, i, vp]
     lib.vla_program_run_host.restype = st
     lib.vla_program_run_host.argtypes = [vp, ctypes.POINTER(vla_copy), i, ctypes.POINTER(vla_copy), i, vp]
     lib.vla_program_release.restype = st
@@ -203,6 +205,21 @@ def _marshal_stages(stages):
         arr[si] = vla_prog_stage(_ptr(sd["x"]), int(sd["M"]), int(sd["K"]), int(sd.get("depends", 0)), len(lins), lins,
                                  _ptr(sd.get("xq_opt")), _ptr(sd.get("x_scale_opt")))
     return arr, keep
+
+
+def make_linears(linears):
+    """[{packed, w_scale, out, N, out_dtype}] -> ctypes array of vla_prog_linear (marshalled once, reusable)."""
+    arr = (vla_prog_linear * len(linears))()
+    for li, ld in enumerate(linears):
+        arr[li] = vla_prog_linear(_ptr(ld["packed"]), _ptr(ld["w_scale"]), _ptr(ld["out"]), int(ld["N"]), int(ld["out_dtype"]))
+    return arr
+
+
+def vla_ternary_gemm_grouped(linears, xq, x_scale, M, K, path=VLA_PATH_AUTO, stream=None):
+    """linears: a ctypes array from make_linears (or a list of dicts, marshalled on the fly)."""
+    arr = linears if not isinstance(linears, (list, tuple)) else make_linears(linears)
+    _check(_lib.vla_ternary_gemm_grouped(arr, len(arr), _ptr(xq), _ptr(x_scale), M, K, path, _stream(stream)),
+           "vla_ternary_gemm_grouped")
 
 
 def vla_program_bytes(stages):

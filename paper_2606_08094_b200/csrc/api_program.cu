@@ -231,6 +231,53 @@ vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in, int n_
     return VLA_OK;
 }
 
+vla_status vla_ternary_gemm_grouped(const vla_prog_linear* lins, int n_linears, const int8_t* xq, const float* x_scale,
+                                    int M, int K, vla_path path, void* stream) {
+    if (!lins || !xq) return VLA_ERR_NULL;
+    if (n_linears < 1 || n_linears > 8 || M < 1 || K < 128 || K % 128 != 0 || K > 65536) return VLA_ERR_SHAPE;
+    if ((int)path < 0 || (int)path > 3) return VLA_ERR_DTYPE;
+    if (!aligned16(xq) || (x_scale && !aligned16(x_scale))) return VLA_ERR_ALIGN;
+    bool need_scale = false;
+    for (int j = 0; j < n_linears; ++j) {
+        const vla_prog_linear& l = lins[j];
+        if (l.out_dtype < 0 || l.out_dtype > 2) return VLA_ERR_DTYPE;
+        if (!l.packed || !l.out || (l.out_dtype != VLA_I32 && !l.w_scale)) return VLA_ERR_NULL;
+        if (l.N < 128 || l.N % 128 != 0) return VLA_ERR_SHAPE;
+        if (!aligned16(l.packed) || !aligned16(l.out) || (reinterpret_cast<uintptr_t>(l.w_scale) & 3u)) return VLA_ERR_ALIGN;
+        need_scale = need_scale || l.out_dtype != VLA_I32;
+    }
+    if (need_scale && !x_scale) return VLA_ERR_NULL;
+    const bool large = (path == VLA_PATH_LARGE) || (path == VLA_PATH_AUTO && vla_ternary_auto_path(M, lins[0].N, K) == VLA_PATH_LARGE);
+    if (!large) {                                           // small-M: one launch per linear (or use a program)
+        for (int j = 0; j < n_linears; ++j) {
+            vla_status st = vla_ternary_gemm(lins[j].packed, lins[j].w_scale, xq, x_scale, M, lins[j].N, K, lins[j].out,
+                                             (vla_dtype)lins[j].out_dtype, path, nullptr, 0, stream);
+            if (st != VLA_OK) return st;
+        }
+        return VLA_OK;
+    }
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return VLA_ERR_ARCH;
+    }
+    if (major != 10) return VLA_ERR_ARCH;
+    vla::LgGroup g = {};
+    g.n = n_linears;
+    g.ct_begin[0] = 0;
+    for (int j = 0; j < n_linears; ++j) {
+        g.packed[j] = reinterpret_cast<const uint8_t*>(lins[j].packed);
+        g.beta[j] = lins[j].w_scale;
+        g.out[j] = lins[j].out;
+        g.N[j] = lins[j].N;
+        g.dtype[j] = lins[j].out_dtype;
+        g.ct_begin[j + 1] = g.ct_begin[j] + lins[j].N / 128;
+    }
+    cudaError_t e = vla::launch_gemm_large_grouped(g, xq, x_scale, M, K, (cudaStream_t)stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+    return VLA_OK;
+}
+
 vla_status vla_program_release(const void* prog_dev) {
     if (!prog_dev) return VLA_ERR_NULL;
     std::lock_guard<std::mutex> lk(g_mu);

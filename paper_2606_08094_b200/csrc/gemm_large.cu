@@ -53,9 +53,8 @@ __device__ __forceinline__ uint4 lds128_nv(uint32_t addr) {
 }
 
 __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
-    const __grid_constant__ CUtensorMap tmap_x, const uint8_t* __restrict__ packed,
-    const float* __restrict__ w_scale, const float* __restrict__ x_scale, void* __restrict__ out,
-    int M, int N, int K, int TN, int NS, int out_dtype) {
+    const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ LgGroup grp,
+    const float* __restrict__ x_scale, int M, int K, int TN, int NS) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
@@ -77,7 +76,7 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int num_kb = K / TILE_K;
-    const int tiles_n = N / TILE_N, tiles_m = (M + TN - 1) / TN;
+    const int tiles_n = grp.ct_begin[grp.n], tiles_m = (M + TN - 1) / TN;      // channel tiles over all linears of the group
     const int ntiles = tiles_n * tiles_m;
     const uint32_t ns = (uint32_t)NS;
 
@@ -100,8 +99,11 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         if (lane < 4) {
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-                const int nb = tile % tiles_n;
-                const uint8_t* wsrc = packed + (size_t)(nb * 4 + lane) * num_kb * 1024;
+                const int ct = tile % tiles_n;
+                int li = 0;
+                for (int j = 1; j < grp.n; ++j) if (ct >= grp.ct_begin[j]) li = j;
+                const int nb = ct - grp.ct_begin[li];
+                const uint8_t* wsrc = grp.packed[li] + (size_t)(nb * 4 + lane) * num_kb * 1024;
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
                     const uint32_t s = it % LG_SW;
                     if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
@@ -194,13 +196,17 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     } else {
         // ---------------- epilogue warps ----------------
         const int lq = warp & 3;                              // TMEM lane quarter this warp may read
-        const float beta = (out_dtype == 2) ? 0.0f : *w_scale;
         float* sc = pScale + lq * 256;                        // this warp's alpha_m * beta of the tile's tokens
         const uint32_t sc_addr = sW + LG_SW * LG_W_BYTES + (uint32_t)lq * 1024u;
         pdl_wait();                                           // x_scale comes from the previous kernel
         uint32_t ti = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++ti) {
-            const int nb = tile % tiles_n, m0 = (tile / tiles_n) * TN;
+            const int ct = tile % tiles_n, m0 = (tile / tiles_n) * TN;
+            int li = 0;
+            for (int j = 1; j < grp.n; ++j) if (ct >= grp.ct_begin[j]) li = j;
+            const int nb = ct - grp.ct_begin[li], N = grp.N[li], out_dtype = grp.dtype[li];
+            void* __restrict__ out = grp.out[li];
+            const float beta = (out_dtype == 2) ? 0.0f : *grp.beta[li];
             const uint32_t ab = ti & 1;
             const int ch = nb * TILE_N + lq * 32 + lane;
             if (out_dtype != 2)
@@ -309,8 +315,9 @@ static int pick_tn(int M, int N, int sms) {
     return best;
 }
 
-cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
-                              int M, int N, int K, void* out, int out_dtype, cudaStream_t s) {
+cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const float* x_scale, int M, int K,
+                                      cudaStream_t s) {
+    const int N = g.ct_begin[g.n] * TILE_N;                  // all channels of the group
     EncodeTiledFn enc = get_encode();
     if (!enc) return cudaErrorNotSupported;
     static int sms = 0;
@@ -354,8 +361,21 @@ cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const in
     cfg.attrs = at;
     cfg.numAttrs = 1;
     count_launch();
-    return cudaLaunchKernelEx(&cfg, gemm_large_kernel, tm, (const uint8_t*)packed, w_scale, x_scale, out,
-                              M, N, K, TN, NS, out_dtype);
+    return cudaLaunchKernelEx(&cfg, gemm_large_kernel, tm, g, x_scale, M, K, TN, NS);
+}
+
+cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
+                              int M, int N, int K, void* out, int out_dtype, cudaStream_t s) {
+    LgGroup g = {};
+    g.packed[0] = (const uint8_t*)packed;
+    g.beta[0] = w_scale;
+    g.out[0] = out;
+    g.N[0] = N;
+    g.dtype[0] = out_dtype;
+    g.ct_begin[0] = 0;
+    g.ct_begin[1] = N / TILE_N;
+    g.n = 1;
+    return launch_gemm_large_grouped(g, xq, x_scale, M, K, s);
 }
 
 // ---------------------------------------------------------------- INT8 tensor-pipe issue-rate probe

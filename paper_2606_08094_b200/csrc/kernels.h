@@ -17,6 +17,17 @@ cudaError_t launch_act_quant(const void* x_bf16, int M, int K, int8_t* xq, float
 // out_dtype: 0 fp32, 1 bf16, 2 raw int32 (vla_dtype)
 cudaError_t launch_gemm_small(bool use_mma, const void* packed, const float* w_scale, const int8_t* xq,
                               const float* x_scale, int M, int N, int K, void* out, int out_dtype, cudaStream_t s);
+// up to 8 ternary linears that share one activation matrix, run as ONE tcgen05 launch (per-output-group scales)
+struct LgGroup {
+    const uint8_t* packed[8];
+    const float* beta[8];
+    void* out[8];
+    int N[8];
+    int dtype[8];
+    int ct_begin[9];           // prefix sum of N / 128 (channel tiles)
+    int n;
+};
+cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const float* x_scale, int M, int K, cudaStream_t s);
 cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
                               int M, int N, int K, void* out, int out_dtype, cudaStream_t s);
 // persistent program kernel (gemm_program.cu); the program header travels as a kernel parameter

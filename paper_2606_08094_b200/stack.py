@@ -70,15 +70,20 @@ class Stack:
         M = self.M
         self.xq = {K: torch.empty((M, K), dtype=torch.int8, device=self.device) for K in (2560, 6912)}
         self.xs = torch.empty((M,), dtype=torch.float32, device=self.device)
+        self._groups = {}
 
     def run_stack_calls(self):
-        """One activation quant per stage and one GEMM call per linear (any M; the large-M route)."""
+        """One activation quant per stage and one grouped GEMM call per stage (any M; one tcgen05 launch per stage for
+        M > 32, one launch per linear otherwise)."""
         M = self.M
         for layer in range(self.layers):
             for (src, names) in STAGES:
                 x = self._input_of(layer, src)
                 K = _DIMS[names[0]][0]
                 vla.vla_act_quant(x, M, K, self.xq[K], self.xs)
-                for n in names:
-                    vla.vla_ternary_gemm(self.packed[layer][n], self.beta[layer][n], self.xq[K], self.xs, M,
-                                         _DIMS[n][1], K, self.out[layer][n], vla.VLA_BF16, vla.VLA_PATH_AUTO, None, 0)
+                key = (layer, src)
+                if key not in self._groups:
+                    self._groups[key] = vla.make_linears(
+                        [dict(packed=self.packed[layer][n], w_scale=self.beta[layer][n], out=self.out[layer][n],
+                              N=_DIMS[n][1], out_dtype=vla.VLA_BF16) for n in names])
+                vla.vla_ternary_gemm_grouped(self._groups[key], self.xq[K], self.xs, M, K)

@@ -352,3 +352,33 @@ def test_full_size_large_m_sampled_channels(vla, oracle, M, K, N):
             assert np.all(np.abs(got.astype(np.float64) - ref["y64"]) <= REL_TOL_F32 * np.abs(ref["y64"]))
     assert np.array_equal(xq.cpu().numpy(), ref["a"])
     assert np.array_equal(xs.cpu().numpy().view(np.uint32), ref["alpha"].view(np.uint32))
+
+
+def test_grouped_large_gemm_per_group_scales(vla, oracle):
+    """q|k|v-style group: three linears with their own beta and output type share one quantised activation matrix and
+    run as ONE tcgen05 launch (Eq. 4's per-output-group scales); ragged M, every linear vs the oracle."""
+    M, K = 200, 640
+    x_bits = synth.activations(M, K, 4242, outlier_frac=0.01)
+    x = dev_bf16(x_bits)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(x, M, K, xq, xs)
+    specs = [(256, vla.VLA_BF16, 0.05), (128, vla.VLA_F32, 0.013), (384, vla.VLA_I32, 0.5)]
+    lins, keep = [], []
+    for i, (N, dt, beta) in enumerate(specs):
+        w = synth.ternary_weights(N, K, 0.35, 900 + i)
+        packed = vla.pack_weights(dev(w))
+        beta_d = dev(np.array([beta], np.float32))
+        out = vla.empty_out(M, N, dt)
+        keep.append((w, packed, beta_d, out, np.float32(beta), dt))
+        lins.append(dict(packed=packed, w_scale=beta_d, out=out, N=N, out_dtype=dt))
+    vla.vla_ternary_gemm_grouped(lins, xq, xs, M, K, vla.VLA_PATH_LARGE)
+    torch.cuda.synchronize()
+    for (w, packed, beta_d, out, beta, dt) in keep:
+        ref = oracle.ternary_linear(x_bits, w, beta)
+        if dt == vla.VLA_I32:
+            assert np.array_equal(out.cpu().numpy(), ref["acc"])
+        elif dt == vla.VLA_F32:
+            assert np.array_equal(out.cpu().numpy().view(np.uint32), ref["y32"].view(np.uint32))
+        else:
+            assert np.array_equal(bf16_bits_of(out), ref["ybf16"])
