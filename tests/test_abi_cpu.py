@@ -117,3 +117,17 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 text = open(os.path.join(dirpath, f), errors="ignore").read()
                 assert "import oracle" not in text and "from oracle" not in text and "liboracle" not in text, f
+
+
+def test_grouped_gemm_validates_on_the_host(vla):
+    fake = 0x1000
+    arr = vla.make_linears([dict(packed=fake, w_scale=fake, out=fake, N=256, out_dtype=1)])
+    L = vla._lib
+    assert L.vla_ternary_gemm_grouped(None, 1, fake, fake, 64, 256, 0, None) == vla.VLA_ERR_NULL
+    assert L.vla_ternary_gemm_grouped(arr, 0, fake, fake, 64, 256, 0, None) == vla.VLA_ERR_SHAPE
+    assert L.vla_ternary_gemm_grouped(arr, 9, fake, fake, 64, 256, 0, None) == vla.VLA_ERR_SHAPE
+    assert L.vla_ternary_gemm_grouped(arr, 1, fake, fake, 64, 200, 0, None) == vla.VLA_ERR_SHAPE
+    assert L.vla_ternary_gemm_grouped(arr, 1, fake + 4, fake, 64, 256, 0, None) == vla.VLA_ERR_ALIGN
+    assert L.vla_ternary_gemm_grouped(arr, 1, fake, None, 64, 256, 0, None) == vla.VLA_ERR_NULL
+    bad = vla.make_linears([dict(packed=fake, w_scale=fake, out=fake, N=100, out_dtype=1)])
+    assert L.vla_ternary_gemm_grouped(bad, 1, fake, fake, 64, 256, 0, None) == vla.VLA_ERR_SHAPE

@@ -173,3 +173,42 @@ def test_program_errors(vla):
     with pytest.raises(vla.VlaError) as e:
         vla.vla_program_run(p["out"])          # not a compiled program
     assert e.value.status == vla.VLA_ERR_VALUE
+
+
+def test_mixed_phases_and_token_counts(vla, oracle):
+    """Phase 0: two independent stages (M=8 and M=3); phase 1: a stage that reads phase 0's bf16 output (depends=1)
+    plus an independent M=16 stage that joins it; phase 2: another dependent stage.  Every output vs the oracle."""
+    def lin(N, K, seed, dt=1):
+        w = synth.ternary_weights(N, K, 0.35, seed)
+        beta = synth.weight_scale(seed + 1)
+        return dict(w=w, beta=beta, packed=vla.pack_weights(dev(w)), beta_d=dev(np.array([beta], np.float32)), N=N, K=K, dt=dt)
+    xa = synth.activations(8, 256, 11)
+    xb = synth.activations(3, 512, 12, outlier_frac=0.01)
+    xd = synth.activations(16, 128, 13)
+    A, B, C, D, E_ = lin(384, 256, 21), lin(128, 512, 22, dt=0), lin(256, 384, 23), lin(640, 128, 24, dt=2), lin(128, 256, 25, dt=0)
+    ya = torch.zeros((8, 384), dtype=torch.bfloat16, device="cuda")
+    yb = torch.zeros((3, 128), dtype=torch.float32, device="cuda")
+    yc = torch.zeros((8, 256), dtype=torch.bfloat16, device="cuda")
+    yd = torch.zeros((16, 640), dtype=torch.int32, device="cuda")
+    ye = torch.zeros((8, 128), dtype=torch.float32, device="cuda")
+    def stage(x, M, L, out, depends):
+        return dict(x=x, M=M, K=L["K"], depends=depends,
+                    linears=[dict(packed=L["packed"], w_scale=L["beta_d"], out=out, N=L["N"], out_dtype=L["dt"])])
+    stages = [stage(dev_bf16(xa), 8, A, ya, 0), stage(dev_bf16(xb), 3, B, yb, 0),
+              stage(ya, 8, C, yc, 1), stage(dev_bf16(xd), 16, D, yd, 0),
+              stage(yc, 8, E_, ye, 1)]
+    keep = [s["x"] for s in stages]
+    prog = vla.compile_program(stages)
+    for _ in range(2):
+        vla.vla_program_run(prog)
+    torch.cuda.synchronize()
+    ra = oracle.ternary_linear(xa, A["w"], A["beta"])
+    rb = oracle.ternary_linear(xb, B["w"], B["beta"])
+    rc = oracle.ternary_linear(ra["ybf16"], C["w"], C["beta"])
+    rd = oracle.ternary_linear(xd, D["w"], D["beta"])
+    re_ = oracle.ternary_linear(rc["ybf16"], E_["w"], E_["beta"])
+    assert np.array_equal(bits(ya), ra["ybf16"])
+    assert np.array_equal(yb.cpu().numpy().view(np.uint32), rb["y32"].view(np.uint32))
+    assert np.array_equal(bits(yc), rc["ybf16"])
+    assert np.array_equal(yd.cpu().numpy(), rd["acc"])
+    assert np.array_equal(ye.cpu().numpy().view(np.uint32), re_["y32"].view(np.uint32))
