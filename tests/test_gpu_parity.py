@@ -382,3 +382,29 @@ def test_grouped_large_gemm_per_group_scales(vla, oracle):
             assert np.array_equal(out.cpu().numpy().view(np.uint32), ref["y32"].view(np.uint32))
         else:
             assert np.array_equal(bf16_bits_of(out), ref["ybf16"])
+
+
+@pytest.mark.parametrize("M,path_name", [(7, "small_tc"), (7, "small_alu"), (37, "large"), (200, "large")])
+def test_guard_bands_single_calls(vla, oracle, M, path_name):
+    """Sentinel bytes around xq, alpha and the output survive act_quant + GEMM on every path (ragged M)."""
+    path = {"small_tc": vla.VLA_PATH_SMALL_TC, "small_alu": vla.VLA_PATH_SMALL_ALU, "large": vla.VLA_PATH_LARGE}[path_name]
+    K, N = 384, 256
+    def guarded(shape, dtype):
+        n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+        raw = torch.full((n + 8192,), 0xA5, dtype=torch.uint8, device="cuda")
+        return raw, raw[4096:4096 + n].view(dtype).view(*shape)
+    x_bits = synth.activations(M, K, 55 + M)
+    w = synth.ternary_weights(N, K, 0.35, 56)
+    beta = np.float32(0.07)
+    rq, xq = guarded((M, K), torch.int8)
+    rs, xs = guarded((M,), torch.float32)
+    ro, out = guarded((M, N), torch.float32)
+    packed = vla.pack_weights(dev(w))
+    vla.vla_act_quant(dev_bf16(x_bits), M, K, xq, xs)
+    vla.vla_ternary_gemm(packed, dev(np.array([beta], np.float32)), xq, xs, M, N, K, out, vla.VLA_F32, path, None, 0)
+    torch.cuda.synchronize()
+    ref = oracle.ternary_linear(x_bits, w, beta)
+    assert np.array_equal(out.cpu().numpy().view(np.uint32), ref["y32"].view(np.uint32))
+    for raw in (rq, rs, ro):
+        r = raw.cpu().numpy()
+        assert (r[:4096] == 0xA5).all() and (r[-4096:] == 0xA5).all(), "a kernel wrote outside its buffer"

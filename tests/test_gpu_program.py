@@ -212,3 +212,73 @@ def test_mixed_phases_and_token_counts(vla, oracle):
     assert np.array_equal(bits(yc), rc["ybf16"])
     assert np.array_equal(yd.cpu().numpy(), rd["acc"])
     assert np.array_equal(ye.cpu().numpy().view(np.uint32), re_["y32"].view(np.uint32))
+
+
+def _guarded(shape, dtype, fill):
+    """tensor view with 4 KiB of sentinel bytes on both sides (a hand-made out-of-bounds-write detector)"""
+    n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+    raw = torch.full((n + 8192,), 0xA5, dtype=torch.uint8, device="cuda")
+    view = raw[4096:4096 + n].view(dtype).view(*shape)
+    view.fill_(fill)
+    return raw, view
+
+
+def _guards_intact(raw):
+    r = raw.cpu().numpy()
+    return bool((r[:4096] == 0xA5).all() and (r[-4096:] == 0xA5).all())
+
+
+def test_guard_bands_and_repeatability(vla, oracle):
+    """No kernel writes outside its outputs (sentinels around every output, xq and alpha buffer survive), and 200
+    back-to-back replays of a program with cross-CTA flags give the same bits every time (ragged shapes, M = 5 / 13)."""
+    M, K = 5, 384
+    x_bits = synth.activations(M, K, 321, outlier_frac=0.01)
+    specs = [(128, 1), (384, 0), (256, 2)]
+    raws, lins, refs = [], [], []
+    for i, (N, dt) in enumerate(specs):
+        w = synth.ternary_weights(N, K, 0.35, 700 + i)
+        beta = synth.weight_scale(710 + i)
+        raw, out = _guarded((M, N), _TDT[dt], 0)
+        raws.append(raw)
+        lins.append(dict(packed=vla.pack_weights(dev(w)), w_scale=dev(np.array([beta], np.float32)), out=out, N=N, out_dtype=dt))
+        refs.append((oracle.ternary_linear(x_bits, w, beta), dt, out))
+    rq, xq = _guarded((M, K), torch.int8, 0)
+    rs, xs = _guarded((M,), torch.float32, 0)
+    raws += [rq, rs]
+    # second phase: M = 13 reads the bf16 output of the first linear (N = 128 -> K = 128)
+    M2 = 13
+    x2_bits = synth.activations(M2, 128, 322)
+    w2 = synth.ternary_weights(640, 128, 0.35, 720)
+    b2 = synth.weight_scale(721)
+    raw2, out2 = _guarded((M2, 640), torch.bfloat16, 0)
+    raws.append(raw2)
+    stages = [dict(x=dev_bf16(x_bits), M=M, K=K, depends=0, linears=lins, xq_opt=xq, x_scale_opt=xs),
+              dict(x=dev_bf16(x2_bits), M=M2, K=128, depends=1,
+                   linears=[dict(packed=vla.pack_weights(dev(w2)), w_scale=dev(np.array([b2], np.float32)), out=out2, N=640, out_dtype=1)])]
+    keep = [s["x"] for s in stages]
+    prog = vla.compile_program(stages)
+    g = torch.cuda.CUDAGraph()
+    vla.vla_program_run(prog)
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g):
+        for _ in range(20):
+            vla.vla_program_run(prog)
+    first = None
+    for rep in range(10):                                     # 200 runs
+        g.replay()
+        torch.cuda.synchronize()
+        snap = [o.clone() for (_, _, o) in refs] + [out2.clone()]
+        if first is None:
+            first = snap
+        else:
+            assert all(torch.equal(a.view(torch.uint8), b.view(torch.uint8)) for a, b in zip(first, snap)), "run-to-run difference"
+    for ref, dt, out in refs:
+        if dt == 2:
+            assert np.array_equal(out.cpu().numpy(), ref["acc"])
+        elif dt == 0:
+            assert np.array_equal(out.cpu().numpy().view(np.uint32), ref["y32"].view(np.uint32))
+        else:
+            assert np.array_equal(bits(out), ref["ybf16"])
+    assert np.array_equal(xq.cpu().numpy(), refs[0][0]["a"])
+    assert np.array_equal(bits(out2), oracle.ternary_linear(x2_bits, w2, b2)["ybf16"])
+    assert all(_guards_intact(r) for r in raws), "a kernel wrote outside its buffer"
