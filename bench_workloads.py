@@ -155,6 +155,39 @@ def run_sweep(args, pk, clock_sampler, int8_probe_tops):
                 del x_all
             del ring
             torch.cuda.empty_cache()
+    # NEXT-3: the paper's dp4a -> tensor-core comparison (4.0-4.6x end to end at S=8 on RTX 3060 / AGX Orin,
+    # PAPER.md line 130) restated kernel to kernel on this B200 at M=8: same packed weights, same pre-quantised
+    # activations, VLA_PATH_SMALL_ALU (dp4a on the integer ALUs) vs VLA_PATH_SMALL_TC (IMMA), cold ring, CUDA graph.
+    compare = []
+    for si, (K, N) in enumerate(synth.MODEL_SHAPES):
+        M = 8
+        copies = max(2, -(-2 * l2 // (N * K // 4)))
+        w = synth.ternary_weights(N, K, 0.35, 4900 + si)
+        packed1 = vla.pack_weights(torch.from_numpy(w).to(dev))
+        ring = packed1.unsqueeze(0).repeat(copies, 1).contiguous()
+        del w, packed1
+        beta = torch.tensor([0.05], dtype=torch.float32, device=dev)
+        xq = torch.randint(-127, 128, (M, K), dtype=torch.int8, device=dev)
+        xs = torch.rand(M, device=dev) + 0.01
+        out = torch.empty((M, N), dtype=torch.bfloat16, device=dev)
+        row = {"M": M, "K": K, "N": N}
+        for name, path in (("dp4a_us", vla.VLA_PATH_SMALL_ALU), ("imma_us", vla.VLA_PATH_SMALL_TC)):
+            ncall = min(copies, 64)
+
+            def calls():
+                for c in range(ncall):
+                    vla.vla_ternary_gemm(ring[c], beta, xq, xs, M, N, K, out, vla.VLA_BF16, path, None, 0)
+            calls()
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                calls()
+            row[name] = _time(torch, g.replay, 10) / ncall * 1e6
+            del g
+        row["imma_over_dp4a"] = row["dp4a_us"] / row["imma_us"]
+        compare.append(row)
+        del ring
+        torch.cuda.empty_cache()
     clocks = sampler.stop()
     big = [p for p in pts if p["M"] >= 512]
     small = [p for p in pts if p["M"] <= 16]
@@ -176,6 +209,7 @@ def run_sweep(args, pk, clock_sampler, int8_probe_tops):
             "M<=16 single-call roofline_frac median": float(np.median([p["roofline_frac"] for p in small])) if small else None,
             "M<=16 streaming roofline_frac median": float(np.median([p["stream_roofline_frac"] for p in small
                                                                      if "stream_roofline_frac" in p])) if small else None},
+        "dp4a_vs_imma_M8": compare,
         "points": pts,
     }
     print(json.dumps(line))
