@@ -52,19 +52,24 @@ __device__ __forceinline__ uint4 lds128_nv(uint32_t addr) {
     return r;
 }
 
+// KS = k blocks (of 128) per pipeline stage: 2 for narrow token tiles (eight MMAs per full/empty handoff), else 1.
+template <int KS>
 __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ LgGroup grp,
     const float* __restrict__ x_scale, int M, int K, int TN, int NS) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
-    const uint32_t stride = lg_stage_stride(TN);
+    const uint32_t x_tile = ((uint32_t)TN * TILE_K + 1023u) & ~1023u;
+    const uint32_t stride = KS * (LG_A_BYTES + x_tile);               // [A x KS | X x KS]
+    constexpr uint32_t X_OFF = KS * LG_A_BYTES;
+    constexpr uint32_t W_STAGE = KS * LG_W_BYTES;
     const uint32_t sS = base;                                           // [NS]{A 16384 | X TN*128}
     const uint32_t sW = sS + (uint32_t)NS * stride;                     // [SW][4096]
-    const uint32_t sBar = sW + LG_SW * LG_W_BYTES + LG_SCALE_BYTES;
+    const uint32_t sBar = sW + LG_SW * W_STAGE + LG_SCALE_BYTES;
     uint8_t* pS = base_ptr;
     uint8_t* pW = base_ptr + (size_t)NS * stride;
-    float* pScale = reinterpret_cast<float*>(pW + LG_SW * LG_W_BYTES);
+    float* pScale = reinterpret_cast<float*>(pW + LG_SW * W_STAGE);
     auto bar_full_w = [&](uint32_t s) { return sBar + 8u * s; };
     auto bar_empty_w = [&](uint32_t s) { return sBar + 8u * (LG_SW + s); };
     auto bar_full = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + s); };                  // A decoded + X landed
@@ -96,20 +101,21 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     if (warp == 0) {
         // ---------------- W producer ----------------
         // a 128 x 128 tile is four 1 KiB pieces (one per 32-channel group), 8*K bytes apart: lanes 0-3 copy one each
-        if (lane < 4) {
+        if (lane < 4 * KS) {
+            const int piece = lane & 3, kk = lane >> 2;
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const int ct = tile % tiles_n;
                 int li = 0;
                 for (int j = 1; j < grp.n; ++j) if (ct >= grp.ct_begin[j]) li = j;
                 const int nb = ct - grp.ct_begin[li];
-                const uint8_t* wsrc = grp.packed[li] + (size_t)(nb * 4 + lane) * num_kb * 1024;
-                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                const uint8_t* wsrc = grp.packed[li] + (size_t)(nb * 4 + piece) * num_kb * 1024;
+                for (int kb = 0; kb < num_kb; kb += KS, ++it) {
                     const uint32_t s = it % LG_SW;
                     if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
-                    if (lane == 0) mbar_arrive_expect_tx(bar_full_w(s), LG_W_BYTES);
-                    __syncwarp(0xF);
-                    tma_bulk_g2s(sW + s * LG_W_BYTES + lane * 1024, wsrc + (size_t)kb * 1024, 1024, bar_full_w(s));
+                    if (lane == 0) mbar_arrive_expect_tx(bar_full_w(s), W_STAGE);
+                    __syncwarp((1u << (4 * KS)) - 1u);
+                    tma_bulk_g2s(sW + s * W_STAGE + kk * LG_W_BYTES + piece * 1024, wsrc + (size_t)(kb + kk) * 1024, 1024, bar_full_w(s));
                 }
             }
         }
@@ -120,11 +126,13 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const int m0 = (tile / tiles_n) * TN;
-                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                for (int kb = 0; kb < num_kb; kb += KS, ++it) {
                     const uint32_t s = it % ns;
                     if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
-                    mbar_arrive_expect_tx(bar_full(s), (uint32_t)TN * TILE_K);
-                    tma_tensor2d_g2s(sS + s * stride + LG_A_BYTES, &tmap_x, kb * TILE_K, m0, bar_full(s));
+                    mbar_arrive_expect_tx(bar_full(s), (uint32_t)KS * TN * TILE_K);
+#pragma unroll
+                    for (int kk = 0; kk < KS; ++kk)
+                        tma_tensor2d_g2s(sS + s * stride + X_OFF + kk * x_tile, &tmap_x, (kb + kk) * TILE_K, m0, bar_full(s));
                 }
             }
         }
@@ -138,16 +146,19 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
                 if (ti >= 2) mbar_wait(bar_acc_empty(ab), ((ti >> 1) & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + ab * 256u;
-                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                for (int kb = 0; kb < num_kb; kb += KS, ++it) {
                     const uint32_t s = it % ns;
                     mbar_wait(bar_full(s), (it / ns) & 1);
                     tc_fence_after();
                     LG_STAMP(0, it);
-                    const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride);
-                    const uint64_t b_desc = umma_desc_k_sw128(sS + s * stride + LG_A_BYTES);
 #pragma unroll
-                    for (int k = 0; k < TILE_K / 32; ++k)
-                        mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0);
+                    for (int kk = 0; kk < KS; ++kk) {
+                        const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride + kk * LG_A_BYTES);
+                        const uint64_t b_desc = umma_desc_k_sw128(sS + s * stride + X_OFF + kk * x_tile);
+#pragma unroll
+                        for (int k = 0; k < TILE_K / 32; ++k)
+                            mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | kk | k) != 0);
+                    }
                     mma_commit(bar_empty(s));
                 }
                 mma_commit(bar_acc_full(ab));
@@ -161,27 +172,32 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         const int g = 2 * q + p;
         uint32_t it = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            for (int kb = 0; kb < num_kb; ++kb, ++it) {
+            for (int kb = 0; kb < num_kb; kb += KS, ++it) {
                 if ((int)(it & 1u) != dgrp) continue;
                 const uint32_t sw = it % LG_SW, s = it % ns;
                 mbar_wait(bar_full_w(sw), (it / LG_SW) & 1);
-                const uint8_t* wst = pW + sw * LG_W_BYTES;
-                uint4 wv[2];
+                const uint8_t* wst = pW + sw * W_STAGE;
+                uint4 wv[KS][2];
 #pragma unroll
-                for (int itx = 0; itx < 2; ++itx)
-                    wv[itx] = *reinterpret_cast<const uint4*>(wst + ((i32 * 2 + (p ^ itx)) * 32 + g * 4 + t) * 16);
+                for (int kk = 0; kk < KS; ++kk)
+#pragma unroll
+                    for (int itx = 0; itx < 2; ++itx)
+                        wv[kk][itx] = *reinterpret_cast<const uint4*>(wst + kk * LG_W_BYTES + ((i32 * 2 + (p ^ itx)) * 32 + g * 4 + t) * 16);
                 if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
                 if (threadIdx.x == 96) LG_STAMP(1, it);
-                uint8_t* ast = pS + s * stride;
 #pragma unroll
-                for (int itx = 0; itx < 2; ++itx) {
-                    const int h = p ^ itx;
-                    const uint32_t w4[4] = {wv[itx].x, wv[itx].y, wv[itx].z, wv[itx].w};
-                    const int pos = (4 * h + t) ^ g;          // SWIZZLE_128B: 16-byte chunk index ^ (row & 7)
+                for (int kk = 0; kk < KS; ++kk) {
+                    uint8_t* ast = pS + s * stride + kk * LG_A_BYTES;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        uint4 o = make_uint4(decode64<0>(w4[j]), decode64<1>(w4[j]), decode64<2>(w4[j]), decode64<3>(w4[j]));
-                        *reinterpret_cast<uint4*>(ast + (i32 * 4 + j) * 1024 + g * 128 + pos * 16) = o;
+                    for (int itx = 0; itx < 2; ++itx) {
+                        const int h = p ^ itx;
+                        const uint32_t w4[4] = {wv[kk][itx].x, wv[kk][itx].y, wv[kk][itx].z, wv[kk][itx].w};
+                        const int pos = (4 * h + t) ^ g;      // SWIZZLE_128B: 16-byte chunk index ^ (row & 7)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            uint4 o = make_uint4(decode64<0>(w4[j]), decode64<1>(w4[j]), decode64<2>(w4[j]), decode64<3>(w4[j]));
+                            *reinterpret_cast<uint4*>(ast + (i32 * 4 + j) * 1024 + g * 128 + pos * 16) = o;
+                        }
                     }
                 }
                 fence_proxy_async_smem();                     // generic-proxy stores -> visible to the tensor core
@@ -197,7 +213,7 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         // ---------------- epilogue warps ----------------
         const int lq = warp & 3;                              // TMEM lane quarter this warp may read
         float* sc = pScale + lq * 256;                        // this warp's alpha_m * beta of the tile's tokens
-        const uint32_t sc_addr = sW + LG_SW * LG_W_BYTES + (uint32_t)lq * 1024u;
+        const uint32_t sc_addr = sW + LG_SW * W_STAGE + (uint32_t)lq * 1024u;
         pdl_wait();                                           // x_scale comes from the previous kernel
         uint32_t ti = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++ti) {
@@ -278,6 +294,11 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+static int env_ks() {
+    const char* v = std::getenv("VLA_TUNE_KS");                 // tuning aid: force the k blocks per stage (1 or 2)
+    return v ? std::atoi(v) : 0;
+}
+
 static int env_tn() {
     const char* v = std::getenv("VLA_TUNE_TN");                 // tuning aid: force the token-tile width
     return v ? std::atoi(v) : 0;
@@ -300,7 +321,7 @@ static EncodeTiledFn get_encode() {
 // Measured on B200 (profiles/): a k block costs ~540 cycles at TN = 96 and ~610 at TN = 256 -- the shared-memory
 // traffic of decode + operand fetch dominates, not the 2*TN cycles of the MMAs -- so cycles ~ 500 + 0.42*TN.
 // Ties go to the wider tile (fewer re-decodes of the same weights).
-static int pick_tn(int M, int N, int sms) {
+static int pick_tn(int M, int N, int sms, bool k_even) {
     int best = 16;
     double best_cost = 1e30;
     for (int tn = 16; tn <= 256; tn += 16) {
@@ -308,7 +329,8 @@ static int pick_tn(int M, int N, int sms) {
         if (tn > 16 && (tiles_m * (tn - 16) >= M)) continue;          // a narrower tile covers M with the same count
         const long tiles = (long)tiles_m * (N / TILE_N);
         const long waves = (tiles + sms - 1) / sms;
-        const double per_kb = 500.0 + 0.42 * tn;
+        // narrow tiles run two k blocks per stage (KS = 2): 0.21 us = ~410 cycles per k block at TN = 96
+        const double per_kb = ((tn <= 112 && k_even) ? 370.0 : 500.0) + 0.42 * tn;
         const double cost = (double)waves * per_kb;
         if (cost <= best_cost) { best_cost = cost; best = tn; }
     }
@@ -328,7 +350,7 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
         if (sms <= 0) sms = 148;
     }
     static const int tune_tn = env_tn();
-    const int TN = tune_tn > 0 ? tune_tn : pick_tn(M, N, sms);
+    const int TN = tune_tn > 0 ? tune_tn : pick_tn(M, N, sms, (K / TILE_K) % 2 == 0);
 
     CUtensorMap tm;
     cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)M};
@@ -342,14 +364,21 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
 
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_large_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     const int ntiles = (N / TILE_N) * ((M + TN - 1) / TN);
-    int NS = LG_STAGE_REGION / (int)lg_stage_stride(TN);
+    // narrow token tiles: two k blocks per stage (the MMAs of a 128 x TN x 32 step have a 31 ns floor for TN <= 112,
+    // so four of them do not cover one full/empty handoff; eight do)
+    static const int tune_ks = env_ks();
+    const int KS = (tune_ks > 0) ? tune_ks : ((TN <= 112 && (K / TILE_K) % 2 == 0) ? 2 : 1);
+    const int stage = KS * (int)lg_stage_stride(TN);
+    const int sw_bytes = LG_SW * KS * LG_W_BYTES;
+    int NS = (LG_STAGE_REGION + LG_SW * LG_W_BYTES - sw_bytes) / stage;
     if (NS > LG_NS_MAX) NS = LG_NS_MAX;
-    const int smem = NS * (int)lg_stage_stride(TN) + LG_FIXED_SMEM;
+    const int smem = NS * stage + sw_bytes + LG_SCALE_BYTES + 1024 + 8 * LG_NBAR + 16;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(ntiles < sms ? ntiles : sms));
     cfg.blockDim = dim3(LG_THREADS);
@@ -361,7 +390,8 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     cfg.attrs = at;
     cfg.numAttrs = 1;
     count_launch();
-    return cudaLaunchKernelEx(&cfg, gemm_large_kernel, tm, g, x_scale, M, K, TN, NS);
+    if (KS == 2) return cudaLaunchKernelEx(&cfg, gemm_large_kernel<2>, tm, g, x_scale, M, K, TN, NS);
+    return cudaLaunchKernelEx(&cfg, gemm_large_kernel<1>, tm, g, x_scale, M, K, TN, NS);
 }
 
 cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
