@@ -6,7 +6,7 @@
 //
 // Grid: one CTA per SM, 16 warps.
 //   warp 15 (producer)   streams this CTA's share of the packed weights of EVERY stage, in program order, through
-//                        a 12 x 15 KiB shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
+//                        a 6 x 30 KiB shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
 //                        activations, so HBM stays busy across stage boundaries and grid barriers.
 //   warps 0-14 (consumers) per stage: hold the int8 activations as mma.m16n8k32 B fragments IN REGISTERS (warp w
 //                        owns the 64-wide k blocks kq = w mod 15), read packed words from the ring, decode them
@@ -37,12 +37,14 @@ namespace vla {
 constexpr int PG_W = 15;                         // consumer warps
 constexpr int PG_CONSUMERS = PG_W * 32;          // 480 threads
 constexpr int PG_THREADS = PG_CONSUMERS + 32;    // 512
-constexpr int PG_CHUNK_PIECES = PG_W;            // 15 pieces of 1 KiB = 30 blocks of 32 ch x 64 k: two per warp
+constexpr int PG_BPW = 4;                         // 512-byte blocks per warp per chunk (one mbarrier wait / release)
+constexpr int PG_CHUNK_PIECES = PG_W * PG_BPW / 2;   // 30 pieces of 1 KiB = 60 blocks of 32 ch x 64 k: four per warp
 constexpr int PG_SLOT_BYTES = PG_CHUNK_PIECES * 1024;
 constexpr int PG_XHI_BYTES = 65536;              // M <= 16 variant: B fragments of tokens 8-15 (8 * K bytes, K <= 8192)
-__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 12 : 7; }
+__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 6 : 3; }
 constexpr int PG_DESC_BYTES = 15360;             // stage + linear descriptors cached in shared memory
-constexpr int PG_NBMAX = 10;                     // k blocks per warp per granule (5 chunks x 2)  ->  K <= 8192
+constexpr int PG_NBMAX = 9;                      // k blocks per warp per granule: ceil(128 / 15)  ->  K <= 8192
+constexpr int PG_NCHUNK = 3;                     // chunks of 60 blocks that cover 128 blocks
 constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 7920 ints = 31 680 B
 __host__ __device__ constexpr int pg_smem(int maxmt) {
     return pg_nslot(maxmt) * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + (maxmt == 1 ? 0 : PG_XHI_BYTES) +
@@ -110,7 +112,7 @@ __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uin
 template <int NSLOT>
 __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, int cta,
                                          int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty, uint32_t bar_go) {
-    // The first two chunks go out at once; the rest of the ring is filled only after this CTA's consumers have seen
+    // The first chunk goes out at once; the rest of the ring is filled only after this CTA's consumers have seen
     // their first quantised activations: otherwise 148 rings (26 MB) are requested in the first microsecond and the
     // few KB of activation rows the quant owners need queue behind them (measured: 2.5-10 us before the first MMA).
     uint32_t slot = 0, round = 0, issued = 0;
@@ -127,7 +129,7 @@ __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stage
             const uint8_t* src = lins[l].packed + (size_t)n32 * KB * 1024;      // the granule is one contiguous run
             for (int p0 = 0; p0 < KB; p0 += PG_CHUNK_PIECES) {
                 const int np = min(PG_CHUNK_PIECES, KB - p0);
-                if (issued == 2) mbar_wait(bar_go, 0);
+                if (issued == 1) mbar_wait(bar_go, 0);
                 ++issued;
                 if (round > 0) mbar_wait(bar_empty + 8u * slot, (round - 1) & 1);
                 if (lane == 0) {                              // one bulk copy of up to 15 KiB per chunk
@@ -280,7 +282,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
         }
 
 #pragma unroll
-        for (int ck = 0; ck < PG_NBMAX / 2; ++ck) {           // 5 chunks of 15 KiB cover K <= 8192
+        for (int ck = 0; ck < PG_NCHUNK; ++ck) {              // 3 chunks of 30 KiB cover K <= 8192
             if (ck < nchunks) {
 #ifdef VLA_PROG_TRACE
                 long long tw0 = clock64();
@@ -289,36 +291,45 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
 #ifdef VLA_PROG_TRACE
                 twait += clock64() - tw0;
 #endif
-                // both blocks of this warp in the chunk -> registers, then hand the slot back at once
-                uint4 wv[2];
+                // the four blocks of this warp in the chunk, two at a time; the slot is handed back once the last two
+                // are in registers
 #pragma unroll
-                for (int ii = 0; ii < 2; ++ii)
-                    wv[ii] = ((2 * ck + ii) * PG_W + w < nblk) ? lds128(ring + slot * PG_SLOT_BYTES + ii * (PG_W * 512) + my_off)
-                                                               : make_uint4(0, 0, 0, 0);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_empty + 8u * slot);       // release: ordered after the loads above
-                if (++slot == NSLOT) { slot = 0; phase ^= 1; }
+                for (int half = 0; half < PG_BPW / 2; ++half) {
+                    uint4 wv[2];
 #pragma unroll
-                for (int ii = 0; ii < 2; ++ii) {
-                    const int i = 2 * ck + ii;
-                    if (i * PG_W + w < nblk) {
-                        const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
-                        uint4 xh = make_uint4(0, 0, 0, 0);    // tokens 8-15 of this block (M <= 16 variant)
-                        if (MT == 2) xh = lds128(xhi + (uint32_t)((i * PG_W + w) * 32 + lane) * 16u);
+                    for (int ii = 0; ii < 2; ++ii) {
+                        const int i = PG_BPW * ck + 2 * half + ii;
+                        wv[ii] = (i < PG_NBMAX && i * PG_W + w < nblk)
+                                     ? lds128(ring + slot * PG_SLOT_BYTES + (2 * half + ii) * (PG_W * 512) + my_off)
+                                     : make_uint4(0, 0, 0, 0);
+                    }
+                    if (half == PG_BPW / 2 - 1) {
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_empty + 8u * slot);   // release: ordered after the loads above
+                    }
 #pragma unroll
-                        for (int c = 0; c < 2; ++c) {
-                            const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];     // channels 16c+g and 16c+g+8
-                            const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
-                            const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
-                            mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xv[i].x, xv[i].y);
-                            mma_m16n8k32_s8_nv(acc2[c], e0, e1, e2, e3, xv[i].z, xv[i].w);
-                            if (MT == 2) {
-                                mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh.x, xh.y);
-                                mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh.z, xh.w);
+                    for (int ii = 0; ii < 2; ++ii) {
+                        const int i = PG_BPW * ck + 2 * half + ii;
+                        if (i < PG_NBMAX && i * PG_W + w < nblk) {
+                            const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
+                            uint4 xh = make_uint4(0, 0, 0, 0);    // tokens 8-15 of this block (M <= 16 variant)
+                            if (MT == 2) xh = lds128(xhi + (uint32_t)((i * PG_W + w) * 32 + lane) * 16u);
+#pragma unroll
+                            for (int c = 0; c < 2; ++c) {
+                                const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];     // channels 16c+g and 16c+g+8
+                                const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
+                                const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
+                                mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xv[i < PG_NBMAX ? i : 0].x, xv[i < PG_NBMAX ? i : 0].y);
+                                mma_m16n8k32_s8_nv(acc2[c], e0, e1, e2, e3, xv[i < PG_NBMAX ? i : 0].z, xv[i < PG_NBMAX ? i : 0].w);
+                                if (MT == 2) {
+                                    mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh.x, xh.y);
+                                    mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh.z, xh.w);
+                                }
                             }
                         }
                     }
                 }
+                if (++slot == NSLOT) { slot = 0; phase ^= 1; }
             }
         }
 
