@@ -52,7 +52,7 @@ __device__ __forceinline__ uint4 lds128_nv(uint32_t addr) {
     return r;
 }
 
-// KS = k blocks (of 128) per pipeline stage: 2 for narrow token tiles (eight MMAs per full/empty handoff), else 1.
+// KS = k blocks (of 128) per pipeline stage: 2 for token tiles <= 160 (eight MMAs per full/empty handoff), else 1.
 template <int KS>
 __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ LgGroup grp,
@@ -330,7 +330,7 @@ static int pick_tn(int M, int N, int sms, bool k_even) {
         const long tiles = (long)tiles_m * (N / TILE_N);
         const long waves = (tiles + sms - 1) / sms;
         // narrow tiles run two k blocks per stage (KS = 2): 0.21 us = ~410 cycles per k block at TN = 96
-        const double per_kb = ((tn <= 112 && k_even) ? 370.0 : 500.0) + 0.42 * tn;
+        const double per_kb = ((tn <= 112 && k_even) ? 370.0 : (tn <= 160 && k_even) ? 440.0 : 500.0) + 0.42 * tn;
         const double cost = (double)waves * per_kb;
         if (cost <= best_cost) { best_cost = cost; best = tn; }
     }
@@ -373,7 +373,7 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     // narrow token tiles: two k blocks per stage (the MMAs of a 128 x TN x 32 step have a 31 ns floor for TN <= 112,
     // so four of them do not cover one full/empty handoff; eight do)
     static const int tune_ks = env_ks();
-    const int KS = (tune_ks > 0) ? tune_ks : ((TN <= 112 && (K / TILE_K) % 2 == 0) ? 2 : 1);
+    const int KS = (tune_ks > 0) ? tune_ks : ((TN <= 160 && (K / TILE_K) % 2 == 0) ? 2 : 1);
     const int stage = KS * (int)lg_stage_stride(TN);
     const int sw_bytes = LG_SW * KS * LG_W_BYTES;
     int NS = (LG_STAGE_REGION + LG_SW * LG_W_BYTES - sw_bytes) / stage;
