@@ -4,6 +4,8 @@
 #include <cstring>
 #include <mutex>
 #include <unordered_map>
+#include <algorithm>
+#include <cmath>
 #include <vector>
 #include "kernels.h"
 #include "program.h"
@@ -141,36 +143,62 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     P->n_phases = phase + 1;
     int grid = max_phase_gran < sms ? max_phase_gran : sms;
     if (grid < 16 && sms >= 16) grid = 16;                  // enough CTAs to own one activation row each
-    // Split the grid among the stages of each phase in proportion to their cost (>= 1 CTA each).  Measured per
-    // granule on B200: ~0.65 us fixed (reduction barrier + epilogue) + 0.5 us per 15 KiB chunk of
-    // its K, the chunk part times 1.6 for M > 8 (two token tiles: twice the IMMAs per decoded fragment).
-    auto cost = [&](int s) {
-        const int chunks = (S[s].K / 128 + 14) / 15;
-        return (double)S[s].granules * (0.65 + 0.5 * chunks * (S[s].M > 8 ? 1.6 : 1.0));
+    // Split the grid among the stages of each phase so that the slowest group finishes as early as possible.  Model of a
+    // stage on c CTAs, in SM cycles, from per-CTA clock stamps on B200:
+    //     t(c) = start + ceil(granules / c) * g
+    //     M <= 8:  g = 1076 + 36.2 KB,  start = (M > 1 ? 2580 : 1180) + 56 KB     (KB = K / 128, 1 KiB pieces per granule)
+    //     M > 8 :  g = 2020 + 52.4 KB,  start = 2150 + 85 KB                      (two token tiles; B fragments via smem)
+    // `start` is what precedes the first granule beyond the part common to all groups (the B-fragment load).
+    auto gran_cycles = [&](int s) {
+        const double KB = S[s].K / 128;
+        return S[s].M > 8 ? 2020.0 + 52.4 * KB : 1076.0 + 36.2 * KB;
+    };
+    auto start_cycles = [&](int s) {
+        const double KB = S[s].K / 128;
+        return S[s].M > 8 ? 2150.0 + 85.0 * KB : (S[s].M > 1 ? 2580.0 : 1180.0) + 56.0 * KB;
+    };
+    auto stage_time = [&](int s, int c) {
+        return start_cycles(s) + (double)((S[s].granules + c - 1) / c) * gran_cycles(s);
     };
     for (int s0 = 0; s0 < n_stages;) {
         int s1 = s0 + 1;
         while (s1 < n_stages && S[s1].phase == S[s0].phase) ++s1;
         const int ns = s1 - s0;
         if (ns > grid) return VLA_ERR_SHAPE;                 // more independent stages in one phase than CTAs
-        double total = 0.0;
-        for (int s = s0; s < s1; ++s) total += cost(s);
+        // smallest finish time T for which the groups fit in the grid: candidates are start + r * g of every stage
+        std::vector<double> cand;
+        for (int s = s0; s < s1; ++s)
+            for (int r = 1; r <= S[s].granules; ++r) cand.push_back(start_cycles(s) + r * gran_cycles(s));
+        std::sort(cand.begin(), cand.end());
+        auto need = [&](double T) {                           // CTAs needed to finish every stage by T (or -1)
+            int sum = 0;
+            for (int s = s0; s < s1; ++s) {
+                const int r = (int)std::floor((T - start_cycles(s)) / gran_cycles(s) + 1e-9);
+                if (r < 1) return -1;
+                sum += (S[s].granules + r - 1) / r;
+            }
+            return sum;
+        };
+        size_t lo = 0, hi = cand.size() - 1;                 // cand.back() needs one CTA per stage: always feasible
+        while (lo < hi) {
+            const size_t mid = (lo + hi) / 2;
+            const int n = need(cand[mid]);
+            if (n >= 0 && n <= grid) hi = mid; else lo = mid + 1;
+        }
         int given = 0;
         for (int s = s0; s < s1; ++s) {
-            int c = (int)((double)grid * cost(s) / total);
-            if (c < 1) c = 1;
-            S[s].cta_count = c;
-            given += c;
+            const int r = (int)std::floor((cand[lo] - start_cycles(s)) / gran_cycles(s) + 1e-9);
+            S[s].cta_count = (S[s].granules + r - 1) / r;
+            given += S[s].cta_count;
         }
-        while (given != grid) {                              // hand the remainder to / take the excess from the
-            int best = s0;                                   // stage with the most / least bytes per CTA
-            for (int s = s0; s < s1; ++s) {
-                const double ls = cost(s) / S[s].cta_count;
-                const double lb = cost(best) / S[best].cta_count;
-                if (given < grid ? ls > lb : (S[s].cta_count > 1 && (S[best].cta_count <= 1 || ls < lb))) best = s;
-            }
-            S[best].cta_count += (given < grid) ? 1 : -1;
-            given += (given < grid) ? 1 : -1;
+        while (given < grid) {                               // spare CTAs: to the group that finishes last and can use one
+            int best = -1;
+            for (int s = s0; s < s1; ++s)
+                if (S[s].cta_count < S[s].granules &&
+                    (best < 0 || stage_time(s, S[s].cta_count) > stage_time(best, S[best].cta_count))) best = s;
+            if (best < 0) best = s0;                          // every stage already has one CTA per granule
+            ++S[best].cta_count;
+            ++given;
         }
         int begin = 0;
         for (int s = s0; s < s1; ++s) { S[s].cta_begin = begin; begin += S[s].cta_count; }

@@ -57,8 +57,12 @@ __device__ unsigned long long g_trace[148 * 1024];
 __device__ __forceinline__ void trace(int cta, int& n, int tid) {
     if (tid == 0 && n < 1024) {
         unsigned long long t;
+#ifdef VLA_PROG_TRACE_CLOCK
+        t = (unsigned long long)clock64();               // SM cycles: cheap, per-CTA differences only
+#else
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        g_trace[cta * 1024 + n++] = t;
+#endif
+        g_trace[blockIdx.x * 1024 + n++] = t;
     }
 }
 #define QTRACE(k) do { if (threadIdx.x == 0 && g_trace[blockIdx.x * 1024 + 900 + (k)] == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_trace[blockIdx.x * 1024 + 900 + (k)] = t_; } } while (0)
@@ -334,7 +338,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
         }
 
 #ifdef VLA_PROG_TRACE
-        if (tid == 0 && tr_n < 1024) g_trace[cta * 1024 + tr_n++] = (unsigned long long)twait;   // cycles, not a stamp
+        if (tid == 0 && tr_n < 1024) g_trace[blockIdx.x * 1024 + tr_n++] = (unsigned long long)twait;   // cycles, not a stamp
 #endif
         TRACE();
 #pragma unroll
@@ -422,6 +426,9 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
     // Programmatic dependent launch: everything above (barrier init, the static descriptor tables) may overlap the
     // tail of the previous kernel on this stream; counters, activations, weights-in-flight and outputs come after.
     pdl_wait();
+    // Trigger the next launch NOW: its CTAs take this SM as soon as this CTA exits and run their own prologue (up to their
+    // griddepcontrol.wait, which still waits for this whole grid and its memory) under the tail of this grid.
+    pdl_launch_dependents();
     const DevStage* stages = reinterpret_cast<const DevStage*>(desc);
     const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
 
@@ -472,7 +479,6 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
             TRACE();
         }
     }
-    pdl_launch_dependents();
     // the last CTA to finish re-zeroes the counters, so the next launch of the same program needs no memset
     if (tid == 0) {
         const unsigned prev = atomicAdd(P.done, 1u);
