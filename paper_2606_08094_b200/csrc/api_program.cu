@@ -146,12 +146,12 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     // Split the grid among the stages of each phase so that the slowest group finishes as early as possible.  Model of a
     // stage on c CTAs, in SM cycles, from per-CTA clock stamps on B200:
     //     t(c) = start + ceil(granules / c) * g
-    //     M <= 8:  g = 1076 + 36.2 KB,  start = (M > 1 ? 2580 : 1180) + 56 KB     (KB = K / 128, 1 KiB pieces per granule)
-    //     M > 8 :  g = 2020 + 52.4 KB,  start = 2150 + 85 KB                      (two token tiles; B fragments via smem)
+    //     M <= 8:  g =  954 + 38.8 KB,  start = (M > 1 ? 2580 : 1180) + 56 KB     (KB = K / 128, 1 KiB pieces per granule)
+    //     M > 8 :  g = 1212 + 54.4 KB,  start = 2150 + 85 KB                      (two token tiles; B fragments via smem)
     // `start` is what precedes the first granule beyond the part common to all groups (the B-fragment load).
     auto gran_cycles = [&](int s) {
         const double KB = S[s].K / 128;
-        return S[s].M > 8 ? 2020.0 + 52.4 * KB : 1076.0 + 36.2 * KB;
+        return S[s].M > 8 ? 1212.0 + 54.4 * KB : 954.0 + 38.8 * KB;
     };
     auto start_cycles = [&](int s) {
         const double KB = S[s].K / 128;

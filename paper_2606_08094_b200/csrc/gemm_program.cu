@@ -6,12 +6,12 @@
 //
 // Grid: one CTA per SM, 16 warps.
 //   warp 15 (producer)   streams this CTA's share of the packed weights of EVERY stage, in program order, through
-//                        a 6 x 30 KiB shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
+//                        a 6 x 30 KiB (M <= 16 variant: 4 x 30 KiB) shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
 //                        activations, so HBM stays busy across stage boundaries and grid barriers.
 //   warps 0-14 (consumers) per stage: hold the int8 activations as mma.m16n8k32 B fragments IN REGISTERS (warp w
 //                        owns the 64-wide k blocks kq = w mod 15), read packed words from the ring, decode them
 //                        in registers (2 ALU ops per 4 weights, common.cuh) into A fragments, accumulate int32,
-//                        reduce the 15 partial sums per output through shared memory, and run the dequant
+//                        add the 15 partial sums per output into one shared-memory tile (red.shared.add), and run the dequant
 //                        epilogue  y = (float)acc * (alpha_m * beta).
 // Work unit: a GRANULE = 32 output channels x all of K of one linear (K/128 contiguous 1 KiB pieces of the packed
 // layout).  The stages of one PHASE are independent, so they run CONCURRENTLY on disjoint CTA groups sized by their
@@ -41,11 +41,13 @@ constexpr int PG_BPW = 4;                         // 512-byte blocks per warp pe
 constexpr int PG_CHUNK_PIECES = PG_W * PG_BPW / 2;   // 30 pieces of 1 KiB = 60 blocks of 32 ch x 64 k: four per warp
 constexpr int PG_SLOT_BYTES = PG_CHUNK_PIECES * 1024;
 constexpr int PG_XHI_BYTES = 65536;              // M <= 16 variant: B fragments of tokens 8-15 (8 * K bytes, K <= 8192)
-__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 6 : 3; }
+__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 6 : 4; }
 constexpr int PG_DESC_BYTES = 15360;             // stage + linear descriptors cached in shared memory
 constexpr int PG_NBMAX = 9;                      // k blocks per warp per granule: ceil(128 / 15)  ->  K <= 8192
 constexpr int PG_NCHUNK = 3;                     // chunks of 60 blocks that cover 128 blocks
-constexpr int PG_RED_INTS = PG_W * 16 * 33;      // 7920 ints = 31 680 B
+constexpr int PG_RED_STRIDE = 36;                // ints per token row: fragment lane (g,t) -> bank 8t + g, conflict-free
+constexpr int PG_RED_BUF_INTS = 16 * PG_RED_STRIDE;   // one [16 tokens][32 channels] int32 accumulation tile
+constexpr int PG_RED_INTS = 2 * PG_RED_BUF_INTS; // two tiles (granule parity): 4608 B
 __host__ __device__ constexpr int pg_smem(int maxmt) {
     return pg_nslot(maxmt) * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + (maxmt == 1 ? 0 : PG_XHI_BYTES) +
            2 * pg_nslot(maxmt) * 8 + 64 + 16 + 64 + 128;
@@ -97,6 +99,9 @@ __device__ __forceinline__ int lds32(uint32_t addr) {
 }
 __device__ __forceinline__ void sts32(uint32_t addr, int v) {
     asm volatile("st.shared.s32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_shared_add(uint32_t addr, int v) {
+    asm volatile("red.shared.add.s32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
 }
 
 // publish: every store this CTA made before the preceding consumer_bar() becomes visible before the count does
@@ -226,6 +231,9 @@ __device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)
     const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int K = st.K, nblk = K / BLK_K;
     const int8_t* xq = reinterpret_cast<const int8_t*>(st.xq);
+    // all loads first, then the shared-memory stores: sts128 is a compiler barrier, and a load issued after it would
+    // wait for the previous one (measured: 9 serial L2 round trips = 3.7 us at M = 16)
+    uint4 hi[MAXMT == 1 ? 1 : PG_NBMAX];
 #pragma unroll
     for (int i = 0; i < PG_NBMAX; ++i)
 #pragma unroll
@@ -235,8 +243,15 @@ __device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)
                                 ? __ldcg(reinterpret_cast<const uint4*>(xq + (size_t)tok * K + kq * BLK_K + t * 16))
                                 : make_uint4(0, 0, 0, 0);
             if (mt == 0) xv[i] = v;
-            else if (kq < nblk) sts128(xhi + (uint32_t)(kq * 32 + lane) * 16u, v);
+            else hi[i] = v;
         }
+    if (MAXMT == 2) {
+#pragma unroll
+        for (int i = 0; i < PG_NBMAX; ++i) {
+            const int kq = i * PG_W + w;
+            if (kq < nblk) sts128(xhi + (uint32_t)(kq * 32 + lane) * 16u, hi[MAXMT == 1 ? 0 : i]);
+        }
+    }
 }
 
 // cta / G: rank and size of the stage's CTA group
@@ -345,18 +360,19 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
         for (int c = 0; c < 2; ++c)
 #pragma unroll
             for (int i = 0; i < 4; ++i) acc[c][0][i] += acc2[c][i];
-        // 15 per-warp partial sums -> shared memory -> one thread per output
-        // explicit shared-space accesses (a generic int* would compile to 64-bit generic LD/ST)
-        const uint32_t rb = smem_u32(red) + ((MT == 1) ? (uint32_t)(gcount & 1) * (PG_W * 8 * 33 * 4) : 0u);
+        // The 15 per-warp partial sums of an output are added into one int32 tile in shared memory (red.shared.add:
+        // integer addition is exact in any order), two tiles by granule parity: the epilogue of granule g reads and
+        // re-zeroes tile g & 1 while the faster warps already add granule g+1 into the other one.
+        const uint32_t rb = smem_u32(red) + (uint32_t)(gcount & 1) * (PG_RED_BUF_INTS * 4);
 #pragma unroll
         for (int c = 0; c < 2; ++c)
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) {
-                const uint32_t row0 = rb + (uint32_t)((w * MTOK + mt * 8 + 2 * t) * 33 + 16 * c + g) * 4u;
-                sts32(row0, acc[c][mt][0]);
-                sts32(row0 + 33 * 4, acc[c][mt][1]);
-                sts32(row0 + 8 * 4, acc[c][mt][2]);
-                sts32(row0 + (33 + 8) * 4, acc[c][mt][3]);
+                const uint32_t row0 = rb + (uint32_t)((mt * 8 + 2 * t) * PG_RED_STRIDE + 16 * c + g) * 4u;
+                red_shared_add(row0, acc[c][mt][0]);
+                red_shared_add(row0 + PG_RED_STRIDE * 4, acc[c][mt][1]);
+                red_shared_add(row0 + 8 * 4, acc[c][mt][2]);
+                red_shared_add(row0 + (PG_RED_STRIDE + 8) * 4, acc[c][mt][3]);
             }
         consumer_bar();
         TRACE();
@@ -365,9 +381,9 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
             const bool act = rep == 0 ? eactive : eactive2;
             const int tok = rep == 0 ? etok : 15;
             if (act) {
-                int sum = 0;
-#pragma unroll
-                for (int ww = 0; ww < PG_W; ++ww) sum += lds32(rb + (uint32_t)((ww * MTOK + tok) * 33 + ech) * 4u);
+                const uint32_t cell = rb + (uint32_t)(tok * PG_RED_STRIDE + ech) * 4u;
+                const int sum = lds32(cell);
+                sts32(cell, 0);                               // the tile is all zero again for granule g+2
                 const int a = sum >> 6;                       // the decode's factor 64 leaves exactly
                 const size_t o = (size_t)tok * L.N + (size_t)n32 * BLK_N + ech;
                 if (L.dtype == 2) {
@@ -379,7 +395,6 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
                 }
             }
         }
-        if (MT == 2) consumer_bar();                          // single reduction buffer: wait for the readers
         TRACE();
         ++gcount;
     }
@@ -413,6 +428,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         mbar_init(bar_go, 1);
         fence_barrier_init();
     }
+    for (int i = tid; i < PG_RED_INTS; i += PG_THREADS) red[i] = 0;      // accumulation tiles start at zero
     // descriptor tables -> shared memory (they are read on every granule by producer and consumers)
     const int stage_words = P.n_stages * (int)(sizeof(DevStage) / 8), lin_words = P.n_lin * (int)(sizeof(DevLin) / 8);
     {
