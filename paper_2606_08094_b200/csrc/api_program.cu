@@ -145,41 +145,51 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     if (grid < 16 && sms >= 16) grid = 16;                  // enough CTAs to own one activation row each
     // Split the grid among the stages of each phase so that the slowest group finishes as early as possible.  Model of a
     // stage on c CTAs, in SM cycles, from per-CTA clock stamps on B200:
-    //     t(c) = start + ceil(granules / c) * g
-    //     M <= 8:  g =  954 + 38.8 KB,  start = (M > 1 ? 2580 : 1180) + 56 KB     (KB = K / 128, 1 KiB pieces per granule)
-    //     M > 8 :  g = 1212 + 54.4 KB,  start = 2150 + 85 KB                      (two token tiles; B fragments via smem)
-    // `start` is what precedes the first granule beyond the part common to all groups (the B-fragment load).
-    auto gran_cycles = [&](int s) {
-        const double KB = S[s].K / 128;
-        return S[s].M > 8 ? 1212.0 + 54.4 * KB : 954.0 + 38.8 * KB;
-    };
+    //     t(c) = start + ceil(granules / c) * g                                   (KB = K / 128, 1 KiB pieces per granule)
+    //     15-way k split:  M <= 8:  g =  954 + 38.8 KB        M > 8:  g = 1212 + 54.4 KB
+    //     team mode     :  M <= 8:  g =  400 + 45 KB          M > 8:  g =  700 + 75 KB      (prog_team_mode(), program.h)
+    //     start = (M > 8 ? 2150 + 85 KB : (M > 1 ? 2580 : 1180) + 56 KB): the B-fragment load before the first granule
     auto start_cycles = [&](int s) {
         const double KB = S[s].K / 128;
         return S[s].M > 8 ? 2150.0 + 85.0 * KB : (S[s].M > 1 ? 2580.0 : 1180.0) + 56.0 * KB;
     };
     auto stage_time = [&](int s, int c) {
-        return start_cycles(s) + (double)((S[s].granules + c - 1) / c) * gran_cycles(s);
+        const double KB = S[s].K / 128;
+        const bool team = vla::prog_team_mode(S[s].K, S[s].granules, c);
+        const double g = team ? (S[s].M > 8 ? 700.0 + 75.0 * KB : 400.0 + 45.0 * KB)
+                              : (S[s].M > 8 ? 1212.0 + 54.4 * KB : 954.0 + 38.8 * KB);
+        return start_cycles(s) + (double)((S[s].granules + c - 1) / c) * g;
     };
     for (int s0 = 0; s0 < n_stages;) {
         int s1 = s0 + 1;
         while (s1 < n_stages && S[s1].phase == S[s0].phase) ++s1;
         const int ns = s1 - s0;
         if (ns > grid) return VLA_ERR_SHAPE;                 // more independent stages in one phase than CTAs
-        // smallest finish time T for which the groups fit in the grid: candidates are start + r * g of every stage
+        // smallest finish time T for which the groups fit in the grid; candidates: t(c) of every stage and group size
         std::vector<double> cand;
         for (int s = s0; s < s1; ++s)
-            for (int r = 1; r <= S[s].granules; ++r) cand.push_back(start_cycles(s) + r * gran_cycles(s));
+            for (int c = 1; c <= grid && c <= S[s].granules; ++c) cand.push_back(stage_time(s, c));
         std::sort(cand.begin(), cand.end());
-        auto need = [&](double T) {                           // CTAs needed to finish every stage by T (or -1)
+        auto fewest = [&](int s, double T) {                  // smallest group that finishes stage s by T (or -1);
+            const int cmax = S[s].granules < grid ? S[s].granules : grid;      // t(c) is not monotone at the team threshold
+            for (int c = 1; c <= cmax; ++c)
+                if (stage_time(s, c) <= T + 1e-9) return c;
+            return -1;
+        };
+        auto need = [&](double T) {
             int sum = 0;
             for (int s = s0; s < s1; ++s) {
-                const int r = (int)std::floor((T - start_cycles(s)) / gran_cycles(s) + 1e-9);
-                if (r < 1) return -1;
-                sum += (S[s].granules + r - 1) / r;
+                const int c = fewest(s, T);
+                if (c < 0) return -1;
+                sum += c;
             }
             return sum;
         };
-        size_t lo = 0, hi = cand.size() - 1;                 // cand.back() needs one CTA per stage: always feasible
+        size_t lo = 0, hi = cand.size() - 1;
+        {                                                     // feasibility is monotone in T; the largest candidate may still
+            const int n = need(cand[hi]);                     // need more than `grid` CTAs only if ns > grid (excluded above)
+            if (n < 0 || n > grid) lo = hi;
+        }
         while (lo < hi) {
             const size_t mid = (lo + hi) / 2;
             const int n = need(cand[mid]);
@@ -187,16 +197,26 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
         }
         int given = 0;
         for (int s = s0; s < s1; ++s) {
-            const int r = (int)std::floor((cand[lo] - start_cycles(s)) / gran_cycles(s) + 1e-9);
-            S[s].cta_count = (S[s].granules + r - 1) / r;
-            given += S[s].cta_count;
+            int c = fewest(s, cand[lo]);
+            if (c < 1) c = 1;
+            S[s].cta_count = c;
+            given += c;
         }
-        while (given < grid) {                               // spare CTAs: to the group that finishes last and can use one
+        while (given > grid) {                               // (only if the model was infeasible) shrink the largest group
+            int big = s0;
+            for (int s = s0; s < s1; ++s) if (S[s].cta_count > S[big].cta_count) big = s;
+            --S[big].cta_count;
+            --given;
+        }
+        while (given < grid) {                               // spare CTAs: to the group that finishes last, if one more helps
             int best = -1;
             for (int s = s0; s < s1; ++s)
-                if (S[s].cta_count < S[s].granules &&
+                if (S[s].cta_count < S[s].granules && stage_time(s, S[s].cta_count + 1) <= stage_time(s, S[s].cta_count) &&
                     (best < 0 || stage_time(s, S[s].cta_count) > stage_time(best, S[best].cta_count))) best = s;
-            if (best < 0) best = s0;                          // every stage already has one CTA per granule
+            if (best < 0) {                                   // nobody gains: park the spare CTAs on the largest group
+                best = s0;
+                for (int s = s0; s < s1; ++s) if (S[s].granules > S[best].granules) best = s;
+            }
             ++S[best].cta_count;
             ++given;
         }

@@ -47,10 +47,21 @@ constexpr int PG_NBMAX = 9;                      // k blocks per warp per granul
 constexpr int PG_NCHUNK = 3;                     // chunks of 60 blocks that cover 128 blocks
 constexpr int PG_RED_STRIDE = 36;                // ints per token row: fragment lane (g,t) -> bank 8t + g, conflict-free
 constexpr int PG_RED_BUF_INTS = 16 * PG_RED_STRIDE;   // one [16 tokens][32 channels] int32 accumulation tile
-constexpr int PG_RED_INTS = 2 * PG_RED_BUF_INTS; // two tiles (granule parity): 4608 B
+constexpr int PG_TEAMS = 3, PG_TW = 5;           // team mode (K <= 2880): three teams of five warps, one granule each
+constexpr int PG_TEAM_NBLK = PG_NBMAX * PG_TW;   // 45 k blocks: a team warp still holds its B fragments in 9 x uint4
+static_assert(PG_TEAM_NBLK == 45 && PG_TEAMS == 3, "prog_team_mode() in program.h assumes 45 k blocks and 3 teams");
+constexpr int PG_RED_INTS = 2 * PG_TEAMS * PG_RED_BUF_INTS;   // two tiles (granule parity) per team: 13 824 B
+// Per-CTA digest of the stage table, built in the prologue (before griddepcontrol.wait): one word per stage, so that the
+// scans "which rows do I quantise in this phase" and "which stages is my group in" cost one shared-memory load per stage
+// instead of ~250 cycles of dependent descriptor loads (12 independent stages: 2 x 1.5 us at the head of every launch).
+constexpr int PG_INFO_WORDS = 288;               // >= PG_DESC_BYTES / sizeof(DevStage)
+constexpr uint32_t INFO_RANK = 0xFFFFu;          // rank in the stage's CTA group + 1 (0: not a member)
+constexpr uint32_t INFO_PHASE_START = 1u << 16;  // first stage of its phase
+constexpr uint32_t INFO_PUBLISH = 1u << 17;      // DevStage.flags bit 1
+constexpr uint32_t INFO_OWNS_ROW = 1u << 18;     // grid-wide row ownership and this CTA owns a row of the stage
 __host__ __device__ constexpr int pg_smem(int maxmt) {
     return pg_nslot(maxmt) * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + (maxmt == 1 ? 0 : PG_XHI_BYTES) +
-           2 * pg_nslot(maxmt) * 8 + 64 + 16 + 64 + 128;
+           2 * pg_nslot(maxmt) * 8 + 64 + 16 + 64 + PG_INFO_WORDS * 4 + 128;
 }
 
 #ifdef VLA_PROG_TRACE
@@ -70,7 +81,15 @@ __device__ __forceinline__ void trace(int cta, int& n, int tid) {
 #define QTRACE(k) do { if (threadIdx.x == 0 && g_trace[blockIdx.x * 1024 + 900 + (k)] == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_trace[blockIdx.x * 1024 + 900 + (k)] = t_; } } while (0)
 #define TRACE() trace(cta, tr_n, tid)
 #define TRARG , tr_n
+// launch-to-launch view: stamp k (0 entry, 1 after griddepcontrol.wait, 2 first MMA may start, 3 end) of the last 16
+// launches of every CTA; the launch ordinal rides in the header's magic field (debug build only)
+__device__ unsigned long long g_pdl[148 * 16 * 8];
+__device__ unsigned g_ord;
+#define PDLT(k) do { if (threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_pdl[(blockIdx.x * 16 + (P.magic & 15)) * 8 + (k)] = t_; } } while (0)
+#define QT(k) do { if (threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_pdl[(blockIdx.x * 16 + (g_ord & 15)) * 8 + (k)] = t_; } } while (0)
 #else
+#define PDLT(k) do { } while (0)
+#define QT(k) do { } while (0)
 #define TRACE()
 #define QTRACE(k) do { } while (0)
 #define TRARG
@@ -119,16 +138,16 @@ __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uin
 
 // ---------------------------------------------------------------- producer warp
 template <int NSLOT>
-__device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, int cta,
+__device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, const uint32_t* s_info, int cta,
                                          int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty, uint32_t bar_go) {
     // The first chunk goes out at once; the rest of the ring is filled only after this CTA's consumers have seen
     // their first quantised activations: otherwise 148 rings (26 MB) are requested in the first microsecond and the
     // few KB of activation rows the quant owners need queue behind them (measured: 2.5-10 us before the first MMA).
     uint32_t slot = 0, round = 0, issued = 0;
     for (int s = 0; s < P.n_stages; ++s) {
+        const int rank = (int)(s_info[s] & INFO_RANK) - 1;
+        if (rank < 0) continue;                              // another group's stage
         const DevStage& st = stages[s];
-        const int rank = cta - st.cta_begin;
-        if (rank < 0 || rank >= st.cta_count) continue;      // another group's stage
         const int KB = st.K / TILE_K;                       // 1 KiB pieces per granule
         for (int gi = rank; gi < st.granules; gi += st.cta_count) {
             int l = st.lin_begin;
@@ -159,6 +178,7 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     const uint4* xr = st.x + (size_t)r * nvec;
     const uint4 z = make_uint4(0, 0, 0, 0);
     QTRACE(0);
+    QT(4);
     const uint4 v0 = (tid < nvec) ? __ldcg(xr + tid) : z;
     const uint4 v1 = (tid + PG_CONSUMERS < nvec) ? __ldcg(xr + tid + PG_CONSUMERS) : z;
     const uint4 v2 = (tid + 2 * PG_CONSUMERS < nvec) ? __ldcg(xr + tid + 2 * PG_CONSUMERS) : z;
@@ -169,6 +189,7 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     QTRACE(1);
     consumer_bar();
     QTRACE(2);
+    QT(5);
     m = s_max[0];
 #pragma unroll
     for (int i = 1; i < PG_W; ++i) m = fmaxf(m, s_max[i]);
@@ -181,17 +202,19 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     QTRACE(3);
     consumer_bar();                                          // s_max may be reused; stores precede thread 0's fence
     QTRACE(4);
+    QT(6);
 }
 
 // Row r of stage s is quantised by CTA (row_begin_s + r) mod gridDim.x (row_begin_s is stored reduced mod gridDim.x) -- any CTA, not only the stage's group, so that
 // the rows of all stages of a phase are spread over the whole grid (a 2-CTA group would otherwise quantise 8 rows
 // one after the other).  Called by every CTA at the start of a phase, for all stages [s0, s1) of the phase.
 // own_stage = true: only stage s0, and only if its rows stay inside its group (flag bit 2).
-__device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStage* stages, int s0, int cta, int G, int tid,
-                                                 float* s_max, bool own_stage) {
+__device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStage* stages, const uint32_t* s_info, int s0,
+                                                 int cta, int G, int tid, float* s_max, bool own_stage) {
     const int phase = stages[s0].phase;
     bool waited = false;
-    for (int s = s0; s < (own_stage ? s0 + 1 : P.n_stages) && stages[s].phase == phase; ++s) {
+    for (int s = s0; s < (own_stage ? s0 + 1 : P.n_stages) && (s == s0 || !(s_info[s] & INFO_PHASE_START)); ++s) {
+        if (!own_stage && !(s_info[s] & INFO_OWNS_ROW)) continue;        // nothing of this stage is mine (one load)
         const DevStage& st = stages[s];
         int r, step;
         if (st.flags & 4) {                                   // rows stay inside the stage's own CTA group
@@ -215,6 +238,7 @@ __device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStag
             quant_row(st, r, tid, s_max);
         }
         if (done_rows != 0 && tid == 0) red_release_gpu(P.b2 + s, done_rows);    // one release per stage
+        if (done_rows != 0) QT(7);
     }
 }
 
@@ -226,9 +250,9 @@ __device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStag
 __device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
     asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-template <int MAXMT>
+template <int MAXMT, int W>
 __device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)[PG_NBMAX], uint32_t xhi) {
-    const int w = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int w = (tid >> 5) % W, lane = tid & 31, g = lane >> 2, t = lane & 3;   // W = 5: the warp's index in its team
     const int K = st.K, nblk = K / BLK_K;
     const int8_t* xq = reinterpret_cast<const int8_t*>(st.xq);
     // all loads first, then the shared-memory stores: sts128 is a compiler barrier, and a load issued after it would
@@ -238,7 +262,7 @@ __device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)
     for (int i = 0; i < PG_NBMAX; ++i)
 #pragma unroll
         for (int mt = 0; mt < MAXMT; ++mt) {
-            const int kq = i * PG_W + w, tok = mt * 8 + g;
+            const int kq = i * W + w, tok = mt * 8 + g;
             const uint4 v = (kq < nblk && tok < st.M)
                                 ? __ldcg(reinterpret_cast<const uint4*>(xq + (size_t)tok * K + kq * BLK_K + t * 16))
                                 : make_uint4(0, 0, 0, 0);
@@ -248,7 +272,7 @@ __device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)
     if (MAXMT == 2) {
 #pragma unroll
         for (int i = 0; i < PG_NBMAX; ++i) {
-            const int kq = i * PG_W + w;
+            const int kq = i * W + w;
             if (kq < nblk) sts128(xhi + (uint32_t)(kq * 32 + lane) * 16u, hi[MAXMT == 1 ? 0 : i]);
         }
     }
@@ -400,6 +424,126 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
     }
 }
 
+// ---------------------------------------------------------------- team mode (K <= 2880, >= 2 granules per CTA)
+// The 15 consumer warps work as THREE independent teams of five: team q takes the CTA's granules n = q, q+3, ... of the
+// stage (ring chunk n: with K <= 3840 a chunk is exactly one granule, so the producer is unchanged), its warp j owns the
+// k blocks kq = j (mod 5).  Against the 15-way split a warp runs 8 blocks instead of 3 per mbarrier wait / reduction /
+// barrier / epilogue, and the three teams are in different phases of their granules instead of in lockstep (chunk
+// arrival -> decode burst -> barrier), which is what bounded the 15-way loop.
+__device__ __forceinline__ void team_bar(int team) {
+    asm volatile("bar.sync %0, %1;" :: "r"(2 + team), "n"(PG_TW * 32) : "memory");
+}
+template <int MT, int NSLOT>
+__device__ __forceinline__ void stage_gemm_teams(const DevLin* lins, const DevStage& st, int rank, int G, int tid, uint32_t ring,
+                                                 int* red, const float* s_beta, const float* s_alpha, uint32_t bar_full,
+                                                 uint32_t bar_empty, uint4 (&xv)[PG_NBMAX], uint32_t xhi, uint32_t& slot,
+                                                 uint32_t& phase, uint32_t& gcount) {
+    const int w = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0), lane = tid & 31, g = lane >> 2, t = lane & 3;
+    const int team = w / PG_TW, j = w - team * PG_TW, ttid = tid - team * (PG_TW * 32);
+    const int nblk = st.K / BLK_K, nout = st.M * 32;
+    const int ng = rank < st.granules ? (st.granules - rank + G - 1) / G : 0;      // this CTA's granules (= ring chunks)
+    const uint32_t tiles = smem_u32(red) + (uint32_t)team * (2 * PG_RED_BUF_INTS * 4);
+    uint32_t tpar = 0;
+    for (int n = team; n < ng; n += PG_TEAMS) {
+        const int gi = rank + n * G;
+        int l = st.lin_begin;
+        for (int q = 1; q < st.n_lin; ++q)
+            if (gi >= lins[st.lin_begin + q].gran_begin) l = st.lin_begin + q;
+        const DevLin& L = lins[l];
+        const int n32 = gi - L.gran_begin;
+        const float beta = s_beta[l - st.lin_begin];
+        uint32_t sl = slot + (uint32_t)n;                     // ring position of chunk n of this stage
+        const uint32_t wraps = sl / NSLOT;
+        sl -= wraps * NSLOT;
+        const uint32_t ph = phase ^ (wraps & 1u);
+
+        int acc[2][MT][4], acc2[2][4];
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) acc[c][mt][i] = 0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc2[c][i] = 0;
+        }
+        mbar_wait(bar_full + 8u * sl, ph);
+        const uint32_t src = ring + sl * PG_SLOT_BYTES + (uint32_t)lane * 16u;   // block kq of the granule at kq * 512
+#pragma unroll
+        for (int i0 = 0; i0 < PG_NBMAX; i0 += 3) {
+            uint4 wv[3];
+#pragma unroll
+            for (int ii = 0; ii < 3; ++ii) {
+                const int kq = (i0 + ii) * PG_TW + j;
+                wv[ii] = (kq < nblk) ? lds128(src + (uint32_t)kq * 512u) : make_uint4(0, 0, 0, 0);
+            }
+            if (i0 + 3 >= PG_NBMAX) {                         // last loads are out: hand the slot back
+                __syncwarp();                                 // (the empty barrier counts 15: three arrivals per team warp)
+                if (lane < PG_TEAMS) mbar_arrive(bar_empty + 8u * sl);
+            }
+#pragma unroll
+            for (int ii = 0; ii < 3; ++ii) {
+                const int i = i0 + ii, kq = i * PG_TW + j;
+                if (kq < nblk) {
+                    const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
+                    uint4 xh = make_uint4(0, 0, 0, 0);
+                    if (MT == 2) xh = lds128(xhi + (uint32_t)(kq * 32 + lane) * 16u);
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];
+                        const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
+                        const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
+                        mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xv[i].x, xv[i].y);
+                        mma_m16n8k32_s8_nv(acc2[c], e0, e1, e2, e3, xv[i].z, xv[i].w);
+                        if (MT == 2) {
+                            mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh.x, xh.y);
+                            mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh.z, xh.w);
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc[c][0][i] += acc2[c][i];
+        const uint32_t rb = tiles + tpar * (PG_RED_BUF_INTS * 4);
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const uint32_t row0 = rb + (uint32_t)((mt * 8 + 2 * t) * PG_RED_STRIDE + 16 * c + g) * 4u;
+                red_shared_add(row0, acc[c][mt][0]);
+                red_shared_add(row0 + PG_RED_STRIDE * 4, acc[c][mt][1]);
+                red_shared_add(row0 + 8 * 4, acc[c][mt][2]);
+                red_shared_add(row0 + (PG_RED_STRIDE + 8) * 4, acc[c][mt][3]);
+            }
+        team_bar(team);
+        for (int idx = ttid; idx < nout; idx += PG_TW * 32) {  // one output per thread and pass: token idx / 32, channel idx % 32
+            const int tok = idx >> 5, ech = idx & 31;
+            const uint32_t cell = rb + (uint32_t)(tok * PG_RED_STRIDE + ech) * 4u;
+            const int sum = lds32(cell);
+            sts32(cell, 0);
+            const int a = sum >> 6;
+            const size_t o = (size_t)tok * L.N + (size_t)n32 * BLK_N + ech;
+            if (L.dtype == 2) {
+                reinterpret_cast<int*>(L.out)[o] = a;
+            } else {
+                const float y = dequant(a, __fmul_rn(s_alpha[tok], beta));
+                if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
+                else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
+            }
+        }
+        tpar ^= 1u;
+    }
+    uint32_t sl = slot + (uint32_t)ng;                        // every warp: the ring position after this stage's chunks
+    const uint32_t wraps = sl / NSLOT;
+    slot = sl - wraps * NSLOT;
+    phase ^= (wraps & 1u);
+    gcount += (uint32_t)ng;
+    consumer_bar();                                           // all three teams are done with s_beta / s_alpha / xhi
+}
+
 // ---------------------------------------------------------------- the kernel
 // MAXMT = 1: every stage has M <= 8 (32 registers of B fragments per thread, no spills);  MAXMT = 2: M <= 16.
 template <int MAXMT>
@@ -418,8 +562,10 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
     const uint32_t bar_go = bar_empty + 8u * NSLOT + 64u;    // after s_max (64 B)
     float* s_beta = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT + 64 + 16);   // 16 floats
     float* s_max = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT);
+    uint32_t* s_info = reinterpret_cast<uint32_t*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT + 64 + 16 + 64);
 
     const int tid = threadIdx.x, cta = blockIdx.x, G = gridDim.x;
+    PDLT(0);
     if (tid == 0) {
         for (int s = 0; s < NSLOT; ++s) {
             mbar_init(bar_full + 8u * s, 1);
@@ -439,9 +585,27 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         for (int i = tid; i < lin_words; i += PG_THREADS) d[stage_words + i] = gl[i];
     }
     __syncthreads();
+    for (int s = tid; s < P.n_stages; s += PG_THREADS) {     // the digest of the stage table for this CTA
+        const DevStage& st = reinterpret_cast<const DevStage*>(desc)[s];
+        const int rank = cta - st.cta_begin;
+        uint32_t info = (rank >= 0 && rank < st.cta_count) ? (uint32_t)(rank + 1) : 0u;
+        if (s == 0 || reinterpret_cast<const DevStage*>(desc)[s - 1].phase != st.phase) info |= INFO_PHASE_START;
+        if (st.flags & 2) info |= INFO_PUBLISH;
+        if (!(st.flags & 4)) {
+            int r = cta - st.row_begin;                       // first row with (row_begin + r) % G == cta
+            if (r < 0) r += G;
+            if (r < st.M) info |= INFO_OWNS_ROW;
+        }
+        s_info[s] = info;
+    }
+    __syncthreads();
     // Programmatic dependent launch: everything above (barrier init, the static descriptor tables) may overlap the
     // tail of the previous kernel on this stream; counters, activations, weights-in-flight and outputs come after.
     pdl_wait();
+    PDLT(1);
+#ifdef VLA_PROG_TRACE
+    if (tid == 0) g_ord = P.magic;
+#endif
     // Trigger the next launch NOW: its CTAs take this SM as soon as this CTA exits and run their own prologue (up to their
     // griddepcontrol.wait, which still waits for this whole grid and its memory) under the tail of this grid.
     pdl_launch_dependents();
@@ -449,7 +613,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
     const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
 
     if (tid >= PG_CONSUMERS) {
-        producer<NSLOT>(P, stages, lins, cta, tid & 31, ring, bar_full, bar_empty, bar_go);
+        producer<NSLOT>(P, stages, lins, s_info, cta, tid & 31, ring, bar_full, bar_empty, bar_go);
         return;
     }
 #ifdef VLA_PROG_TRACE
@@ -459,16 +623,18 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
     uint4 xv[PG_NBMAX];
     bool go_sent = false;
     uint32_t slot = 0, phase = 0, gcount = 0;
-    int cur_phase = -1;
     for (int s = 0; s < P.n_stages; ++s) {
-        const DevStage& st = stages[s];
-        if (st.phase != cur_phase) {                         // a new phase: quantise the rows this CTA owns
-            cur_phase = st.phase;
-            quant_phase_rows(P, stages, s, cta, G, tid, s_max, false);
+        const uint32_t info = s_info[s];
+        if (info & INFO_PHASE_START) {                       // a new phase: quantise the rows this CTA owns
+            TRACE();
+            quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, false);
+            TRACE();
         }
-        const int rank = cta - st.cta_begin, count = st.cta_count;
-        if (rank >= 0 && rank < count) {                     // this CTA belongs to the stage's group
-            if (st.flags & 4) quant_phase_rows(P, stages, s, cta, G, tid, s_max, true);
+        const int rank = (int)(info & INFO_RANK) - 1;
+        if (rank >= 0) {                                     // this CTA belongs to the stage's group
+            const DevStage& st = stages[s];
+            const int count = st.cta_count;
+            if (st.flags & 4) quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, true);
             TRACE();
             if (tid == 0) {
                 spin_until(P.b2 + s, (unsigned)st.M);
@@ -482,19 +648,33 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
             }
             consumer_bar();
             TRACE();
-            load_xv<MAXMT>(st, tid, xv, xhi);
-            if (MAXMT == 1 || st.M <= 8)
-                stage_gemm<1, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
-            else
-                stage_gemm<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
+            PDLT(2);
+            // team mode: the B fragments of a five-way k split still fit in registers and every team gets >= 2 granules
+            const bool teams = prog_team_mode(st.K, st.granules, count);
+            if (teams) {
+                if (tid < st.M) s_max[tid] = __ldcg(st.xs + tid);     // alpha_m for the team epilogues (s_max is free here)
+                load_xv<MAXMT, PG_TW>(st, tid, xv, xhi);
+                consumer_bar();                               // s_max and (M > 8) the shared B fragments are complete
+                if (MAXMT == 1 || st.M <= 8)
+                    stage_gemm_teams<1, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, s_max, bar_full, bar_empty, xv, xhi, slot, phase, gcount);
+                else
+                    stage_gemm_teams<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, s_max, bar_full, bar_empty, xv, xhi, slot, phase, gcount);
+            } else {
+                load_xv<MAXMT, PG_W>(st, tid, xv, xhi);
+                if (MAXMT == 1 || st.M <= 8)
+                    stage_gemm<1, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
+                else
+                    stage_gemm<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
+            }
             TRACE();
         }
-        if (st.flags & 2) {                                  // end of a phase that a later phase reads from
+        if (info & INFO_PUBLISH) {                           // end of a phase that a later phase reads from
             consumer_bar();                                  // every output store of this CTA precedes the release
-            if (tid == 0) red_release_gpu(P.bp + st.phase, 1u);
+            if (tid == 0) red_release_gpu(P.bp + stages[s].phase, 1u);
             TRACE();
         }
     }
+    PDLT(3);
     // the last CTA to finish re-zeroes the counters, so the next launch of the same program needs no memset
     if (tid == 0) {
         const unsigned prev = atomicAdd(P.done, 1u);
@@ -528,13 +708,24 @@ cudaError_t launch_program(const DevProg& prog, int grid, int max_m, cudaStream_
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
+#ifdef VLA_PROG_TRACE
+    static unsigned trace_launch = 0;
+    DevProg h = prog;
+    h.magic = trace_launch++;
+    if (max_m <= 8) return cudaLaunchKernelEx(&cfg, program_kernel<1>, h);
+    return cudaLaunchKernelEx(&cfg, program_kernel<2>, h);
+#else
     if (max_m <= 8) return cudaLaunchKernelEx(&cfg, program_kernel<1>, prog);
     return cudaLaunchKernelEx(&cfg, program_kernel<2>, prog);
+#endif
 }
 
 #ifdef VLA_PROG_TRACE
 extern "C" int vla_debug_read_trace(unsigned long long* host, size_t n) {
     return (int)cudaMemcpyFromSymbol(host, g_trace, n * sizeof(unsigned long long));
+}
+extern "C" int vla_debug_read_pdl(unsigned long long* host, size_t n) {
+    return (int)cudaMemcpyFromSymbol(host, g_pdl, n * sizeof(unsigned long long));
 }
 #endif
 

@@ -49,4 +49,12 @@ struct DevProg {
     const DevLin* lins;
 };
 
+// Team mode of the program kernel (gemm_program.cu): the stage's group runs three 5-warp teams on three granules at
+// once.  Needs K <= 2880 (a five-way k split whose B fragments still fit in 9 x uint4 per thread) and at least two
+// granules per team and CTA.  One definition for the kernel and for the partition model of the program compiler.
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+inline bool prog_team_mode(int K, int granules, int cta_count) { return K / 64 <= 45 && granules >= 6 * cta_count; }
+
 }  // namespace vla
