@@ -140,8 +140,8 @@ __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uin
 template <int NSLOT>
 __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, const uint32_t* s_info, int cta,
                                          int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty, uint32_t bar_go) {
-    // The first chunk goes out at once; the rest of the ring is filled only after this CTA's consumers have seen
-    // their first quantised activations: otherwise 148 rings (26 MB) are requested in the first microsecond and the
+    // The first chunk goes out at once; the rest of the ring is filled only after this CTA has its own activation row in
+    // registers (row owners) or has seen its first quantised activations (the others): otherwise 148 rings (26 MB) are requested in the first microsecond and the
     // few KB of activation rows the quant owners need queue behind them (measured: 2.5-10 us before the first MMA).
     uint32_t slot = 0, round = 0, issued = 0;
     for (int s = 0; s < P.n_stages; ++s) {
@@ -173,7 +173,7 @@ __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stage
 
 // ---------------------------------------------------------------- row-owner activation quant (Eq. 4 lines 1-2)
 // All 512 consumer threads of the owner CTA quantise row r of stage st: one pass, the row lives in registers.
-__device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, float* s_max) {
+__device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, float* s_max, uint32_t bar_go, bool& go_sent) {
     const int nvec = st.K / 8;                               // uint4 of 8 bf16; K <= 8192 -> nvec <= 1024
     const uint4* xr = st.x + (size_t)r * nvec;
     const uint4 z = make_uint4(0, 0, 0, 0);
@@ -188,6 +188,10 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
     if ((tid & 31) == 0) s_max[tid >> 5] = m;
     QTRACE(1);
     consumer_bar();
+    if (!go_sent) {                                          // the row is in registers: the ring may fill now
+        if (tid == 0) mbar_arrive(bar_go);
+        go_sent = true;
+    }
     QTRACE(2);
     QT(5);
     m = s_max[0];
@@ -210,7 +214,7 @@ __device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, fl
 // one after the other).  Called by every CTA at the start of a phase, for all stages [s0, s1) of the phase.
 // own_stage = true: only stage s0, and only if its rows stay inside its group (flag bit 2).
 __device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStage* stages, const uint32_t* s_info, int s0,
-                                                 int cta, int G, int tid, float* s_max, bool own_stage) {
+                                                 int cta, int G, int tid, float* s_max, bool own_stage, uint32_t bar_go, bool& go_sent) {
     const int phase = stages[s0].phase;
     bool waited = false;
     for (int s = s0; s < (own_stage ? s0 + 1 : P.n_stages) && (s == s0 || !(s_info[s] & INFO_PHASE_START)); ++s) {
@@ -235,7 +239,7 @@ __device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStag
                 consumer_bar();
                 waited = true;
             }
-            quant_row(st, r, tid, s_max);
+            quant_row(st, r, tid, s_max, bar_go, go_sent);
         }
         if (done_rows != 0 && tid == 0) red_release_gpu(P.b2 + s, done_rows);    // one release per stage
         if (done_rows != 0) QT(7);
@@ -627,14 +631,14 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         const uint32_t info = s_info[s];
         if (info & INFO_PHASE_START) {                       // a new phase: quantise the rows this CTA owns
             TRACE();
-            quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, false);
+            quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, false, bar_go, go_sent);
             TRACE();
         }
         const int rank = (int)(info & INFO_RANK) - 1;
         if (rank >= 0) {                                     // this CTA belongs to the stage's group
             const DevStage& st = stages[s];
             const int count = st.cta_count;
-            if (st.flags & 4) quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, true);
+            if (st.flags & 4) quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, true, bar_go, go_sent);
             TRACE();
             if (tid == 0) {
                 spin_until(P.b2 + s, (unsigned)st.M);
