@@ -234,7 +234,8 @@ __device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStag
         }
         unsigned done_rows = 0;
         for (; r < st.M; r += step, ++done_rows) {
-            if ((st.flags & 1) && !waited) {                  // x is written by the previous phase
+            if (phase > 0 && !waited) {                       // a phase starts only after every earlier phase has completed
+                                                              // (vla_ternary.h: x of ANY of its stages may be an earlier phase's output)
                 if (tid == 0) spin_until(P.bp + (phase - 1), (unsigned)G);
                 consumer_bar();
                 waited = true;

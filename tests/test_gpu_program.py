@@ -214,6 +214,52 @@ def test_mixed_phases_and_token_counts(vla, oracle):
     assert np.array_equal(ye.cpu().numpy().view(np.uint32), re_["y32"].view(np.uint32))
 
 
+@pytest.mark.parametrize("mset", [(8, 3, 1, 5), (8, 16, 3, 1)])
+def test_team_and_fifteen_way_stages_alternate(vla, oracle, mset):
+    """Three dependent phases of 37 independent stages each, so that every stage's group is ~4 CTAs: phase A
+    (K=256, N=1024: 8 granules per CTA -> the kernel's three-team mode, ring wraps twice), phase B (K=1024, N=128: one
+    granule per CTA -> 15-way k split), phase C (K=128, N=1024: team mode again).  Every CTA therefore switches mode
+    twice with the weight ring running across the switches; mset with a 16 selects the M <= 16 kernel variant
+    (4 ring slots, B fragments of tokens 8-15 in shared memory), without it the M <= 8 variant (6 slots).
+    Every output of every phase is compared with the oracle (bf16 chain, last phase fp32 / bf16 / int32)."""
+    S = 37
+    def lin(N, K, seed):
+        w = synth.ternary_weights(N, K, 0.35, seed)
+        beta = synth.weight_scale(seed + 1)
+        return dict(w=w, beta=beta, packed=vla.pack_weights(dev(w)), beta_d=dev(np.array([beta], np.float32)), N=N, K=K)
+    xs, A, B, C, ya, yb, yc, stages = [], [], [], [], [], [], [], []
+    for i in range(S):
+        M = mset[i % 4]
+        xs.append(synth.activations(M, 256, 100 + i, outlier_frac=0.01))
+        A.append(lin(1024, 256, 1000 + 3 * i)); B.append(lin(128, 1024, 2000 + 3 * i)); C.append(lin(1024, 128, 3000 + 3 * i))
+        ya.append(torch.zeros((M, 1024), dtype=torch.bfloat16, device="cuda"))
+        yb.append(torch.zeros((M, 128), dtype=torch.bfloat16, device="cuda"))
+        yc.append(torch.full((M, 1024), -7, dtype=_TDT[i % 3], device="cuda"))
+    def stage(x, M, L, out, depends, dt):
+        return dict(x=x, M=M, K=L["K"], depends=depends,
+                    linears=[dict(packed=L["packed"], w_scale=L["beta_d"], out=out, N=L["N"], out_dtype=dt)])
+    xin = [dev_bf16(x) for x in xs]
+    for i in range(S): stages.append(stage(xin[i], mset[i % 4], A[i], ya[i], 0, 1))
+    for i in range(S): stages.append(stage(ya[i], mset[i % 4], B[i], yb[i], 1 if i == 0 else 0, 1))
+    for i in range(S): stages.append(stage(yb[i], mset[i % 4], C[i], yc[i], 1 if i == 0 else 0, i % 3))
+    prog = vla.compile_program(stages)
+    for _ in range(3):
+        vla.vla_program_run(prog)
+    torch.cuda.synchronize()
+    for i in range(S):
+        ra = oracle.ternary_linear(xs[i], A[i]["w"], A[i]["beta"])
+        rb = oracle.ternary_linear(ra["ybf16"], B[i]["w"], B[i]["beta"])
+        rc = oracle.ternary_linear(rb["ybf16"], C[i]["w"], C[i]["beta"])
+        assert np.array_equal(bits(ya[i]), ra["ybf16"]), "phase A stage %d" % i
+        assert np.array_equal(bits(yb[i]), rb["ybf16"]), "phase B stage %d" % i
+        if i % 3 == 2:
+            assert np.array_equal(yc[i].cpu().numpy(), rc["acc"]), "phase C stage %d" % i
+        elif i % 3 == 0:
+            assert np.array_equal(yc[i].cpu().numpy().view(np.uint32), rc["y32"].view(np.uint32)), "phase C stage %d" % i
+        else:
+            assert np.array_equal(bits(yc[i]), rc["ybf16"]), "phase C stage %d" % i
+
+
 def _guarded(shape, dtype, fill):
     """tensor view with 4 KiB of sentinel bytes on both sides (a hand-made out-of-bounds-write detector)"""
     n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
