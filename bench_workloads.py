@@ -188,6 +188,40 @@ def run_sweep(args, pk, clock_sampler, int8_probe_tops):
         compare.append(row)
         del ring
         torch.cuda.empty_cache()
+    # Row a6 evidence for 16 < M <= 32: the IMMA kernel and the tcgen05 kernel, forced, on the same fused
+    # vla_ternary_linear call over cold weights; "auto" is what VLA_PATH_AUTO resolves to.
+    crossover = []
+    for si, (K, N) in enumerate(list(synth.SWEEP_SHAPES) + [(2560, 640)]):
+        copies = max(2, -(-2 * l2 // (N * K // 4)))
+        w = synth.ternary_weights(N, K, 0.33, 4950 + si)
+        packed1 = vla.pack_weights(torch.from_numpy(w).to(dev))
+        ring = packed1.unsqueeze(0).repeat(copies, 1).contiguous()
+        del w, packed1
+        beta = torch.tensor([0.05], dtype=torch.float32, device=dev)
+        xb = synth.activations(32, K, 505000 + si)
+        x_all = torch.from_numpy(xb.view(np.int16)).to(dev).view(torch.bfloat16)
+        for M in (17, 24, 32):
+            x = x_all[:M].contiguous()
+            out = torch.empty((M, N), dtype=torch.float32, device=dev)
+            xq = torch.empty((M, K), dtype=torch.int8, device=dev)
+            xs = torch.empty((M,), dtype=torch.float32, device=dev)
+            row = {"M": M, "K": K, "N": N, "auto": int(vla.vla_ternary_auto_path(M, N, K))}
+            for name, path in (("small_tc_us", vla.VLA_PATH_SMALL_TC), ("large_us", vla.VLA_PATH_LARGE)):
+                ncall = min(copies, 32)
+
+                def calls():
+                    for c in range(ncall):
+                        vla.vla_ternary_linear(ring[c], beta, x, M, N, K, out, vla.VLA_F32, path, xq, xs, None, 0)
+                calls()
+                torch.cuda.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    calls()
+                row[name] = _time(torch, g.replay, 10) / ncall * 1e6
+                del g
+            crossover.append(row)
+        del ring, x_all
+        torch.cuda.empty_cache()
     clocks = sampler.stop()
     big = [p for p in pts if p["M"] >= 512]
     small = [p for p in pts if p["M"] <= 16]
@@ -210,6 +244,7 @@ def run_sweep(args, pk, clock_sampler, int8_probe_tops):
             "M<=16 streaming roofline_frac median": float(np.median([p["stream_roofline_frac"] for p in small
                                                                      if "stream_roofline_frac" in p])) if small else None},
         "dp4a_vs_imma_M8": compare,
+        "path_crossover_M17_32": crossover,
         "points": pts,
     }
     print(json.dumps(line))

@@ -53,7 +53,7 @@ typedef enum {
 } vla_dtype;
 
 typedef enum {
-    VLA_PATH_AUTO = 0,      /* library chooses by M (table in DESIGN.md, justified by ncu) */
+    VLA_PATH_AUTO = 0,      /* library chooses by M, and by (N,K) for 16 < M <= 32 (table in DESIGN.md 6d, measured) */
     VLA_PATH_SMALL_ALU = 1, /* in-register decode + dp4a on the integer ALUs; M <= 16 */
     VLA_PATH_SMALL_TC = 2,  /* in-register decode + warp-level int8 MMA; M <= 64 */
     VLA_PATH_LARGE = 3      /* TMA -> decode warps -> tcgen05.mma kind::i8 -> TMEM; any M */

@@ -42,9 +42,17 @@ inline vla_status from_cuda(cudaError_t e) {
 }
 
 // The dispatch table: which kernel family runs a given M.
-vla_path auto_path(int M) {
-    if (M <= 32) return VLA_PATH_SMALL_TC;
-    return VLA_PATH_LARGE;
+// Row a6.  M <= 16 and M > 32 are decided by M alone.  For 16 < M <= 32 both kernels run one token tile and
+// neither is faster everywhere; measured on cold weights (profiles/r01d_path_probe.md): the IMMA kernel costs
+// 7.5 us + 0.208 us per million weights, the tcgen05 kernel 4.1 us + 0.224 us per 128-wide k block per wave of
+// 148 channel tiles.  The faster model wins.
+vla_path auto_path(int M, int N, int K) {
+    if (M <= 16) return VLA_PATH_SMALL_TC;
+    if (M > 32) return VLA_PATH_LARGE;
+    const double small_us = 7.5 + 0.208e-6 * (double)N * (double)K;
+    const int waves = (N / 128 + 147) / 148;
+    const double large_us = 4.1 + 0.224 * (double)(K / 128) * (double)waves;
+    return large_us < small_us ? VLA_PATH_LARGE : VLA_PATH_SMALL_TC;
 }
 
 bool path_supports(vla_path p, int M) {
@@ -88,8 +96,7 @@ size_t vla_ternary_workspace_bytes(int M, int N, int K, vla_path path) {
 }
 
 vla_path vla_ternary_auto_path(int M, int N, int K) {
-    (void)N; (void)K;
-    return auto_path(M);
+    return auto_path(M, N, K);
 }
 
 vla_status vla_ternary_pack(const int8_t* w, int N, int K, void* packed, size_t packed_bytes, void* stream) {
@@ -138,7 +145,7 @@ vla_status vla_ternary_gemm(const void* packed, const float* w_scale, const int8
     if (!packed || !xq || !out) return VLA_ERR_NULL;
     if (out_dtype != VLA_I32 && (!w_scale || !x_scale)) return VLA_ERR_NULL;
     if (M < 1 || !shape_ok(N, K)) return VLA_ERR_SHAPE;
-    if (path == VLA_PATH_AUTO) path = auto_path(M);
+    if (path == VLA_PATH_AUTO) path = auto_path(M, N, K);
     if (!path_supports(path, M)) return VLA_ERR_SHAPE;
     if (!aligned16(packed) || !aligned16(xq) || !aligned16(out) || (x_scale && !aligned16(x_scale)) ||
         (w_scale && (reinterpret_cast<uintptr_t>(w_scale) & 3u)))

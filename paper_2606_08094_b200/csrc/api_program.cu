@@ -295,7 +295,9 @@ vla_status vla_ternary_gemm_grouped(const vla_prog_linear* lins, int n_linears, 
         need_scale = need_scale || l.out_dtype != VLA_I32;
     }
     if (need_scale && !x_scale) return VLA_ERR_NULL;
-    const bool large = (path == VLA_PATH_LARGE) || (path == VLA_PATH_AUTO && vla_ternary_auto_path(M, lins[0].N, K) == VLA_PATH_LARGE);
+    int n_total = 0;                                        // the grouped launch runs the group as one [sum N, K] linear
+    for (int j = 0; j < n_linears; ++j) n_total += lins[j].N;
+    const bool large = (path == VLA_PATH_LARGE) || (path == VLA_PATH_AUTO && vla_ternary_auto_path(M, n_total, K) == VLA_PATH_LARGE);
     if (!large) {                                           // small-M: one launch per linear (or use a program)
         for (int j = 0; j < n_linears; ++j) {
             vla_status st = vla_ternary_gemm(lins[j].packed, lins[j].w_scale, xq, x_scale, M, lins[j].N, K, lins[j].out,

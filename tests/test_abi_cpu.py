@@ -107,6 +107,16 @@ def test_auto_path_table(vla):
     assert vla.vla_ternary_auto_path(1, 2560, 2560) in (vla.VLA_PATH_SMALL_ALU, vla.VLA_PATH_SMALL_TC)
     assert vla.vla_ternary_auto_path(544, 2560, 2560) == vla.VLA_PATH_LARGE
     assert vla.vla_ternary_auto_path(4096, 8192, 8192) == vla.VLA_PATH_LARGE
+    # 16 < M <= 32: by (N,K), from the measured per-path cost model (profiles/r01d_path_probe.md)
+    for M in (17, 24, 32):
+        assert vla.vla_ternary_auto_path(M, 8192, 8192) == vla.VLA_PATH_LARGE
+        assert vla.vla_ternary_auto_path(M, 6912, 2560) == vla.VLA_PATH_LARGE
+        assert vla.vla_ternary_auto_path(M, 2560, 2560) == vla.VLA_PATH_LARGE
+        assert vla.vla_ternary_auto_path(M, 2560, 6912) == vla.VLA_PATH_SMALL_TC
+        assert vla.vla_ternary_auto_path(M, 640, 2560) == vla.VLA_PATH_SMALL_TC
+    for shape in ((2560, 2560), (640, 2560), (6912, 2560), (2560, 6912), (8192, 8192)):
+        assert vla.vla_ternary_auto_path(16, *shape) == vla.VLA_PATH_SMALL_TC
+        assert vla.vla_ternary_auto_path(33, *shape) == vla.VLA_PATH_LARGE
 
 
 def test_product_does_not_import_the_oracle():

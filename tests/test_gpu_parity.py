@@ -354,6 +354,41 @@ def test_full_size_large_m_sampled_channels(vla, oracle, M, K, N):
     assert np.array_equal(xs.cpu().numpy().view(np.uint32), ref["alpha"].view(np.uint32))
 
 
+@pytest.mark.parametrize("M", [17, 32])
+@pytest.mark.parametrize("N,K,want", [(2560, 2560, "large"), (640, 2560, "small_tc"), (2560, 6912, "small_tc")])
+def test_auto_path_between_16_and_32_tokens(vla, oracle, M, N, K, want):
+    """Row a6: for 16 < M <= 32 VLA_PATH_AUTO picks by (N,K); whichever kernel it picks, the call matches
+    the oracle bit for bit."""
+    expect = vla.VLA_PATH_LARGE if want == "large" else vla.VLA_PATH_SMALL_TC
+    assert vla.vla_ternary_auto_path(M, N, K) == expect
+    w = synth.ternary_weights(N, K, 0.35, 77 + N + K)
+    x = synth.activations(M, K, 1700 + M + K, outlier_frac=0.01)
+    packed = vla.pack_weights(dev(w))
+    check_outputs(vla, oracle, packed, w, np.float32(0.021), x, M, N, K, vla.VLA_PATH_AUTO)
+
+
+def test_grouped_auto_at_24_tokens_matches_per_linear_calls(vla, oracle):
+    """q|k|v at M = 24 through VLA_PATH_AUTO: the group's total N decides the kernel; outputs are the oracle's."""
+    M, K = 24, 2560
+    x_bits = synth.activations(M, K, 2424, outlier_frac=0.01)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(x_bits), M, K, xq, xs)
+    lins, keep = [], []
+    for i, (N, beta) in enumerate([(2560, 0.05), (640, 0.013), (640, 0.5)]):
+        w = synth.ternary_weights(N, K, 0.35, 950 + i)
+        packed = vla.pack_weights(dev(w))
+        beta_d = dev(np.array([beta], np.float32))
+        out = vla.empty_out(M, N, vla.VLA_F32)
+        keep.append((w, packed, beta_d, out, np.float32(beta)))
+        lins.append(dict(packed=packed, w_scale=beta_d, out=out, N=N, out_dtype=vla.VLA_F32))
+    vla.vla_ternary_gemm_grouped(lins, xq, xs, M, K, vla.VLA_PATH_AUTO)
+    torch.cuda.synchronize()
+    for (w, packed, beta_d, out, beta) in keep:
+        ref = oracle.ternary_linear(x_bits, w, beta)
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), ref["y32"].view(np.uint32))
+
+
 def test_grouped_large_gemm_per_group_scales(vla, oracle):
     """q|k|v-style group: three linears with their own beta and output type share one quantised activation matrix and
     run as ONE tcgen05 launch (Eq. 4's per-output-group scales); ragged M, every linear vs the oracle."""
