@@ -155,8 +155,8 @@ typedef struct {
 } vla_prog_stage;
 
 /* Eq. 4 for up to 8 linears that share ONE pre-quantised activation matrix (per-output-group scales beta_g(n),
- * q|k|v, gate|up) in as few launches as the path allows: one tcgen05 launch for M > 32, one
- * launch per linear otherwise.  `lins` is a HOST array; its pointers are device pointers (see vla_prog_linear).
+ * q|k|v, gate|up) in as few launches as the path allows: one tcgen05 launch where the path is
+ * VLA_PATH_LARGE (VLA_PATH_AUTO: M > 32, and 16 < M <= 32 by the group's total N and K), one launch per linear otherwise.  `lins` is a HOST array; its pointers are device pointers (see vla_prog_linear).
  * Every linear has the same K.  Asynchronous on `stream`, capturable. */
 vla_status vla_ternary_gemm_grouped(const vla_prog_linear* lins /*host*/, int n_linears, const int8_t* xq,
                                     const float* x_scale, int M, int K, vla_path path, void* stream);
