@@ -1,6 +1,7 @@
 // api_program.cu -- host side of the program API of include/vla_ternary.h: validation, compilation of the
 // descriptor tables into device memory, and the single launch.  Nothing here computes.
 #include "../../include/vla_ternary.h"
+#include <cstdio>
 #include <cstring>
 #include <mutex>
 #include <unordered_map>
@@ -9,6 +10,24 @@
 #include <vector>
 #include "kernels.h"
 #include "program.h"
+
+// partition model constants (SM cycles; see vla_program_build).  Compile-time defaults, overridable for calibration.
+#ifndef VLA_PROG_GATE
+#define VLA_PROG_GATE 0
+#endif
+#ifndef VLA_PG_START0
+#define VLA_PG_START0 3300.0
+#define VLA_PG_START1 2.5
+#define VLA_PG_START_COOP 10000.0
+#define VLA_PG_T1A 400.0
+#define VLA_PG_T1B 45.0
+#define VLA_PG_T2A 700.0
+#define VLA_PG_T2B 75.0
+#define VLA_PG_F1A 954.0
+#define VLA_PG_F1B 50.0
+#define VLA_PG_F2A 1212.0
+#define VLA_PG_F2B 75.0
+#endif
 
 namespace {
 
@@ -44,12 +63,16 @@ vla_status check_stages(const vla_prog_stage* st, int n) {
     }
     size_t n_lin = 0;
     for (int s = 0; s < n; ++s) n_lin += (size_t)st[s].n_linears;
-    if (sizeof(DevStage) * (size_t)n + sizeof(DevLin) * n_lin > vla::program_desc_capacity()) return VLA_ERR_SHAPE;
+    // shared memory of the launch: descriptors + the largest quantised activation matrix + at least two ring slots
+    int need = 0;                                             // worst CTA: its stage's activations + two ring slots
+    for (int s = 0; s < n; ++s)
+        need = std::max(need, ((vla::pg_xq_bytes(st[s].M, st[s].K) + 127) & ~127) + vla::PG_NSLOT_MIN * vla::pg_slot_bytes(st[s].K));
+    if ((size_t)vla::pg_off_xq(n, (int)n_lin) + need > (size_t)vla::PG_SMEM_LIMIT) return VLA_ERR_SHAPE;
     return VLA_OK;
 }
 
 struct Layout {
-    size_t off_stages, off_lins, off_counters, off_act, total;
+    size_t off_stages, off_lins, off_counters, off_stamps, off_act, total;
     int n_lin;
 };
 
@@ -61,8 +84,13 @@ Layout layout_of(const vla_prog_stage* st, int n) {
     L.off_stages = o;   o += round256(sizeof(DevStage) * (size_t)n);
     L.off_lins = o;     o += round256(sizeof(DevLin) * (size_t)L.n_lin);
     L.off_counters = o; o += round256(sizeof(unsigned) * (2 * (size_t)n + 1));
-    L.off_act = o;
-    for (int s = 0; s < n; ++s) o += round256((size_t)st[s].M * st[s].K) + 256;      // int8 [M,K] + alpha [M]
+    L.off_act = o;                                           // cooperative stages: int8 fragments + alpha [16]
+    for (int s = 0; s < n; ++s)
+        if (!vla::pg_local_quant(st[s].M, st[s].K)) o += round256((size_t)vla::pg_xq_bytes(st[s].M, st[s].K)) + 256;
+    L.off_stamps = o;
+#ifdef VLA_PROG_STAMPS
+    o += round256(sizeof(unsigned long long) * 32 * 256);
+#endif
     L.total = o;
     return L;
 }
@@ -100,27 +128,36 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     P->n_stages = n_stages;
     P->n_lin = L.n_lin;
     P->bp = reinterpret_cast<unsigned*>(base + L.off_counters);
-    P->b2 = P->bp + n_stages;
-    P->done = P->b2 + n_stages;
+    P->cnt = P->bp + n_stages;
+    P->done = P->cnt + n_stages;
+#ifdef VLA_PROG_STAMPS
+    P->stamps = reinterpret_cast<unsigned long long*>(base + L.off_stamps);
+#else
+    P->stamps = nullptr;
+#endif
     P->stages = reinterpret_cast<const DevStage*>(base + L.off_stages);
     P->lins = reinterpret_cast<const DevLin*>(base + L.off_lins);
+    int li = 0, max_m = 0, phase = 0, max_phase_gran = 0, phase_gran = 0, max_need = 0, n_coop = 0;
     size_t act = L.off_act;
-    int li = 0, max_m = 0, phase = 0, max_phase_gran = 0, phase_gran = 0, rows = 0;
     for (int s = 0; s < n_stages; ++s) {
         const vla_prog_stage& a = stages[s];
         DevStage& d = S[s];
         d.x = reinterpret_cast<const uint4*>(a.x_bf16);
-        const size_t qbytes = round256((size_t)a.M * a.K);
-        d.xq = reinterpret_cast<uint2*>(a.xq_opt ? (void*)a.xq_opt : (void*)(base + act));
-        d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + act + qbytes);
-        act += qbytes + 256;
+        d.xq_out = a.xq_opt;
+        d.xs_out = a.x_scale_opt;
+        d.coop = nullptr;
+        if (!vla::pg_local_quant(a.M, a.K)) {
+            d.coop = base + act;
+            act += round256((size_t)vla::pg_xq_bytes(a.M, a.K)) + 256;
+            ++n_coop;
+        }
+        max_need = std::max(max_need, ((vla::pg_xq_bytes(a.M, a.K) + 127) & ~127) + vla::PG_NSLOT_MAX * vla::pg_slot_bytes(a.K));
+        d.inv_cpr = (uint32_t)((0x100000000ull + (unsigned)(a.K / 16) - 1u) / (unsigned)(a.K / 16));
         d.M = (int16_t)a.M;
         d.K = (int16_t)a.K;
         d.flags = (int16_t)((s == 0) ? 0 : a.depends);      // nothing precedes the first stage
         if (d.flags & 1) { ++phase; phase_gran = 0; }        // a dependent stage opens a new phase
         d.phase = phase;
-        d.row_begin = rows;
-        rows += a.M;
         if (a.M > max_m) max_m = a.M;
         d.lin_begin = li;
         d.n_lin = (int16_t)a.n_linears;
@@ -142,22 +179,36 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     }
     P->n_phases = phase + 1;
     int grid = max_phase_gran < sms ? max_phase_gran : sms;
-    if (grid < 16 && sms >= 16) grid = 16;                  // enough CTAs to own one activation row each
+    // dynamic shared memory: everything up to the activation region, the largest activation matrix, and as many ring
+    // slots as fit (a CTA whose own stages need less activation room gets more slots)
+    const int fixed = vla::pg_off_xq(n_stages, L.n_lin);
+    int smem = fixed + max_need;
+    if (smem > vla::PG_SMEM_LIMIT) smem = vla::PG_SMEM_LIMIT;
+    P->smem_bytes = smem;
+    P->gate = VLA_PROG_GATE;
+    P->n_coop = n_coop;
+    P->pad = 0;
+    if (P->n_phases > 1 || n_coop > 0) {
+        // CTAs of a multi-phase program wait for each other: all of them must be resident at once
+        int per_sm = 0;
+        if (vla::program_max_ctas_per_sm(max_m, smem, &per_sm) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+        if (per_sm < 1) return VLA_ERR_CUDA;
+        if (grid > per_sm * sms) grid = per_sm * sms;
+    }
     // Split the grid among the stages of each phase so that the slowest group finishes as early as possible.  Model of a
     // stage on c CTAs, in SM cycles, from per-CTA clock stamps on B200:
     //     t(c) = start + ceil(granules / c) * g                                   (KB = K / 128, 1 KiB pieces per granule)
-    //     15-way k split:  M <= 8:  g =  954 + 38.8 KB        M > 8:  g = 1212 + 54.4 KB
-    //     team mode     :  M <= 8:  g =  400 + 45 KB          M > 8:  g =  700 + 75 KB      (prog_team_mode(), program.h)
-    //     start = (M > 8 ? 2150 + 85 KB : (M > 1 ? 2580 : 1180) + 56 KB): the B-fragment load before the first granule
-    auto start_cycles = [&](int s) {
-        const double KB = S[s].K / 128;
-        return S[s].M > 8 ? 2150.0 + 85.0 * KB : (S[s].M > 1 ? 2580.0 : 1180.0) + 56.0 * KB;
+    //     15-way k split:  M <= 8:  g = F1A + F1B KB        M > 8:  g = F2A + F2B KB
+    //     team mode     :  M <= 8:  g = T1A + T1B KB        M > 8:  g = T2A + T2B KB      (prog_team_mode(), program.h)
+    //     start = START0 + START1 * (16-element tasks) for a locally quantised stage, START_COOP for a cooperative one
+    auto start_cycles = [&](int s) {                          // fused quant before the first granule (measured, profiles/r02*)
+        return vla::pg_local_quant(S[s].M, S[s].K) ? VLA_PG_START0 + VLA_PG_START1 * (S[s].M * (S[s].K / 16)) : VLA_PG_START_COOP;
     };
     auto stage_time = [&](int s, int c) {
         const double KB = S[s].K / 128;
-        const bool team = vla::prog_team_mode(S[s].K, S[s].granules, c);
-        const double g = team ? (S[s].M > 8 ? 700.0 + 75.0 * KB : 400.0 + 45.0 * KB)
-                              : (S[s].M > 8 ? 1212.0 + 54.4 * KB : 954.0 + 38.8 * KB);
+        const bool team = vla::prog_team_mode(S[s].granules, c);
+        const double g = team ? (S[s].M > 8 ? VLA_PG_T2A + VLA_PG_T2B * KB : VLA_PG_T1A + VLA_PG_T1B * KB)
+                              : (S[s].M > 8 ? VLA_PG_F2A + VLA_PG_F2B * KB : VLA_PG_F1A + VLA_PG_F1B * KB);
         return start_cycles(s) + (double)((S[s].granules + c - 1) / c) * g;
     };
     for (int s0 = 0; s0 < n_stages;) {
@@ -223,18 +274,18 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
         int begin = 0;
         for (int s = s0; s < s1; ++s) { S[s].cta_begin = begin; begin += S[s].cta_count; }
         if (s1 < n_stages) S[s1 - 1].flags |= 2;             // publish: the next phase opens with a dependent stage
-        // Activation rows: spread over the whole grid (<= 2 rows per CTA) unless the phase has so many rows that
-        // every CTA is busy quantising anyway; then each stage's own group quantises its rows (no cross-group wait).
-        int phase_rows = 0;
-        for (int s = s0; s < s1; ++s) phase_rows += S[s].M;
-        if (phase_rows > 2 * grid)
-            for (int s = s0; s < s1; ++s) S[s].flags |= 4;
-        for (int s = s0; s < s1; ++s) S[s].row_begin %= grid;
         s0 = s1;
     }
 
+#ifdef VLA_PROG_STAMPS
+    for (int s = 0; s < n_stages && s < 16; ++s)
+        fprintf(stderr, "stage %d: M=%d K=%d granules=%d phase=%d ctas [%d,+%d) model %.0f cycles\n", s, S[s].M, S[s].K,
+                S[s].granules, S[s].phase, S[s].cta_begin, S[s].cta_count, stage_time(s, S[s].cta_count));
+#endif
     cudaStream_t cs = (cudaStream_t)stream;
     cudaError_t e = cudaMemcpyAsync(prog_dev, host.data(), host.size(), cudaMemcpyHostToDevice, cs);
+    // the scratch of cooperative stages starts at zero: the fragments of padding rows (M .. 8 or 16) are never written
+    if (e == cudaSuccess && L.total > L.off_act) e = cudaMemsetAsync(base + L.off_act, 0, L.total - L.off_act, cs);
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     std::lock_guard<std::mutex> lk(g_mu);

@@ -6,22 +6,27 @@
 //
 // Grid: one CTA per SM, 16 warps.
 //   warp 15 (producer)   streams this CTA's share of the packed weights of EVERY stage, in program order, through
-//                        a 6 x 30 KiB (M <= 16 variant: 4 x 30 KiB) shared-memory ring with cp.async.bulk (TMA) + mbarriers.  It never waits on
-//                        activations, so HBM stays busy across stage boundaries and grid barriers.
-//   warps 0-14 (consumers) per stage: hold the int8 activations as mma.m16n8k32 B fragments IN REGISTERS (warp w
-//                        owns the 64-wide k blocks kq = w mod 15), read packed words from the ring, decode them
-//                        in registers (2 ALU ops per 4 weights, common.cuh) into A fragments, accumulate int32,
-//                        add the 15 partial sums per output into one shared-memory tile (red.shared.add), and run the dequant
-//                        epilogue  y = (float)acc * (alpha_m * beta).
-// Work unit: a GRANULE = 32 output channels x all of K of one linear (K/128 contiguous 1 KiB pieces of the packed
-// layout).  The stages of one PHASE are independent, so they run CONCURRENTLY on disjoint CTA groups sized by their
-// weight bytes (no serialisation between them, and each activation matrix is read by its own group only instead
-// of by all 148 SMs); granule gi of a stage goes to CTA (gi mod group size) of its group.
-// Activation quant (Eq. 4 lines 1-2): row r of stage s is quantised by ONE owner CTA (absmax over the row, then
-// the true-division quantiser of quant.cuh) into global int8 + alpha; counters in global memory order the phases:
-//   bp[p] = CTAs that finished phase p   (a dependent stage's row owners wait for bp[p-1] == gridDim.x)
-//   b2[s] = rows of stage s quantised    (the stage's group waits for b2[s] == M_s before it loads its B fragments)
-// int32 sums are exact in any order, so the
+//                        a ring of 30 KiB shared-memory slots with cp.async.bulk (TMA) + mbarriers.  It starts before
+//                        griddepcontrol.wait (weights never depend on the previous kernel) and never waits on
+//                        activations, so HBM stays busy across launch, stage and phase boundaries.
+//   warps 0-14 (consumers) per stage:
+//     1. activation quant, Eq. 4 lines 1-2, FUSED INTO THE PROLOGUE: every CTA of the stage's group reads the bf16
+//        rows itself (L2 hits after the first CTA), takes the row absmax, and quantises straight into shared memory
+//        in mma.m16n8k32 B-fragment order.  No CTA ever waits for another CTA's quantised activations: there is no
+//        int8 round trip through global memory and no flag (the caller's optional xq / alpha outputs are written by
+//        the group's first CTA on the side).
+//     2. GEMM: packed words from the ring are decoded in registers (2 ALU ops per 4 weights, common.cuh) into A
+//        fragments, B fragments come from shared memory, int32 accumulation on the warp-level int8 MMA.  Either
+//        three TEAMS of five warps work on three granules at once (each team's warps split the k blocks of its
+//        granule), or -- when the CTA has fewer than three granules of the stage -- all 15 warps split one granule.
+//        Partial sums meet in an int32 tile in shared memory (red.shared.add: exact in any order).
+//     3. dequant epilogue  y = (float)acc * (alpha_m * beta), fp32 / bf16 RNE / raw int32.
+// Work unit: a GRANULE = 32 output channels x all of K of one linear (one contiguous run of 8*K bytes).  The stages
+// of one PHASE are independent, so they run CONCURRENTLY on disjoint CTA groups sized by the program compiler
+// (api_program.cu); granule gi of a stage goes to CTA (gi mod group size) of its group.
+// The only grid-wide synchronisation left is between dependent phases:
+//   bp[p] = CTAs that finished phase p   (a dependent phase's CTAs wait for bp[p-1] == gridDim.x before reading x)
+// Every sum is an exact integer sum and the quantiser reproduces the two true divisions of Eq. 4 bit for bit, so the
 // result is bit-identical to the per-call kernels and to the oracle.
 #include <cuda_bf16.h>
 #include "common.cuh"
@@ -31,86 +36,47 @@
 
 namespace vla {
 
-// 15 consumer warps + 1 producer = 16 warps = 4 per SM sub-partition -> 128 registers per thread.  (A 17th warp puts
-// five warps on one sub-partition and caps every thread at 96 registers: the B fragments then spill, and with 227 KB
-// of shared memory there is no L1 to catch the spills.)
-constexpr int PG_W = 15;                         // consumer warps
+// 15 consumer warps + 1 producer = 16 warps = 4 per SM sub-partition -> 128 registers per thread.
 constexpr int PG_CONSUMERS = PG_W * 32;          // 480 threads
 constexpr int PG_THREADS = PG_CONSUMERS + 32;    // 512
-constexpr int PG_BPW = 4;                         // 512-byte blocks per warp per chunk (one mbarrier wait / release)
-constexpr int PG_CHUNK_PIECES = PG_W * PG_BPW / 2;   // 30 pieces of 1 KiB = 60 blocks of 32 ch x 64 k: four per warp
-constexpr int PG_SLOT_BYTES = PG_CHUNK_PIECES * 1024;
-constexpr int PG_XHI_BYTES = 65536;              // M <= 16 variant: B fragments of tokens 8-15 (8 * K bytes, K <= 8192)
-__host__ __device__ constexpr int pg_nslot(int maxmt) { return maxmt == 1 ? 6 : 4; }
-constexpr int PG_DESC_BYTES = 15360;             // stage + linear descriptors cached in shared memory
-constexpr int PG_NBMAX = 9;                      // k blocks per warp per granule: ceil(128 / 15)  ->  K <= 8192
-constexpr int PG_NCHUNK = 3;                     // chunks of 60 blocks that cover 128 blocks
-constexpr int PG_RED_STRIDE = 36;                // ints per token row: fragment lane (g,t) -> bank 8t + g, conflict-free
-constexpr int PG_RED_BUF_INTS = 16 * PG_RED_STRIDE;   // one [16 tokens][32 channels] int32 accumulation tile
-constexpr int PG_TEAMS = 3, PG_TW = 5;           // team mode (K <= 2880): three teams of five warps, one granule each
-constexpr int PG_TEAM_NBLK = PG_NBMAX * PG_TW;   // 45 k blocks: a team warp still holds its B fragments in 9 x uint4
-static_assert(PG_TEAM_NBLK == 45 && PG_TEAMS == 3, "prog_team_mode() in program.h assumes 45 k blocks and 3 teams");
-constexpr int PG_RED_INTS = 2 * PG_TEAMS * PG_RED_BUF_INTS;   // two tiles (granule parity) per team: 13 824 B
-// Per-CTA digest of the stage table, built in the prologue (before griddepcontrol.wait): one word per stage, so that the
-// scans "which rows do I quantise in this phase" and "which stages is my group in" cost one shared-memory load per stage
-// instead of ~250 cycles of dependent descriptor loads (12 independent stages: 2 x 1.5 us at the head of every launch).
-constexpr int PG_INFO_WORDS = 288;               // >= PG_DESC_BYTES / sizeof(DevStage)
-constexpr uint32_t INFO_RANK = 0xFFFFu;          // rank in the stage's CTA group + 1 (0: not a member)
-constexpr uint32_t INFO_PHASE_START = 1u << 16;  // first stage of its phase
+constexpr uint32_t INFO_STAGE = 0xFFFFu;         // s_info[phase]: the stage this CTA runs in the phase + 1 (0: none)
 constexpr uint32_t INFO_PUBLISH = 1u << 17;      // DevStage.flags bit 1
-constexpr uint32_t INFO_OWNS_ROW = 1u << 18;     // grid-wide row ownership and this CTA owns a row of the stage
-__host__ __device__ constexpr int pg_smem(int maxmt) {
-    return pg_nslot(maxmt) * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES + (maxmt == 1 ? 0 : PG_XHI_BYTES) +
-           2 * pg_nslot(maxmt) * 8 + 64 + 16 + 64 + PG_INFO_WORDS * 4 + 128;
-}
+static_assert(PG_TEAMS * PG_TW == PG_W, "teams must cover the consumer warps");
 
-#ifdef VLA_PROG_TRACE
-// debug-only (never defined in the product build): per-CTA globaltimer stamps, read back by vla_debug_read_trace
-__device__ unsigned long long g_trace[148 * 1024];
-__device__ __forceinline__ void trace(int cta, int& n, int tid) {
-    if (tid == 0 && n < 1024) {
-        unsigned long long t;
-#ifdef VLA_PROG_TRACE_CLOCK
-        t = (unsigned long long)clock64();               // SM cycles: cheap, per-CTA differences only
+#ifdef VLA_PROG_STAMPS
+// debug builds only: stamp k of this CTA (globaltimer ns) into the program buffer, 32 slots per CTA
+#define PG_STAMP(k) do { if (threadIdx.x == 0 && P.stamps) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.stamps[blockIdx.x * 32 + (k)] = t_; } } while (0)
 #else
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+#define PG_STAMP(k) do { } while (0)
 #endif
-        g_trace[blockIdx.x * 1024 + n++] = t;
-    }
-}
-#define QTRACE(k) do { if (threadIdx.x == 0 && g_trace[blockIdx.x * 1024 + 900 + (k)] == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_trace[blockIdx.x * 1024 + 900 + (k)] = t_; } } while (0)
-#define TRACE() trace(cta, tr_n, tid)
-#define TRARG , tr_n
-// launch-to-launch view: stamp k (0 entry, 1 after griddepcontrol.wait, 2 first MMA may start, 3 end) of the last 16
-// launches of every CTA; the launch ordinal rides in the header's magic field (debug build only)
-__device__ unsigned long long g_pdl[148 * 16 * 8];
-__device__ unsigned g_ord;
-#define PDLT(k) do { if (threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_pdl[(blockIdx.x * 16 + (P.magic & 15)) * 8 + (k)] = t_; } } while (0)
-#define QT(k) do { if (threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_pdl[(blockIdx.x * 16 + (g_ord & 15)) * 8 + (k)] = t_; } } while (0)
-#else
-#define PDLT(k) do { } while (0)
-#define QT(k) do { } while (0)
-#define TRACE()
-#define QTRACE(k) do { } while (0)
-#define TRARG
-#endif
+#define PG_STAMPP(k, p) PG_STAMP(((k) - 2) + 2 + 6 * ((p) & 3) + 2)
 
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(PG_CONSUMERS) : "memory"); }
+__device__ __forceinline__ void team_bar(int team) {
+    asm volatile("bar.sync %0, %1;" :: "r"(2 + team), "n"(PG_TW * 32) : "memory");
+}
 
 __device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned* p) {
     unsigned v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+// A CTA that never becomes resident (the grid is sized for co-residency at build time, but the device may be shared)
+// would make this spin forever: after ~2 s the kernel traps, so a hang becomes a launch error (VLA_ERR_CUDA).
 __device__ __forceinline__ void spin_until(const unsigned* p, unsigned target) {
-    while (ld_acquire_gpu(p) < target) { }
+    const long long t0 = clock64();
+    while (ld_acquire_gpu(p) < target) {
+        if (clock64() - t0 > (1ll << 32)) __trap();
+    }
 }
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 r;
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr) : "memory");
     return r;
 }
-
+__device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 __device__ __forceinline__ int lds32(uint32_t addr) {
     int r;
     asm volatile("ld.shared.s32 %0, [%1];" : "=r"(r) : "r"(addr));
@@ -122,12 +88,10 @@ __device__ __forceinline__ void sts32(uint32_t addr, int v) {
 __device__ __forceinline__ void red_shared_add(uint32_t addr, int v) {
     asm volatile("red.shared.add.s32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
 }
-
 // publish: every store this CTA made before the preceding consumer_bar() becomes visible before the count does
 __device__ __forceinline__ void red_release_gpu(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
-
 // non-volatile form: the compiler may interleave it with the decode of the next block
 __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
                                                    uint32_t b0, uint32_t b1) {
@@ -136,450 +100,385 @@ __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uin
         : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
+// ---------------------------------------------------------------- ring bookkeeping
+// chunk number `seq` of this CTA (in producer order) lives in slot seq % nslot, in ring round seq / nslot
+struct Ring { uint32_t base, slot_bytes, nslot, bar_full, bar_empty; };
+struct RingPos { uint32_t slot, parity; };
+__device__ __forceinline__ RingPos ring_pos(uint32_t seq, uint32_t nslot) {
+    const uint32_t round = seq / nslot;
+    return RingPos{seq - round * nslot, round & 1u};
+}
+
 // ---------------------------------------------------------------- producer warp
-template <int NSLOT>
-__device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, const uint32_t* s_info, int cta,
-                                         int lane, uint32_t ring, uint32_t bar_full, uint32_t bar_empty, uint32_t bar_go) {
-    // The first chunk goes out at once; the rest of the ring is filled only after this CTA has its own activation row in
-    // registers (row owners) or has seen its first quantised activations (the others): otherwise 148 rings (26 MB) are requested in the first microsecond and the
-    // few KB of activation rows the quant owners need queue behind them (measured: 2.5-10 us before the first MMA).
-    uint32_t slot = 0, round = 0, issued = 0;
-    for (int s = 0; s < P.n_stages; ++s) {
-        const int rank = (int)(s_info[s] & INFO_RANK) - 1;
-        if (rank < 0) continue;                              // another group's stage
+__device__ __forceinline__ void producer(const DevProg& P, const DevStage* stages, const DevLin* lins, const uint32_t* s_info,
+                                         int cta, int lane, const Ring& R, uint32_t bar_go) {
+    uint32_t seq = 0;
+    for (int p = 0; p < P.n_phases; ++p) {
+        const int s = (int)(s_info[p] & INFO_STAGE) - 1;
+        if (s < 0) continue;                                 // no stage of this phase runs on this CTA
         const DevStage& st = stages[s];
-        const int KB = st.K / TILE_K;                       // 1 KiB pieces per granule
+        const int rank = cta - st.cta_begin;
+        const int KB = st.K / TILE_K;                        // 1 KiB pieces per granule
+        const int cp = pg_chunk_pieces(KB);
         for (int gi = rank; gi < st.granules; gi += st.cta_count) {
             int l = st.lin_begin;
             for (int j = 1; j < st.n_lin; ++j)
                 if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
             const int n32 = gi - lins[l].gran_begin;
             const uint8_t* src = lins[l].packed + (size_t)n32 * KB * 1024;      // the granule is one contiguous run
-            for (int p0 = 0; p0 < KB; p0 += PG_CHUNK_PIECES) {
-                const int np = min(PG_CHUNK_PIECES, KB - p0);
-                if (issued == 1) mbar_wait(bar_go, 0);
-                ++issued;
-                if (round > 0) mbar_wait(bar_empty + 8u * slot, (round - 1) & 1);
-                if (lane == 0) {                              // one bulk copy of up to 15 KiB per chunk
-                    mbar_arrive_expect_tx(bar_full + 8u * slot, (uint32_t)np * 1024u);
-                    tma_bulk_g2s(ring + slot * PG_SLOT_BYTES, src + (size_t)p0 * 1024, (uint32_t)np * 1024u,
-                                 bar_full + 8u * slot);
+            for (int p0 = 0; p0 < KB; p0 += cp, ++seq) {
+                const int np = min(cp, KB - p0);
+                if (P.gate && seq == 1) mbar_wait(bar_go, 0);
+                const RingPos rp = ring_pos(seq, R.nslot);
+                if (seq >= R.nslot) mbar_wait(R.bar_empty + 8u * rp.slot, rp.parity ^ 1u);
+                if (lane == 0) {                              // one bulk copy of up to 30 KiB per chunk
+                    mbar_arrive_expect_tx(R.bar_full + 8u * rp.slot, (uint32_t)np * 1024u);
+                    tma_bulk_g2s(R.base + rp.slot * R.slot_bytes, src + (size_t)p0 * 1024, (uint32_t)np * 1024u,
+                                 R.bar_full + 8u * rp.slot);
                 }
-                if (++slot == NSLOT) { slot = 0; ++round; }
             }
         }
     }
 }
 
-// ---------------------------------------------------------------- row-owner activation quant (Eq. 4 lines 1-2)
-// All 512 consumer threads of the owner CTA quantise row r of stage st: one pass, the row lives in registers.
-__device__ __forceinline__ void quant_row(const DevStage& st, int r, int tid, float* s_max, uint32_t bar_go, bool& go_sent) {
-    const int nvec = st.K / 8;                               // uint4 of 8 bf16; K <= 8192 -> nvec <= 1024
-    const uint4* xr = st.x + (size_t)r * nvec;
-    const uint4 z = make_uint4(0, 0, 0, 0);
-    QTRACE(0);
-    QT(4);
-    const uint4 v0 = (tid < nvec) ? __ldcg(xr + tid) : z;
-    const uint4 v1 = (tid + PG_CONSUMERS < nvec) ? __ldcg(xr + tid + PG_CONSUMERS) : z;
-    const uint4 v2 = (tid + 2 * PG_CONSUMERS < nvec) ? __ldcg(xr + tid + 2 * PG_CONSUMERS) : z;
-    float m = absmax8(v2, absmax8(v1, absmax8(v0, 0.0f)));
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
-    if ((tid & 31) == 0) s_max[tid >> 5] = m;
-    QTRACE(1);
-    consumer_bar();
-    if (!go_sent) {                                          // the row is in registers: the ring may fill now
-        if (tid == 0) mbar_arrive(bar_go);
-        go_sent = true;
-    }
-    QTRACE(2);
-    QT(5);
-    m = s_max[0];
-#pragma unroll
-    for (int i = 1; i < PG_W; ++i) m = fmaxf(m, s_max[i]);
-    const float alpha = alpha_of(m);
-    if (tid == 0) st.xs[r] = alpha;
-    uint2* qr = st.xq + (size_t)r * nvec;
-    if (tid < nvec) qr[tid] = quant8(v0, alpha);
-    if (tid + PG_CONSUMERS < nvec) qr[tid + PG_CONSUMERS] = quant8(v1, alpha);
-    if (tid + 2 * PG_CONSUMERS < nvec) qr[tid + 2 * PG_CONSUMERS] = quant8(v2, alpha);
-    QTRACE(3);
-    consumer_bar();                                          // s_max may be reused; stores precede thread 0's fence
-    QTRACE(4);
-    QT(6);
+// ---------------------------------------------------------------- fused activation quant (Eq. 4 lines 1-2)
+// Exact shortcut for  a = rint(x / alpha)  (quant.cuh's q1, two true divisions):  with  inv = RN(1 / alpha),
+// the products x * inv * (1 -+ 2^-19) bracket fl(x / alpha) (which is x / alpha within 2^-24 relative), and an FMA with
+// 1.5 * 2^23 rounds each of them to the nearest integer, ties to even, exactly.  rint(fl(.)) is monotone, so when both
+// ends give the same integer it IS the result; when they differ (a rounding boundary inside the bracket: < 5e-4 of the
+// elements) the 16 elements are redone with the true-division quantiser.  |x / alpha| <= 127 (1 + 2^-23): no clamp.
+// Two elements per instruction: fma.rn.f32x2.
+__device__ __forceinline__ uint32_t quant4_fast(uint32_t u0, uint32_t u1, float2 ilo, float2 ihi, uint32_t& diff) {
+    const float2 MAGIC = make_float2(12582912.0f, 12582912.0f);
+    const float2 x01 = make_float2(bf16lo(u0), bf16hi(u0)), x23 = make_float2(bf16lo(u1), bf16hi(u1));
+    const float2 a01 = __ffma2_rn(x01, ilo, MAGIC), b01 = __ffma2_rn(x01, ihi, MAGIC);
+    const float2 a23 = __ffma2_rn(x23, ilo, MAGIC), b23 = __ffma2_rn(x23, ihi, MAGIC);
+    const uint32_t a0 = __float_as_uint(a01.x), a1 = __float_as_uint(a01.y), a2 = __float_as_uint(a23.x), a3 = __float_as_uint(a23.y);
+    diff |= (a0 ^ __float_as_uint(b01.x)) | (a1 ^ __float_as_uint(b01.y));
+    diff |= (a2 ^ __float_as_uint(b23.x)) | (a3 ^ __float_as_uint(b23.y));
+    // the int8 result is the low byte of each sum (0x4B400000 + r)
+    return __byte_perm(__byte_perm(a0, a1, 0x0040), __byte_perm(a2, a3, 0x0040), 0x5410);
+}
+// Rare path (a rounding boundary inside an element's bracket): redo exactly those elements with the true-division
+// quantiser of quant.cuh.  One out-of-line copy; the fast path is inlined per task.
+__device__ __forceinline__ uint32_t patch2(uint32_t u, uint32_t o2, int shift, float4 sc) {
+    const float MAGIC = 12582912.0f;
+    const float x0 = bf16lo(u), x1 = bf16hi(u);
+    if (__float_as_uint(__fmaf_rn(x0, sc.y, MAGIC)) != __float_as_uint(__fmaf_rn(x0, sc.z, MAGIC)))
+        o2 = (o2 & ~(0xFFu << shift)) | (q1(x0, sc.x) << shift);
+    if (__float_as_uint(__fmaf_rn(x1, sc.y, MAGIC)) != __float_as_uint(__fmaf_rn(x1, sc.z, MAGIC)))
+        o2 = (o2 & ~(0xFF00u << shift)) | (q1(x1, sc.x) << (shift + 8));
+    return o2;
+}
+__device__ __noinline__ uint4 quant16_patch(uint4 a, uint4 b, float4 sc, uint4 o) {
+    o.x = patch2(a.y, patch2(a.x, o.x, 0, sc), 16, sc);
+    o.y = patch2(a.w, patch2(a.z, o.y, 0, sc), 16, sc);
+    o.z = patch2(b.y, patch2(b.x, o.z, 0, sc), 16, sc);
+    o.w = patch2(b.w, patch2(b.z, o.w, 0, sc), 16, sc);
+    return o;
+}
+__device__ __forceinline__ uint4 quant16(uint4 a, uint4 b, float4 sc) {      // sc = {alpha, inv_lo, inv_hi, -}
+    const float2 ilo = make_float2(sc.y, sc.y), ihi = make_float2(sc.z, sc.z);
+    uint32_t diff = 0;
+    uint4 o;
+    o.x = quant4_fast(a.x, a.y, ilo, ihi, diff);
+    o.y = quant4_fast(a.z, a.w, ilo, ihi, diff);
+    o.z = quant4_fast(b.x, b.y, ilo, ihi, diff);
+    o.w = quant4_fast(b.z, b.w, ilo, ihi, diff);
+    if (diff != 0u) o = quant16_patch(a, b, sc, o);          // rare: a rounding boundary is too close
+    return o;
+}
+// absmax of 8 bf16 as a packed pair of 15-bit magnitudes (bf16 magnitudes order like unsigned integers)
+__device__ __forceinline__ uint32_t absmax8_packed(uint4 v, uint32_t m) {
+    m = __vmaxu2(m, v.x & 0x7FFF7FFFu);
+    m = __vmaxu2(m, v.y & 0x7FFF7FFFu);
+    m = __vmaxu2(m, v.z & 0x7FFF7FFFu);
+    m = __vmaxu2(m, v.w & 0x7FFF7FFFu);
+    return m;
 }
 
-// Row r of stage s is quantised by CTA (row_begin_s + r) mod gridDim.x (row_begin_s is stored reduced mod gridDim.x) -- any CTA, not only the stage's group, so that
-// the rows of all stages of a phase are spread over the whole grid (a 2-CTA group would otherwise quantise 8 rows
-// one after the other).  Called by every CTA at the start of a phase, for all stages [s0, s1) of the phase.
-// own_stage = true: only stage s0, and only if its rows stay inside its group (flag bit 2).
-__device__ __forceinline__ void quant_phase_rows(const DevProg& P, const DevStage* stages, const uint32_t* s_info, int s0,
-                                                 int cta, int G, int tid, float* s_max, bool own_stage, uint32_t bar_go, bool& go_sent) {
-    const int phase = stages[s0].phase;
-    bool waited = false;
-    for (int s = s0; s < (own_stage ? s0 + 1 : P.n_stages) && (s == s0 || !(s_info[s] & INFO_PHASE_START)); ++s) {
-        if (!own_stage && !(s_info[s] & INFO_OWNS_ROW)) continue;        // nothing of this stage is mine (one load)
-        const DevStage& st = stages[s];
-        int r, step;
-        if (st.flags & 4) {                                   // rows stay inside the stage's own CTA group
-            if (!own_stage) continue;                         // (quantised when the group reaches the stage)
-            r = cta - st.cta_begin;
-            step = st.cta_count;
-            if (r < 0 || r >= step) continue;
-        } else {                                              // first row with (row_begin + r) % G == cta
-            if (own_stage) continue;
-            r = cta - st.row_begin;                           // row_begin is already reduced mod gridDim.x
-            if (r < 0) r += G;
-            step = G;
+// The quantised activations of a stage are stored in mma B-fragment order,
+//   base + ((kq * MTS + mt) * 32 + lane) * 16  holds  a[8 mt + lane/4][64 kq + 16 (lane%4) .. +15],
+// either straight into this CTA's shared memory (LOCAL stages: few elements, every CTA of the group quantises all rows
+// itself) or into the stage's scratch in global memory (COOPERATIVE stages: row r is quantised once, by CTA r mod c of
+// the stage's group, and every CTA of the group then pulls the finished fragments with one bulk copy).
+// A TASK is 16 consecutive elements of one row (two 16-byte loads, one 16-byte fragment store).  The rows this CTA
+// handles are first, first + step, ... (< M); task f of a round is handled row f / (K/16), elements 16 (f mod K/16)..,
+// and thread tid takes tasks tid and tid + 480: consecutive threads read consecutive 32 bytes, and one row or eight
+// spread over all threads.  A round holds its rows in registers between the absmax and the quantisation.
+template <bool TO_GLOBAL>
+__device__ __forceinline__ void quant_rows(const DevProg& P, const DevStage& st, int tid, int first, int step, int mts, uint32_t xq_s,
+                                           uint8_t* frag_g, float* alpha_g, float4* s_scale, unsigned* s_rowmax, bool write_out) {
+    const int lane = tid & 31;
+    const int K = st.K, M = st.M, cpr = K / 16;              // tasks per row
+    const uint32_t inv_cpr = st.inv_cpr;                     // f / cpr = umulhi(f, inv_cpr): exact for f * cpr < 2^32
+    const int n_owned = first < M ? (M - first + step - 1) / step : 0;
+    const int rpr = max(1, (PG_QNB * PG_CONSUMERS) / cpr);   // rows per round
+    for (int j0 = 0; j0 < n_owned; j0 += rpr) {
+        const int nt = min(rpr, n_owned - j0) * cpr;
+        uint4 v[2 * PG_QNB];
+#pragma unroll
+        for (int i = 0; i < PG_QNB; ++i) {
+            const int f = tid + i * PG_CONSUMERS;
+            const int j = (int)__umulhi((uint32_t)f, inv_cpr), c = f - j * cpr;
+            const int row = first + (j0 + j) * step;
+            const bool ok = f < nt;
+            const uint4* src = st.x + ((size_t)row * K) / 8 + c * 2;
+            v[2 * i] = ok ? __ldcg(src) : make_uint4(0, 0, 0, 0);
+            v[2 * i + 1] = ok ? __ldcg(src + 1) : make_uint4(0, 0, 0, 0);
         }
-        unsigned done_rows = 0;
-        for (; r < st.M; r += step, ++done_rows) {
-            if (phase > 0 && !waited) {                       // a phase starts only after every earlier phase has completed
-                                                              // (vla_ternary.h: x of ANY of its stages may be an earlier phase's output)
-                if (tid == 0) spin_until(P.bp + (phase - 1), (unsigned)G);
-                consumer_bar();
-                waited = true;
+#pragma unroll
+        for (int i = 0; i < PG_QNB; ++i) {
+            const int f = tid + i * PG_CONSUMERS;
+            if (f - lane < nt) {                              // (warp-uniform)
+                const int row = first + (j0 + (int)__umulhi((uint32_t)f, inv_cpr)) * step;
+                const uint32_t m2 = absmax8_packed(v[2 * i + 1], absmax8_packed(v[2 * i], 0u));
+                const uint32_t mine = max(m2 & 0xFFFFu, m2 >> 16) << 16;      // fp32 bits of the task's absmax
+                const int row_first = __shfl_sync(0xFFFFFFFFu, row, 0), row_last = __shfl_sync(0xFFFFFFFFu, row, 31);
+                if (row_first == row_last) {                  // the usual case: the warp's 32 tasks are in one row
+                    const uint32_t mw = __reduce_max_sync(0xFFFFFFFFu, mine);
+                    if (lane == 0) atomicMax(s_rowmax + row, mw);
+                } else if (f < nt) {
+                    atomicMax(s_rowmax + row, mine);
+                }
             }
-            quant_row(st, r, tid, s_max, bar_go, go_sent);
         }
-        if (done_rows != 0 && tid == 0) red_release_gpu(P.b2 + s, done_rows);    // one release per stage
-        if (done_rows != 0) QT(7);
+        PG_STAMP(26);
+        consumer_bar();
+        PG_STAMP(27);
+        if (tid < 16) {                                      // per row: alpha_m and the bracketing reciprocals
+            const float alpha = alpha_of(__uint_as_float(s_rowmax[tid]));
+            const float inv = __frcp_rn(alpha);
+            s_scale[tid] = make_float4(alpha, __fmul_rn(inv, 1.0f - 1.9073486328125e-06f), __fmul_rn(inv, 1.0f + 1.9073486328125e-06f), 0.0f);
+            const int j = (tid - first) / step;              // is row tid one of this round's rows?
+            if (tid >= first && tid < M && (tid - first) % step == 0 && j >= j0 && j < j0 + rpr) {
+                if (TO_GLOBAL) alpha_g[tid] = alpha;
+                if (write_out && st.xs_out) st.xs_out[tid] = alpha;
+            }
+        }
+        consumer_bar();
+        PG_STAMP(28);
+#pragma unroll
+        for (int i = 0; i < PG_QNB; ++i) {
+            const int f = tid + i * PG_CONSUMERS;
+            if (f < nt) {
+                const int j = (int)__umulhi((uint32_t)f, inv_cpr), c = f - j * cpr;
+                const int row = first + (j0 + j) * step;
+                const uint32_t off = (uint32_t)((((c >> 2) * mts + (row >> 3)) * 32 + (row & 7) * 4 + (c & 3)) * 16);
+                const uint4 q = quant16(v[2 * i], v[2 * i + 1], s_scale[row]);
+                if (TO_GLOBAL) *reinterpret_cast<uint4*>(frag_g + off) = q;
+                else sts128(xq_s + off, q);
+                if (write_out && st.xq_out) *reinterpret_cast<uint4*>(st.xq_out + (size_t)row * K + c * 16) = q;
+            }
+        }
+        PG_STAMP(29);
     }
 }
 
-// ---------------------------------------------------------------- one stage's granules on the consumer warps
-// int8 activations of this warp's k blocks (kq = 16 i + w), as mma B fragments, in registers for the whole stage
-// Tokens 0-7 stay in registers (xv); in the M <= 16 variant the fragments of tokens 8-15 go to this thread's private
-// 16-byte slots of the shared-memory region xhi (64 registers of fragments would spill, and with 227 KB of shared
-// memory there is no L1 left to catch spills).
-__device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
-    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-template <int MAXMT, int W>
-__device__ __forceinline__ void load_xv(const DevStage& st, int tid, uint4 (&xv)[PG_NBMAX], uint32_t xhi) {
-    const int w = (tid >> 5) % W, lane = tid & 31, g = lane >> 2, t = lane & 3;   // W = 5: the warp's index in its team
-    const int K = st.K, nblk = K / BLK_K;
-    const int8_t* xq = reinterpret_cast<const int8_t*>(st.xq);
-    // all loads first, then the shared-memory stores: sts128 is a compiler barrier, and a load issued after it would
-    // wait for the previous one (measured: 9 serial L2 round trips = 3.7 us at M = 16)
-    uint4 hi[MAXMT == 1 ? 1 : PG_NBMAX];
+// ---------------------------------------------------------------- the MMAs of one warp on one ring chunk
+// Blocks lb = first, first + STRIDE, ... (< nb) of the chunk at `slot_addr`; block lb is k block kq0 + lb of the granule.
+// The slot goes back to the producer (NARR arrivals on `bar_empty` by this warp) as soon as the warp's last packed words
+// are in registers, before their MMAs.
+template <int MT, int STRIDE, int GRP, int NARR>
+__device__ __forceinline__ void chunk_mma(uint32_t slot_addr, uint32_t bar_empty, uint32_t xq_s, int first, int nb, int kq0,
+                                          int lane, int (&acc)[2][MT][4], int (&acc2)[2][4]) {
+    const uint32_t wl = slot_addr + (uint32_t)lane * 16u, xl = xq_s + (uint32_t)lane * 16u;
+    int lb0 = first;
+    do {
+        uint4 wv[GRP], xb[GRP], xh[MT == 2 ? GRP : 1];
 #pragma unroll
-    for (int i = 0; i < PG_NBMAX; ++i)
-#pragma unroll
-        for (int mt = 0; mt < MAXMT; ++mt) {
-            const int kq = i * W + w, tok = mt * 8 + g;
-            const uint4 v = (kq < nblk && tok < st.M)
-                                ? __ldcg(reinterpret_cast<const uint4*>(xq + (size_t)tok * K + kq * BLK_K + t * 16))
-                                : make_uint4(0, 0, 0, 0);
-            if (mt == 0) xv[i] = v;
-            else hi[i] = v;
+        for (int ii = 0; ii < GRP; ++ii) {
+            const int lb = lb0 + ii * STRIDE;
+            const bool ok = lb < nb;
+            wv[ii] = ok ? lds128(wl + (uint32_t)lb * 512u) : make_uint4(0, 0, 0, 0);
+            xb[ii] = ok ? lds128(xl + (uint32_t)((kq0 + lb) * MT) * 512u) : make_uint4(0, 0, 0, 0);
+            if (MT == 2) xh[ii] = ok ? lds128(xl + (uint32_t)((kq0 + lb) * MT + 1) * 512u) : make_uint4(0, 0, 0, 0);
         }
-    if (MAXMT == 2) {
+        if (lb0 + GRP * STRIDE >= nb) {                       // the last loads of this chunk are out
+            __syncwarp();
+            if (lane < NARR) mbar_arrive(bar_empty);
+        }
 #pragma unroll
-        for (int i = 0; i < PG_NBMAX; ++i) {
-            const int kq = i * W + w;
-            if (kq < nblk) sts128(xhi + (uint32_t)(kq * 32 + lane) * 16u, hi[MAXMT == 1 ? 0 : i]);
+        for (int ii = 0; ii < GRP; ++ii) {
+            if (lb0 + ii * STRIDE < nb) {
+                const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];     // channels 16c+g and 16c+g+8
+                    const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
+                    const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
+                    mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xb[ii].x, xb[ii].y);
+                    mma_m16n8k32_s8_nv(acc2[c], e0, e1, e2, e3, xb[ii].z, xb[ii].w);
+                    if (MT == 2) {
+                        mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh[MT == 2 ? ii : 0].x, xh[MT == 2 ? ii : 0].y);
+                        mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh[MT == 2 ? ii : 0].z, xh[MT == 2 ? ii : 0].w);
+                    }
+                }
+            }
+        }
+        lb0 += GRP * STRIDE;
+    } while (lb0 < nb);
+}
+
+template <int MT>
+__device__ __forceinline__ void zero_acc(int (&acc)[2][MT][4], int (&acc2)[2][4]) {
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc[c][mt][i] = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc2[c][i] = 0;
+    }
+}
+// the warp's partial sums of a granule -> the int32 tile at `rb` ([16 tokens][PG_RED_STRIDE])
+template <int MT>
+__device__ __forceinline__ void add_to_tile(uint32_t rb, int g, int t, int (&acc)[2][MT][4], int (&acc2)[2][4]) {
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[c][0][i] += acc2[c][i];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            const uint32_t row0 = rb + (uint32_t)((mt * 8 + 2 * t) * PG_RED_STRIDE + 16 * c + g) * 4u;
+            red_shared_add(row0, acc[c][mt][0]);
+            red_shared_add(row0 + PG_RED_STRIDE * 4, acc[c][mt][1]);
+            red_shared_add(row0 + 8 * 4, acc[c][mt][2]);
+            red_shared_add(row0 + (PG_RED_STRIDE + 8) * 4, acc[c][mt][3]);
         }
     }
 }
+// one output of a finished tile: read the cell, leave zero behind, dequant (Eq. 4 line 3), store
+__device__ __forceinline__ void emit(uint32_t rb, int tok, int ech, const DevLin& L, int n32, float alpha, float beta) {
+    const uint32_t cell = rb + (uint32_t)(tok * PG_RED_STRIDE + ech) * 4u;
+    const int sum = lds32(cell);
+    sts32(cell, 0);                                           // the tile is all zero again for its next granule
+    const int a = sum >> 6;                                   // the decode's factor 64 leaves exactly
+    const size_t o = (size_t)tok * L.N + (size_t)n32 * BLK_N + ech;
+    if (L.dtype == 2) {
+        reinterpret_cast<int*>(L.out)[o] = a;
+    } else {
+        const float y = dequant(a, __fmul_rn(alpha, beta));
+        if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
+        else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
+    }
+}
+__device__ __forceinline__ int lin_of(const DevLin* lins, const DevStage& st, int gi) {
+    int l = st.lin_begin;
+    for (int j = 1; j < st.n_lin; ++j)
+        if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
+    return l;
+}
 
-// cta / G: rank and size of the stage's CTA group
-template <int MT, int NSLOT>
-__device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& st, int cta, int G,
-                                           int tid, uint32_t ring, int* red, const float* s_beta, uint32_t bar_full, uint32_t bar_empty,
-                                           uint4 (&xv)[PG_NBMAX], uint32_t xhi, uint32_t& slot, uint32_t& phase, uint32_t& gcount
-#ifdef VLA_PROG_TRACE
-                                           , int& tr_n
-#endif
-                                           ) {
-    constexpr int MTOK = MT * 8;
-    // w through a shuffle: the compiler then knows it is warp-uniform and the per-block range checks below become
-    // uniform branches (no BSSY/BSYNC reconvergence around every block)
+// ---------------------------------------------------------------- a stage on all 15 warps (fewer than 3 granules per CTA)
+// rank / G: rank and size of the stage's CTA group.  Warp w takes the k blocks w, w + 15, ... of every chunk.
+template <int MT>
+__device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& st, int rank, int G, int tid, const Ring& R,
+                                           uint32_t red, uint32_t xq_s, const float* s_beta, const float4* s_scale,
+                                           uint32_t& seq, uint32_t& gcount) {
+    // w through a shuffle: the compiler then knows it is warp-uniform
     const int w = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0), lane = tid & 31, g = lane >> 2, t = lane & 3;
-    const int M = st.M, nblk = st.K / BLK_K, KB = st.K / TILE_K;
-    const int nchunks = (KB + PG_CHUNK_PIECES - 1) / PG_CHUNK_PIECES;
-    // epilogue role: output (token tid/32, channel tid%32); the 32 threads of warp 0 also take token 15
-    const int etok = tid >> 5, ech = tid & 31;
-    const bool eactive = (etok < M) && (etok < MTOK);
-    const bool eactive2 = (MT == 2) && (tid < 32) && (M == 16);
-    const float alpha = eactive ? __ldcg(st.xs + etok) : 0.0f;
-    const float alpha2 = eactive2 ? __ldcg(st.xs + 15) : 0.0f;
-    const uint32_t my_off = (uint32_t)(w * 512 + lane * 16);  // block b = ii*15 + w of the chunk
-
-    for (int gi = cta; gi < st.granules; gi += G) {
-        TRACE();
-        int l = st.lin_begin;
-        for (int j = 1; j < st.n_lin; ++j)
-            if (gi >= lins[st.lin_begin + j].gran_begin) l = st.lin_begin + j;
+    const int KB = st.K / TILE_K, cp = pg_chunk_pieces(KB), nout = st.M * 32;
+    for (int gi = rank; gi < st.granules; gi += G) {
+        const int l = lin_of(lins, st, gi);
         const DevLin& L = lins[l];
         const int n32 = gi - L.gran_begin;
         const float beta = s_beta[l - st.lin_begin];          // staged once per stage
-
-#ifdef VLA_PROG_TRACE
-        long long twait = 0;
-#endif
         int acc[2][MT][4], acc2[2][4];                        // acc2: second IMMA chain of token tile 0 (ILP)
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-#pragma unroll
-            for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) acc[c][mt][i] = 0;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) acc2[c][i] = 0;
+        zero_acc<MT>(acc, acc2);
+        for (int p0 = 0; p0 < KB; p0 += cp, ++seq) {
+            const int np = min(cp, KB - p0);
+            const RingPos rp = ring_pos(seq, R.nslot);
+            mbar_wait(R.bar_full + 8u * rp.slot, rp.parity);
+            chunk_mma<MT, PG_W, 2, 1>(R.base + rp.slot * R.slot_bytes, R.bar_empty + 8u * rp.slot, xq_s, w, 2 * np, 2 * p0,
+                                      lane, acc, acc2);       // 15 arrivals (one per warp) hand the slot back
         }
-
-#pragma unroll
-        for (int ck = 0; ck < PG_NCHUNK; ++ck) {              // 3 chunks of 30 KiB cover K <= 8192
-            if (ck < nchunks) {
-#ifdef VLA_PROG_TRACE
-                long long tw0 = clock64();
-#endif
-                mbar_wait(bar_full + 8u * slot, phase);
-#ifdef VLA_PROG_TRACE
-                twait += clock64() - tw0;
-#endif
-                // the four blocks of this warp in the chunk, two at a time; the slot is handed back once the last two
-                // are in registers
-#pragma unroll
-                for (int half = 0; half < PG_BPW / 2; ++half) {
-                    uint4 wv[2];
-#pragma unroll
-                    for (int ii = 0; ii < 2; ++ii) {
-                        const int i = PG_BPW * ck + 2 * half + ii;
-                        wv[ii] = (i < PG_NBMAX && i * PG_W + w < nblk)
-                                     ? lds128(ring + slot * PG_SLOT_BYTES + (2 * half + ii) * (PG_W * 512) + my_off)
-                                     : make_uint4(0, 0, 0, 0);
-                    }
-                    if (half == PG_BPW / 2 - 1) {
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(bar_empty + 8u * slot);   // release: ordered after the loads above
-                    }
-#pragma unroll
-                    for (int ii = 0; ii < 2; ++ii) {
-                        const int i = PG_BPW * ck + 2 * half + ii;
-                        if (i < PG_NBMAX && i * PG_W + w < nblk) {
-                            const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
-                            uint4 xh = make_uint4(0, 0, 0, 0);    // tokens 8-15 of this block (M <= 16 variant)
-                            if (MT == 2) xh = lds128(xhi + (uint32_t)((i * PG_W + w) * 32 + lane) * 16u);
-#pragma unroll
-                            for (int c = 0; c < 2; ++c) {
-                                const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];     // channels 16c+g and 16c+g+8
-                                const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
-                                const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
-                                mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xv[i < PG_NBMAX ? i : 0].x, xv[i < PG_NBMAX ? i : 0].y);
-                                mma_m16n8k32_s8_nv(acc2[c], e0, e1, e2, e3, xv[i < PG_NBMAX ? i : 0].z, xv[i < PG_NBMAX ? i : 0].w);
-                                if (MT == 2) {
-                                    mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh.x, xh.y);
-                                    mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh.z, xh.w);
-                                }
-                            }
-                        }
-                    }
-                }
-                if (++slot == NSLOT) { slot = 0; phase ^= 1; }
-            }
-        }
-
-#ifdef VLA_PROG_TRACE
-        if (tid == 0 && tr_n < 1024) g_trace[blockIdx.x * 1024 + tr_n++] = (unsigned long long)twait;   // cycles, not a stamp
-#endif
-        TRACE();
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) acc[c][0][i] += acc2[c][i];
-        // The 15 per-warp partial sums of an output are added into one int32 tile in shared memory (red.shared.add:
-        // integer addition is exact in any order), two tiles by granule parity: the epilogue of granule g reads and
-        // re-zeroes tile g & 1 while the faster warps already add granule g+1 into the other one.
-        const uint32_t rb = smem_u32(red) + (uint32_t)(gcount & 1) * (PG_RED_BUF_INTS * 4);
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-#pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-                const uint32_t row0 = rb + (uint32_t)((mt * 8 + 2 * t) * PG_RED_STRIDE + 16 * c + g) * 4u;
-                red_shared_add(row0, acc[c][mt][0]);
-                red_shared_add(row0 + PG_RED_STRIDE * 4, acc[c][mt][1]);
-                red_shared_add(row0 + 8 * 4, acc[c][mt][2]);
-                red_shared_add(row0 + (PG_RED_STRIDE + 8) * 4, acc[c][mt][3]);
-            }
+        // The 15 per-warp partial sums of an output are added into one int32 tile (two tiles by granule parity: the
+        // epilogue of granule g reads and re-zeroes tile g & 1 while the faster warps already add granule g+1 into the other).
+        const uint32_t rb = red + (uint32_t)(gcount & 1) * (PG_RED_BUF_INTS * 4);
+        add_to_tile<MT>(rb, g, t, acc, acc2);
         consumer_bar();
-        TRACE();
-#pragma unroll
-        for (int rep = 0; rep < MT; ++rep) {
-            const bool act = rep == 0 ? eactive : eactive2;
-            const int tok = rep == 0 ? etok : 15;
-            if (act) {
-                const uint32_t cell = rb + (uint32_t)(tok * PG_RED_STRIDE + ech) * 4u;
-                const int sum = lds32(cell);
-                sts32(cell, 0);                               // the tile is all zero again for granule g+2
-                const int a = sum >> 6;                       // the decode's factor 64 leaves exactly
-                const size_t o = (size_t)tok * L.N + (size_t)n32 * BLK_N + ech;
-                if (L.dtype == 2) {
-                    reinterpret_cast<int*>(L.out)[o] = a;
-                } else {
-                    const float y = dequant(a, __fmul_rn(rep == 0 ? alpha : alpha2, beta));
-                    if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
-                    else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
-                }
-            }
-        }
-        TRACE();
+        for (int idx = tid; idx < nout; idx += PG_CONSUMERS) emit(rb, idx >> 5, idx & 31, L, n32, s_scale[idx >> 5].x, beta);
         ++gcount;
     }
 }
 
-// ---------------------------------------------------------------- team mode (K <= 2880, >= 2 granules per CTA)
-// The 15 consumer warps work as THREE independent teams of five: team q takes the CTA's granules n = q, q+3, ... of the
-// stage (ring chunk n: with K <= 3840 a chunk is exactly one granule, so the producer is unchanged), its warp j owns the
-// k blocks kq = j (mod 5).  Against the 15-way split a warp runs 8 blocks instead of 3 per mbarrier wait / reduction /
-// barrier / epilogue, and the three teams are in different phases of their granules instead of in lockstep (chunk
-// arrival -> decode burst -> barrier), which is what bounded the 15-way loop.
-__device__ __forceinline__ void team_bar(int team) {
-    asm volatile("bar.sync %0, %1;" :: "r"(2 + team), "n"(PG_TW * 32) : "memory");
-}
-template <int MT, int NSLOT>
-__device__ __forceinline__ void stage_gemm_teams(const DevLin* lins, const DevStage& st, int rank, int G, int tid, uint32_t ring,
-                                                 int* red, const float* s_beta, const float* s_alpha, uint32_t bar_full,
-                                                 uint32_t bar_empty, uint4 (&xv)[PG_NBMAX], uint32_t xhi, uint32_t& slot,
-                                                 uint32_t& phase, uint32_t& gcount) {
+// ---------------------------------------------------------------- a stage on three teams of five warps
+// Team q takes the CTA's granules n = q, q+3, ... of the stage (ring chunks n * nchunks ..), its warp j the k blocks
+// j, j + 5, ... of every chunk.  Against the 15-way split a warp runs three times as many blocks per mbarrier wait /
+// reduction / barrier / epilogue, and the teams are in different phases of their granules instead of in lockstep.
+template <int MT>
+__device__ __forceinline__ void stage_gemm_teams(const DevLin* lins, const DevStage& st, int rank, int G, int tid, const Ring& R,
+                                                 uint32_t red, uint32_t xq_s, const float* s_beta, const float4* s_scale,
+                                                 uint32_t& seq, uint32_t& gcount) {
     const int w = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0), lane = tid & 31, g = lane >> 2, t = lane & 3;
     const int team = w / PG_TW, j = w - team * PG_TW, ttid = tid - team * (PG_TW * 32);
-    const int nblk = st.K / BLK_K, nout = st.M * 32;
-    const int ng = rank < st.granules ? (st.granules - rank + G - 1) / G : 0;      // this CTA's granules (= ring chunks)
-    const uint32_t tiles = smem_u32(red) + (uint32_t)team * (2 * PG_RED_BUF_INTS * 4);
+    const int KB = st.K / TILE_K, cp = pg_chunk_pieces(KB), nch = pg_chunks(KB), nout = st.M * 32;
+    const int ng = rank < st.granules ? (st.granules - rank + G - 1) / G : 0;      // this CTA's granules of the stage
+    const uint32_t tiles = red + (uint32_t)team * (2 * PG_RED_BUF_INTS * 4);
     uint32_t tpar = 0;
     for (int n = team; n < ng; n += PG_TEAMS) {
         const int gi = rank + n * G;
-        int l = st.lin_begin;
-        for (int q = 1; q < st.n_lin; ++q)
-            if (gi >= lins[st.lin_begin + q].gran_begin) l = st.lin_begin + q;
+        const int l = lin_of(lins, st, gi);
         const DevLin& L = lins[l];
         const int n32 = gi - L.gran_begin;
         const float beta = s_beta[l - st.lin_begin];
-        uint32_t sl = slot + (uint32_t)n;                     // ring position of chunk n of this stage
-        const uint32_t wraps = sl / NSLOT;
-        sl -= wraps * NSLOT;
-        const uint32_t ph = phase ^ (wraps & 1u);
-
         int acc[2][MT][4], acc2[2][4];
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-#pragma unroll
-            for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) acc[c][mt][i] = 0;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) acc2[c][i] = 0;
+        zero_acc<MT>(acc, acc2);
+        uint32_t cs = seq + (uint32_t)(n * nch);
+        for (int p0 = 0; p0 < KB; p0 += cp, ++cs) {
+            const int np = min(cp, KB - p0);
+            const RingPos rp = ring_pos(cs, R.nslot);
+            mbar_wait(R.bar_full + 8u * rp.slot, rp.parity);
+            chunk_mma<MT, PG_TW, 3, PG_TEAMS>(R.base + rp.slot * R.slot_bytes, R.bar_empty + 8u * rp.slot, xq_s, j, 2 * np,
+                                              2 * p0, lane, acc, acc2);       // (the empty barrier counts 15: three arrivals per team warp)
         }
-        mbar_wait(bar_full + 8u * sl, ph);
-        const uint32_t src = ring + sl * PG_SLOT_BYTES + (uint32_t)lane * 16u;   // block kq of the granule at kq * 512
-#pragma unroll
-        for (int i0 = 0; i0 < PG_NBMAX; i0 += 3) {
-            uint4 wv[3];
-#pragma unroll
-            for (int ii = 0; ii < 3; ++ii) {
-                const int kq = (i0 + ii) * PG_TW + j;
-                wv[ii] = (kq < nblk) ? lds128(src + (uint32_t)kq * 512u) : make_uint4(0, 0, 0, 0);
-            }
-            if (i0 + 3 >= PG_NBMAX) {                         // last loads are out: hand the slot back
-                __syncwarp();                                 // (the empty barrier counts 15: three arrivals per team warp)
-                if (lane < PG_TEAMS) mbar_arrive(bar_empty + 8u * sl);
-            }
-#pragma unroll
-            for (int ii = 0; ii < 3; ++ii) {
-                const int i = i0 + ii, kq = i * PG_TW + j;
-                if (kq < nblk) {
-                    const uint32_t w4[4] = {wv[ii].x, wv[ii].y, wv[ii].z, wv[ii].w};
-                    uint4 xh = make_uint4(0, 0, 0, 0);
-                    if (MT == 2) xh = lds128(xhi + (uint32_t)(kq * 32 + lane) * 16u);
-#pragma unroll
-                    for (int c = 0; c < 2; ++c) {
-                        const uint32_t wa = w4[2 * c], wb = w4[2 * c + 1];
-                        const uint32_t a0 = decode64<0>(wa), a1 = decode64<0>(wb), a2 = decode64<1>(wa), a3 = decode64<1>(wb);
-                        const uint32_t e0 = decode64<2>(wa), e1 = decode64<2>(wb), e2 = decode64<3>(wa), e3 = decode64<3>(wb);
-                        mma_m16n8k32_s8_nv(acc[c][0], a0, a1, a2, a3, xv[i].x, xv[i].y);
-                        mma_m16n8k32_s8_nv(acc2[c], e0, e1, e2, e3, xv[i].z, xv[i].w);
-                        if (MT == 2) {
-                            mma_m16n8k32_s8_nv(acc[c][1], a0, a1, a2, a3, xh.x, xh.y);
-                            mma_m16n8k32_s8_nv(acc[c][1], e0, e1, e2, e3, xh.z, xh.w);
-                        }
-                    }
-                }
-            }
-        }
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) acc[c][0][i] += acc2[c][i];
         const uint32_t rb = tiles + tpar * (PG_RED_BUF_INTS * 4);
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-#pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-                const uint32_t row0 = rb + (uint32_t)((mt * 8 + 2 * t) * PG_RED_STRIDE + 16 * c + g) * 4u;
-                red_shared_add(row0, acc[c][mt][0]);
-                red_shared_add(row0 + PG_RED_STRIDE * 4, acc[c][mt][1]);
-                red_shared_add(row0 + 8 * 4, acc[c][mt][2]);
-                red_shared_add(row0 + (PG_RED_STRIDE + 8) * 4, acc[c][mt][3]);
-            }
+        add_to_tile<MT>(rb, g, t, acc, acc2);
         team_bar(team);
-        for (int idx = ttid; idx < nout; idx += PG_TW * 32) {  // one output per thread and pass: token idx / 32, channel idx % 32
-            const int tok = idx >> 5, ech = idx & 31;
-            const uint32_t cell = rb + (uint32_t)(tok * PG_RED_STRIDE + ech) * 4u;
-            const int sum = lds32(cell);
-            sts32(cell, 0);
-            const int a = sum >> 6;
-            const size_t o = (size_t)tok * L.N + (size_t)n32 * BLK_N + ech;
-            if (L.dtype == 2) {
-                reinterpret_cast<int*>(L.out)[o] = a;
-            } else {
-                const float y = dequant(a, __fmul_rn(s_alpha[tok], beta));
-                if (L.dtype == 0) reinterpret_cast<float*>(L.out)[o] = y;
-                else reinterpret_cast<__nv_bfloat16*>(L.out)[o] = __float2bfloat16_rn(y);
-            }
-        }
+        for (int idx = ttid; idx < nout; idx += PG_TW * 32) emit(rb, idx >> 5, idx & 31, L, n32, s_scale[idx >> 5].x, beta);
         tpar ^= 1u;
     }
-    uint32_t sl = slot + (uint32_t)ng;                        // every warp: the ring position after this stage's chunks
-    const uint32_t wraps = sl / NSLOT;
-    slot = sl - wraps * NSLOT;
-    phase ^= (wraps & 1u);
+    seq += (uint32_t)(ng * nch);
     gcount += (uint32_t)ng;
-    consumer_bar();                                           // all three teams are done with s_beta / s_alpha / xhi
 }
 
 // ---------------------------------------------------------------- the kernel
-// MAXMT = 1: every stage has M <= 8 (32 registers of B fragments per thread, no spills);  MAXMT = 2: M <= 16.
+// MAXMT = 1: every stage has M <= 8;  MAXMT = 2: M <= 16 (two token tiles).
 template <int MAXMT>
 __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_constant__ DevProg P) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 127u) & ~127u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
-    const uint32_t ring = base;
-    constexpr int NSLOT = pg_nslot(MAXMT);
-    constexpr int XHI = (MAXMT == 1) ? 0 : PG_XHI_BYTES;
-    int* red = reinterpret_cast<int*>(base_ptr + NSLOT * PG_SLOT_BYTES);
-    uint8_t* desc = base_ptr + NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4;
-    const uint32_t xhi = base + NSLOT * PG_SLOT_BYTES + PG_RED_INTS * 4 + PG_DESC_BYTES;
-    const uint32_t bar_full = xhi + XHI;
-    const uint32_t bar_empty = bar_full + 8u * NSLOT;
-    const uint32_t bar_go = bar_empty + 8u * NSLOT + 64u;    // after s_max (64 B)
-    float* s_beta = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT + 64 + 16);   // 16 floats
-    float* s_max = reinterpret_cast<float*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT);
-    uint32_t* s_info = reinterpret_cast<uint32_t*>(desc + PG_DESC_BYTES + XHI + 16 * NSLOT + 64 + 16 + 64);
+    const uint32_t bar_full = base + PG_OFF_BAR, bar_empty = bar_full + 8u * PG_NSLOT_MAX, bar_go = bar_empty + 8u * PG_NSLOT_MAX;
+    const uint32_t bar_xq = bar_go + 8u;
+    float4* s_scale = reinterpret_cast<float4*>(base_ptr + PG_OFF_ALPHA);
+    float* s_beta = reinterpret_cast<float*>(base_ptr + PG_OFF_BETA);
+    unsigned* s_rowmax = reinterpret_cast<unsigned*>(base_ptr + PG_OFF_ROWMAX);
+    unsigned* s_misc = reinterpret_cast<unsigned*>(base_ptr + PG_OFF_MISC);
+    int* red_ptr = reinterpret_cast<int*>(base_ptr + PG_OFF_RED);
+    const uint32_t red = base + PG_OFF_RED;
+    uint32_t* s_info = reinterpret_cast<uint32_t*>(base_ptr + PG_OFF_INFO);        // per PHASE: this CTA's stage + 1, publish bit
+    uint8_t* desc = base_ptr + pg_off_desc(P.n_stages);
+    const uint32_t xq_s = base + (uint32_t)pg_off_xq(P.n_stages, P.n_lin);
 
     const int tid = threadIdx.x, cta = blockIdx.x, G = gridDim.x;
-    PDLT(0);
+    PG_STAMP(0);
     if (tid == 0) {
-        for (int s = 0; s < NSLOT; ++s) {
+        for (int s = 0; s < PG_NSLOT_MAX; ++s) {
             mbar_init(bar_full + 8u * s, 1);
             mbar_init(bar_empty + 8u * s, PG_W);
         }
         mbar_init(bar_go, 1);
+        mbar_init(bar_xq, 1);
         fence_barrier_init();
+        s_misc[0] = 0u;
+        s_misc[1] = 0u;
     }
-    for (int i = tid; i < PG_RED_INTS; i += PG_THREADS) red[i] = 0;      // accumulation tiles start at zero
+    if (tid < 16) s_rowmax[tid] = 0u;
+    for (int i = tid; i < P.n_phases; i += PG_THREADS) s_info[i] = 0u;
+    for (int i = tid; i < PG_RED_INTS; i += PG_THREADS) red_ptr[i] = 0;  // accumulation tiles start at zero
     // descriptor tables -> shared memory (they are read on every granule by producer and consumers)
     const int stage_words = P.n_stages * (int)(sizeof(DevStage) / 8), lin_words = P.n_lin * (int)(sizeof(DevLin) / 8);
     {
@@ -590,156 +489,168 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         for (int i = tid; i < lin_words; i += PG_THREADS) d[stage_words + i] = gl[i];
     }
     __syncthreads();
-    for (int s = tid; s < P.n_stages; s += PG_THREADS) {     // the digest of the stage table for this CTA
-        const DevStage& st = reinterpret_cast<const DevStage*>(desc)[s];
+    const DevStage* stages = reinterpret_cast<const DevStage*>(desc);
+    const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
+    // Digest of the stage table for this CTA: the groups of one phase are disjoint, so a CTA runs at most one stage per
+    // phase; s_info[phase] = that stage + 1 (0: none), plus the phase's publish bit.
+    for (int s = tid; s < P.n_stages; s += PG_THREADS) {
+        const DevStage& st = stages[s];
         const int rank = cta - st.cta_begin;
-        uint32_t info = (rank >= 0 && rank < st.cta_count) ? (uint32_t)(rank + 1) : 0u;
-        if (s == 0 || reinterpret_cast<const DevStage*>(desc)[s - 1].phase != st.phase) info |= INFO_PHASE_START;
-        if (st.flags & 2) info |= INFO_PUBLISH;
-        if (!(st.flags & 4)) {
-            int r = cta - st.row_begin;                       // first row with (row_begin + r) % G == cta
-            if (r < 0) r += G;
-            if (r < st.M) info |= INFO_OWNS_ROW;
+        if (st.flags & 2) atomicOr(s_info + st.phase, INFO_PUBLISH);
+        if (rank >= 0 && rank < st.cta_count) {
+            atomicOr(s_info + st.phase, (uint32_t)(s + 1));
+            atomicMax(s_misc, (unsigned)pg_xq_bytes(st.M, st.K));      // this CTA's largest activation matrix
+            atomicMax(s_misc + 1, (unsigned)pg_slot_bytes(st.K));      // and largest ring chunk
         }
-        s_info[s] = info;
     }
     __syncthreads();
-    // Programmatic dependent launch: everything above (barrier init, the static descriptor tables) may overlap the
-    // tail of the previous kernel on this stream; counters, activations, weights-in-flight and outputs come after.
+    // the ring takes what the descriptors and this CTA's quantised activations leave free, in slots of its largest chunk
+    Ring R;
+    R.base = xq_s + ((s_misc[0] + 127u) & ~127u);
+    R.slot_bytes = max(s_misc[1], 1024u);
+    R.nslot = min((uint32_t)PG_NSLOT_MAX, (base + (uint32_t)P.smem_bytes - R.base) / R.slot_bytes);
+    R.bar_full = bar_full;
+    R.bar_empty = bar_empty;
+
+    if (tid >= PG_CONSUMERS) {
+        // Weights never depend on the previous kernel on the stream: the ring starts filling under its tail.
+        pdl_launch_dependents();
+        producer(P, stages, lins, s_info, cta, tid & 31, R, bar_go);
+        return;
+    }
+    // Programmatic dependent launch: everything above (barrier init, the static descriptor tables, the first ring
+    // chunks) may overlap the tail of the previous kernel on this stream; counters, activations and outputs come after.
     pdl_wait();
-    PDLT(1);
-#ifdef VLA_PROG_TRACE
-    if (tid == 0) g_ord = P.magic;
-#endif
     // Trigger the next launch NOW: its CTAs take this SM as soon as this CTA exits and run their own prologue (up to their
     // griddepcontrol.wait, which still waits for this whole grid and its memory) under the tail of this grid.
     pdl_launch_dependents();
-    const DevStage* stages = reinterpret_cast<const DevStage*>(desc);
-    const DevLin* lins = reinterpret_cast<const DevLin*>(desc + (size_t)stage_words * 8);
+    PG_STAMP(1);
 
-    if (tid >= PG_CONSUMERS) {
-        producer<NSLOT>(P, stages, lins, s_info, cta, tid & 31, ring, bar_full, bar_empty, bar_go);
-        return;
-    }
-#ifdef VLA_PROG_TRACE
-    int tr_n = 0;
-#endif
-    TRACE();
-    uint4 xv[PG_NBMAX];
     bool go_sent = false;
-    uint32_t slot = 0, phase = 0, gcount = 0;
+    uint32_t seq = 0, gcount = 0, xq_par = 0;
     unsigned done_prev = 0xFFFFFFFFu;                        // thread 0: what its early arrival on `done` returned
-    for (int s = 0; s < P.n_stages; ++s) {
-        const uint32_t info = s_info[s];
-        if (info & INFO_PHASE_START) {                       // a new phase: quantise the rows this CTA owns
-            TRACE();
-            quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, false, bar_go, go_sent);
-            TRACE();
-        }
-        const int rank = (int)(info & INFO_RANK) - 1;
-        if (rank >= 0) {                                     // this CTA belongs to the stage's group
+    for (int p = 0; p < P.n_phases; ++p) {
+        const uint32_t info = s_info[p];
+        const int s = (int)(info & INFO_STAGE) - 1;
+        if (s >= 0) {                                        // this CTA runs stage s in phase p
             const DevStage& st = stages[s];
-            const int count = st.cta_count;
-            if (st.flags & 4) quant_phase_rows(P, stages, s_info, s, cta, G, tid, s_max, true, bar_go, go_sent);
-            TRACE();
-            if (tid == 0) {
-                spin_until(P.b2 + s, (unsigned)st.M);
-                if (!go_sent) mbar_arrive(bar_go);            // let the producer fill the rest of the ring
-                if (P.n_phases == 1) {
-                    // Single-phase program (a CTA is in exactly one group): this was the CTA's last access to the program's
-                    // counters.  Count it as done NOW: the round trip of the atomic overlaps the stage's GEMM instead of
-                    // sitting between the last CTA's last store and the end of the grid (~0.4 us of an 18 us decode step).
-                    // Every counter the reset clears has its final value by then: a stage's members pass their spin only
-                    // after all of its rows' arrivals, and they count themselves done after that spin (no fence needed).
-                    done_prev = atomicAdd(P.done, 1u);
-                }
+            const int count = st.cta_count, rank = cta - st.cta_begin;
+            PG_STAMPP(6, p);
+            if (p > 0) {                                     // a phase starts only after every earlier phase has completed
+                                                              // (vla_ternary.h: x of ANY of its stages may be an earlier phase's output)
+                if (tid == 0) spin_until(P.bp + (p - 1), (unsigned)G);
+                consumer_bar();
             }
-            go_sent = true;
+            PG_STAMPP(2, p);
             // the stage's scales beta -> shared memory (one L2 round trip per stage instead of one per granule)
+            // (loaded now, stored after the quantisation: a cold scale costs a DRAM round trip that must not delay this
+            // warp's activation loads)
+            float beta_r = 0.0f;
             if (tid >= 32 && tid < 32 + st.n_lin) {
                 const DevLin& L = lins[st.lin_begin + tid - 32];
-                s_beta[tid - 32] = (L.dtype != 2) ? __ldcg(L.beta) : 0.0f;
+                if (L.dtype != 2) beta_r = __ldcg(L.beta);
             }
-            consumer_bar();
-            TRACE();
-            PDLT(2);
-            // team mode: the B fragments of a five-way k split still fit in registers and every team gets >= 2 granules
-            const bool teams = prog_team_mode(st.K, st.granules, count);
-            if (teams) {
-                if (tid < st.M) s_max[tid] = __ldcg(st.xs + tid);     // alpha_m for the team epilogues (s_max is free here)
-                load_xv<MAXMT, PG_TW>(st, tid, xv, xhi);
-                consumer_bar();                               // s_max and (M > 8) the shared B fragments are complete
-                if (MAXMT == 1 || st.M <= 8)
-                    stage_gemm_teams<1, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, s_max, bar_full, bar_empty, xv, xhi, slot, phase, gcount);
-                else
-                    stage_gemm_teams<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, s_max, bar_full, bar_empty, xv, xhi, slot, phase, gcount);
+            const int mts = (MAXMT == 2 && st.M > 8) ? 2 : 1;
+            if (st.coop != nullptr) {
+                // cooperative quant: this CTA's rows (rank, rank + count, ...) -> the stage's scratch, then publish
+                float* alpha_g = reinterpret_cast<float*>(st.coop + pg_xq_bytes(st.M, st.K));
+                quant_rows<true>(P, st, tid, rank, count, mts, 0u, st.coop, alpha_g, s_scale, s_rowmax, true);
+                consumer_bar();                              // every fragment store of this CTA precedes the release
+                if (tid == 0) {
+                    const int mine = rank < st.M ? (st.M - rank + count - 1) / count : 0;
+                    if (mine) red_release_gpu(P.cnt + s, (unsigned)mine);
+                    spin_until(P.cnt + s, (unsigned)st.M);    // all rows of the stage are in the scratch
+                    if (P.n_phases == 1) done_prev = atomicAdd(P.done, 1u);      // (its last counter access: see the end)
+                    asm volatile("fence.proxy.async.global;" ::: "memory");     // generic-proxy writes -> the bulk copy's reads
+                    const uint32_t bytes = (uint32_t)pg_xq_bytes(st.M, st.K);
+                    mbar_arrive_expect_tx(bar_xq, bytes);
+                    for (uint32_t o = 0; o < bytes; o += 32768u)
+                        tma_bulk_g2s(xq_s + o, st.coop + o, min(32768u, bytes - o), bar_xq);
+                    if (!go_sent) mbar_arrive(bar_go);
+                }
+                go_sent = true;
+                mbar_wait(bar_xq, xq_par);
+                xq_par ^= 1u;
+                if (tid < 16) s_scale[tid].x = __ldcg(alpha_g + tid);
             } else {
-                load_xv<MAXMT, PG_W>(st, tid, xv, xhi);
-                if (MAXMT == 1 || st.M <= 8)
-                    stage_gemm<1, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
-                else
-                    stage_gemm<MAXMT, NSLOT>(lins, st, rank, count, tid, ring, red, s_beta, bar_full, bar_empty, xv, xhi, slot, phase, gcount TRARG);
+                // small stage: every CTA of the group quantises all rows into its own shared memory
+                quant_rows<false>(P, st, tid, 0, 1, mts, xq_s, nullptr, nullptr, s_scale, s_rowmax, rank == 0);
+                const int cpr = st.K / 16, npad = (8 * mts - st.M) * cpr;      // padding rows are zero fragments
+                for (int idx = tid; idx < npad; idx += PG_CONSUMERS) {
+                    const int j = (int)__umulhi((uint32_t)idx, st.inv_cpr), c = idx - j * cpr, row = st.M + j;
+                    sts128(xq_s + (uint32_t)((((c >> 2) * mts + (row >> 3)) * 32 + (row & 7) * 4 + (c & 3)) * 16), make_uint4(0, 0, 0, 0));
+                }
+                if (!go_sent) {
+                    if (tid == 0) mbar_arrive(bar_go);
+                    go_sent = true;
+                }
             }
-            TRACE();
+            if (tid >= 32 && tid < 32 + st.n_lin) s_beta[tid - 32] = beta_r;
+#ifdef VLA_PROG_STAMPS
+            if ((tid & 31) == 0 && P.stamps) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.stamps[(148 + blockIdx.x) * 32 + (tid >> 5)] = t_; }
+#endif
+            consumer_bar();                                  // fragments and scales are complete
+            if (tid < 16) s_rowmax[tid] = 0u;                // (the next stage's atomics come after its own barriers)
+            PG_STAMPP(3, p);
+            const bool teams = prog_team_mode(st.granules, count);
+            if (MAXMT == 1 || st.M <= 8) {
+                if (teams) stage_gemm_teams<1>(lins, st, rank, count, tid, R, red, xq_s, s_beta, s_scale, seq, gcount);
+                else stage_gemm<1>(lins, st, rank, count, tid, R, red, xq_s, s_beta, s_scale, seq, gcount);
+            } else {
+                if (teams) stage_gemm_teams<MAXMT>(lins, st, rank, count, tid, R, red, xq_s, s_beta, s_scale, seq, gcount);
+                else stage_gemm<MAXMT>(lins, st, rank, count, tid, R, red, xq_s, s_beta, s_scale, seq, gcount);
+            }
+            consumer_bar();                                  // everybody is done with xq_s / s_beta / s_scale of this stage
+            PG_STAMPP(4, p);
         }
         if (info & INFO_PUBLISH) {                           // end of a phase that a later phase reads from
             consumer_bar();                                  // every output store of this CTA precedes the release
-            if (tid == 0) red_release_gpu(P.bp + stages[s].phase, 1u);
-            TRACE();
+            if (tid == 0) red_release_gpu(P.bp + p, 1u);
+            PG_STAMPP(5, p);
         }
     }
-    PDLT(3);
-    // the last CTA to finish re-zeroes the counters, so the next launch of the same program needs no memset
-    if (tid == 0) {
+    if (!go_sent && tid == 0) mbar_arrive(bar_go);           // (a CTA without a stage: its producer has nothing to copy)
+    PG_STAMP(5);
+    // Programs with counters (phases, cooperative stages): the last CTA past its last counter access re-zeroes them, so the
+    // next launch needs no memset.  In a single-phase program that access is the CTA's spin on its stage's row count (its
+    // own rows were released before): it counted itself there, and the atomic's round trip overlapped the GEMM.
+    if ((P.n_phases > 1 || P.n_coop > 0) && tid == 0) {
         const unsigned prev = (done_prev != 0xFFFFFFFFu) ? done_prev : atomicAdd(P.done, 1u);
         if (prev == (unsigned)G - 1u) {                      // every CTA is past its last counter access
-            for (int s = 0; s < P.n_stages; ++s) P.b2[s] = 0u;
-            for (int q = 0; q < P.n_phases; ++q) P.bp[q] = 0u;
+            for (int q = 0; q < P.n_stages; ++q) { P.bp[q] = 0u; P.cnt[q] = 0u; }
             *P.done = 0u;                                     // (kernel completion makes these visible to the next launch)
         }
     }
 }
 
-size_t program_desc_capacity() { return PG_DESC_BYTES; }
+int program_threads() { return PG_THREADS; }
+
+cudaError_t program_max_ctas_per_sm(int max_m, int smem_bytes, int* out) {
+    cudaError_t e = cudaFuncSetAttribute(max_m <= 8 ? (const void*)program_kernel<1> : (const void*)program_kernel<2>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes + 128);
+    if (e != cudaSuccess) return e;
+    if (max_m <= 8) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, program_kernel<1>, PG_THREADS, (size_t)smem_bytes + 128);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, program_kernel<2>, PG_THREADS, (size_t)smem_bytes + 128);
+}
 
 cudaError_t launch_program(const DevProg& prog, int grid, int max_m, cudaStream_t s) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(program_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg_smem(1));
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(program_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, pg_smem(2));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // the attribute is per device and cheap to set: no process-wide cache (a process may drive several devices)
+    cudaError_t e = cudaFuncSetAttribute(max_m <= 8 ? (const void*)program_kernel<1> : (const void*)program_kernel<2>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, prog.smem_bytes + 128);
+    if (e != cudaSuccess) return e;
     count_launch();
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(PG_THREADS);
-    cfg.dynamicSmemBytes = (size_t)pg_smem(max_m <= 8 ? 1 : 2);
+    cfg.dynamicSmemBytes = (size_t)prog.smem_bytes + 128;
     cfg.stream = s;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-#ifdef VLA_PROG_TRACE
-    static unsigned trace_launch = 0;
-    DevProg h = prog;
-    h.magic = trace_launch++;
-    if (max_m <= 8) return cudaLaunchKernelEx(&cfg, program_kernel<1>, h);
-    return cudaLaunchKernelEx(&cfg, program_kernel<2>, h);
-#else
     if (max_m <= 8) return cudaLaunchKernelEx(&cfg, program_kernel<1>, prog);
     return cudaLaunchKernelEx(&cfg, program_kernel<2>, prog);
-#endif
 }
-
-#ifdef VLA_PROG_TRACE
-extern "C" int vla_debug_read_trace(unsigned long long* host, size_t n) {
-    return (int)cudaMemcpyFromSymbol(host, g_trace, n * sizeof(unsigned long long));
-}
-extern "C" int vla_debug_read_pdl(unsigned long long* host, size_t n) {
-    return (int)cudaMemcpyFromSymbol(host, g_pdl, n * sizeof(unsigned long long));
-}
-#endif
 
 }  // namespace vla

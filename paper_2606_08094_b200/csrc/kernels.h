@@ -33,7 +33,7 @@ cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const in
 // persistent program kernel (gemm_program.cu); the program header travels as a kernel parameter
 struct DevProg;
 cudaError_t launch_program(const DevProg& prog, int grid, int max_m, cudaStream_t s);
-size_t program_desc_capacity();      // bytes of stage + linear descriptors a program may hold
+cudaError_t program_max_ctas_per_sm(int max_m, int smem_bytes, int* out);      // co-residency of the persistent grid
 cudaError_t run_i8_mma_probe(int ctas, int mmas_per_cta, float* ms_out);
 
 }  // namespace vla
