@@ -19,13 +19,14 @@ def stage(M=8, K=2560, N=2560, depends=0, n=1, dtype=1):
 
 def test_program_bytes_counts_tables_counters_and_cooperative_scratch(vla):
     """the device buffer holds the descriptor tables, the counters and, for stages quantised cooperatively (more than
-    960 sixteen-element tasks), the int8 fragments + alpha; small stages are quantised in shared memory and add nothing"""
+    1440 sixteen-element tasks), the int8 fragments + alpha; small stages are quantised in shared memory and add nothing"""
     small = vla.vla_program_bytes([stage(M=1)])                      # 160 tasks: local
     assert small % 256 == 0 and 512 <= small < 4096
-    one = vla.vla_program_bytes([stage()])                           # M=8, K=2560: cooperative, 8*2560 B of fragments
-    assert small + 8 * 2560 <= one < small + 8 * 2560 + 1024
-    two = vla.vla_program_bytes([stage(), stage(M=16, K=6912, depends=1)])
-    assert one + 16 * 6912 <= two < one + 16 * 6912 + 1024
+    assert vla.vla_program_bytes([stage()]) == small                 # M=8, K=2560: 1280 tasks, still local
+    one = vla.vla_program_bytes([stage(M=16)])                       # 2560 tasks: cooperative, 16*2560 B of fragments
+    assert small + 16 * 2560 <= one < small + 16 * 2560 + 1024
+    two = vla.vla_program_bytes([stage(M=16), stage(M=8, K=6912, depends=1)])
+    assert one + 8 * 6912 <= two < one + 8 * 6912 + 1024
 
 
 @pytest.mark.parametrize("bad", [dict(M=0), dict(M=17), dict(K=100), dict(K=8192 + 128), dict(N=100), dict(N=0),
