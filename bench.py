@@ -31,6 +31,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+METRIC = "ternary GEMM TOPS & HBM GB/s vs M; fraction of INT8/HBM roofline (1 B200)"      # BASELINE.json:metric
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
 NOMINAL_HBM_GBS = 8000.0           # BASELINE.json north_star "~8 TB/s"
 NOMINAL_INT8_TOPS = 4500.0         # dense int8, datasheet (same rate as fp8)
@@ -189,7 +190,7 @@ def run_reference(args):
     val = nbytes / sec / 1e9
     sample = "all 12 points, all rows" if cap is None else "first %d rows of each of the 4 points" % cap
     line = {
-        "impl": "reference", "metric": "ternary_linear_algorithmic_hbm_gbs", "value": val, "unit": "GB/s",
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s",
         "n_gpus": args.gpus, "steps": done, "warmup": min(args.warmup, 1), "ms_per_step": sec / done * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8*ternary->int32",
         "data": "synthetic", "tops": nops / sec / 1e12,
@@ -471,6 +472,14 @@ def run_gpu(args):
                           "route": "single vla_ternary_linear call (quant kernel + GEMM kernel)"})
             del g
 
+    # ---- the metric is "vs M": both halves (HBM-bound M <= 16, tensor-bound M >= 512) in the same line
+    vs_m, roof_tensor = None, None
+    if args.workload == "decode" and not args.no_vs_m:
+        import bench_workloads as bw
+        vs_m, roof_tensor = bw.run_vs_m(pk, int8_probe_tops(vla))
+        if roof_tensor is not None:
+            roof_tensor["traffic"] = ncu_traffic("gemm_large")
+
     # ---- the oracle on this box's host cores, bounded sample
     from oracle import oracle as orc
     orc.build()
@@ -485,18 +494,21 @@ def run_gpu(args):
 
     value = total_bytes / (ms * 1e-3) / 1e9
     line = {
-        "metric": "ternary_linear_algorithmic_hbm_gbs", "value": value, "unit": "GB/s", "n_gpus": world,
+        "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int8*ternary->int32", "data": "synthetic",
         "tops": total_ops / (ms * 1e-3) / 1e12,
         "config": {"workload": workload_name(args.workload),
                    "cold_weights": "ring of %d packed copies per shape (%.0f MB > 2 x L2 %.0f MB), next slot every use"
                    % (wl.copies, wl.copies * sum(r.shape[1] for r in wl.ring) / 1e6, wl.l2 / 1e6),
+                   "value_is": ("algorithmic HBM GB/s of the configs[1] decode step (the M <= 16 half of the metric); both halves "
+                                "per (shape, M) are in vs_M, the dominant kernel of the M >= 512 half in roofline_tensor")
+                   if args.workload == "decode" else "algorithmic HBM GB/s of the configs[2] prefill step; TOPS beside it",
                    "launch": ("CUDA graphs of %d program launches" if args.workload == "decode" else "CUDA graphs of %d steps + PDL") % rev, "parallelism": "replicas" if world > 1 else "single"},
         "clocks": clocks, "gpu_launches": launches,
         "e2e": {"value": e2e_bytes / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": wl.h2d,
                 "d2h_bytes_per_step": wl.d2h, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
-        "roofline": roof, "cpu_baseline": cpu, "points": table,
+        "roofline": roof, "roofline_tensor": roof_tensor, "cpu_baseline": cpu, "points": table, "vs_M": vs_m,
         "step_roofline_frac_hbm": value / pk["hbm_gbs"],
     }
     print(json.dumps(line))
@@ -540,6 +552,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle timing for cpu_baseline")
     ap.add_argument("--no-points", action="store_true", help="skip the per-point table")
+    ap.add_argument("--no-vs-m", action="store_true", help="skip the vs-M block (both halves of the metric)")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.workload in ("stack", "sweep"):

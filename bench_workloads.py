@@ -249,3 +249,99 @@ def run_sweep(args, pk, clock_sampler, int8_probe_tops):
     }
     print(json.dumps(line))
     return 0
+
+
+# ----------------------------------------------------------------------------- the metric "vs M" (default bench.py line)
+VS_M_SHAPES = [(2560, 2560), (2560, 640), (2560, 6912), (6912, 2560), (8192, 8192)]
+VS_M_M = [1, 8, 16, 64, 512, 544, 1024, 4096]
+
+
+def run_vs_m(pk, int8_probe_tops, Ms=None, shapes=None):
+    """BASELINE.json's metric is "TOPS & HBM GB/s vs M; fraction of INT8/HBM roofline": the four model shapes and 8192^2
+    at M in {1, 8, 16, 64, 512, 544, 1024, 4096}, fused quant (vla_ternary_linear, VLA_PATH_AUTO, fp32 out), every call
+    of a CUDA graph on its own packed-weight copy of a ring larger than 2 x L2 (cold weights); for M <= 16 also the program
+    route (the ring as independent stages of persistent launches).  Returns (points, roofline_tensor) where
+    roofline_tensor is the record of the dominant kernel of the M >= 512 half (gemm_large_kernel, timed alone on
+    pre-quantised activations at the four model shapes, M = 544)."""
+    import torch
+    from paper_2606_08094_b200 import binding as vla, synth
+    dev = torch.device("cuda", torch.cuda.current_device())
+    l2 = torch.cuda.get_device_properties(dev).L2_cache_size
+    peak_i8 = pk["bf16_tflops"] * 2.0
+    Ms = Ms or VS_M_M
+    shapes = shapes or VS_M_SHAPES
+    pts = []
+    gemm_only = []
+    for si, (K, N) in enumerate(shapes):
+        copies = min(700, max(2, -(-2 * l2 // (N * K // 4))))
+        w = synth.ternary_weights(N, K, 0.35, 4100 + si)
+        packed1 = vla.pack_weights(torch.from_numpy(w).to(dev))
+        ring = packed1.unsqueeze(0).repeat(copies, 1).contiguous()
+        del w, packed1
+        beta = torch.tensor([0.05], dtype=torch.float32, device=dev)
+        Mmax = max(Ms)
+        xb = synth.activations(Mmax, K, 504500 + si)
+        x_all = torch.from_numpy(xb.view(np.int16)).to(dev).view(torch.bfloat16)
+        for M in Ms:
+            x = x_all[:M].contiguous()
+            out = torch.empty((M, N), dtype=torch.float32, device=dev)
+            xq = torch.empty((M, K), dtype=torch.int8, device=dev)
+            xs = torch.empty((M,), dtype=torch.float32, device=dev)
+            ncall = copies if M <= 1024 else min(copies, 16)      # (large M: the activations alone exceed L2)
+
+            def calls():
+                for c in range(ncall):
+                    vla.vla_ternary_linear(ring[c], beta, x, M, N, K, out, vla.VLA_F32, vla.VLA_PATH_AUTO, xq, xs, None, 0)
+            calls()
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                calls()
+            sec = _time(torch, g.replay, 3) / ncall
+            by = N * K // 4 + 4 + 2 * M * K + 4 * M * N
+            op = 2.0 * M * N * K
+            t_mem, t_cmp = by / (pk["hbm_gbs"] * 1e9), op / (peak_i8 * 1e12)
+            p = {"M": M, "K": K, "N": N, "us": sec * 1e6, "TOPS": op / sec / 1e12, "GBs": by / sec / 1e9,
+                 "roofline_frac": max(t_mem, t_cmp) / sec, "bound": "hbm" if t_mem > t_cmp else "tensor",
+                 "path": int(vla.vla_ternary_auto_path(M, N, K)), "route": "single vla_ternary_linear call"}
+            if p["bound"] == "tensor":
+                p["frac_of_probe"] = (op / (int8_probe_tops * 1e12)) / sec
+            del g
+            if M <= 16:
+                nst = min(copies, 128)
+                outs = [torch.empty((M, N), dtype=torch.float32, device=dev) for _ in range(nst)]
+                stages = [dict(x=x, M=M, K=K, depends=0,
+                               linears=[dict(packed=ring[c], w_scale=beta, out=outs[c], N=N, out_dtype=vla.VLA_F32)])
+                          for c in range(nst)]
+                prog = vla.compile_program(stages, dev)
+                secp = _time(torch, lambda: vla.vla_program_run(prog), 5) / nst
+                p["program_us"] = secp * 1e6
+                p["program_GBs"] = by / secp / 1e9
+                p["program_roofline_frac"] = t_mem / secp
+                vla.vla_program_release(prog)
+                del prog, outs
+            if M == synth.PREFILL_M and (K, N) in synth.MODEL_SHAPES:
+                def gcalls():
+                    for c in range(ncall):
+                        vla.vla_ternary_gemm(ring[c], beta, xq, xs, M, N, K, out, vla.VLA_F32, vla.VLA_PATH_AUTO, None, 0)
+                gcalls()
+                torch.cuda.synchronize()
+                gg = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gg):
+                    gcalls()
+                gemm_only.append((op, _time(torch, gg.replay, 3) / ncall))
+                del gg
+            pts.append(p)
+        del ring, x_all
+        torch.cuda.empty_cache()
+    roof_t = None
+    if gemm_only:
+        ops = sum(o for o, _ in gemm_only) / len(gemm_only)
+        sec = sum(s for _, s in gemm_only) / len(gemm_only)
+        ach = ops / sec / 1e12
+        roof_t = {"bound": "tensor", "achieved": ach, "peak": peak_i8, "unit": "TOP/s", "frac": ach / peak_i8,
+                  "kernel": "gemm_large_kernel", "alg_ops_per_launch": ops, "us_per_launch": sec * 1e6,
+                  "workload": "the four model shapes at M=544, pre-quantised activations, cold weights",
+                  "peak_source": "MEASURED_PEAKS.json bf16_tflops x 2 (int8:bf16 nominal ratio)",
+                  "int8_probe_tops": int8_probe_tops, "frac_of_probe": ach / int8_probe_tops}
+    return pts, roof_t

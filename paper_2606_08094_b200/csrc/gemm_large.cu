@@ -97,6 +97,10 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    // Let the next kernel on the stream be scheduled NOW: its CTAs take an SM as soon as one of ours exits and run their
+    // prologue (weight prefetch, decode of the first stages) under our tail; its own griddepcontrol.wait still waits for
+    // this whole grid and its memory.
+    pdl_launch_dependents();
 
     if (warp == 0) {
         // ---------------- W producer ----------------
@@ -283,7 +287,6 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
             if (threadIdx.x == 11 * 32) LG_STAMP(3, 2 * ti + 1);
         }
     }
-    pdl_launch_dependents();
     tc_fence_before();
     __syncthreads();
     if (warp == 2) tmem_dealloc(tmem_base, 512u);

@@ -101,12 +101,27 @@ __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uin
 }
 
 // ---------------------------------------------------------------- ring bookkeeping
-// chunk number `seq` of this CTA (in producer order) lives in slot seq % nslot, in ring round seq / nslot
-struct Ring { uint32_t base, slot_bytes, nslot, bar_full, bar_empty; };
+// Chunk number `seq` of this CTA (in producer order, over all its stages) lives in slot seq % nslot, in ring round
+// seq / nslot.  An mbarrier only tells the PARITY of a phase, so a consumer may wait for round r of a slot only once
+// round r-1 of that slot has landed; teams skip over each other's chunks and could otherwise be two rounds ahead of a
+// slot.  s_got[slot] = seq + 1 of the newest chunk of the slot whose arrival a consumer has seen: the consumer of chunk
+// seq first waits for s_got[slot] >= seq + 1 - nslot, then on the mbarrier.
+struct Ring { uint32_t base, slot_bytes, nslot, bar_full, bar_empty, got; };
 struct RingPos { uint32_t slot, parity; };
 __device__ __forceinline__ RingPos ring_pos(uint32_t seq, uint32_t nslot) {
     const uint32_t round = seq / nslot;
     return RingPos{seq - round * nslot, round & 1u};
+}
+__device__ __forceinline__ RingPos ring_wait(const Ring& R, uint32_t seq, int lane) {
+    const RingPos rp = ring_pos(seq, R.nslot);
+    const uint32_t got = R.got + 4u * rp.slot;
+    if (seq >= R.nslot) {
+        uint32_t v;
+        do { asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(got) : "memory"); } while (v + R.nslot < seq + 1u);
+    }
+    mbar_wait(R.bar_full + 8u * rp.slot, rp.parity);
+    if (lane == 0) asm volatile("st.volatile.shared.u32 [%0], %1;" :: "r"(got), "r"(seq + 1u) : "memory");
+    return rp;
 }
 
 // ---------------------------------------------------------------- producer warp
@@ -130,7 +145,7 @@ __device__ __forceinline__ void producer(const DevProg& P, const DevStage* stage
                 const int np = min(cp, KB - p0);
                 if (P.gate && seq == 1) mbar_wait(bar_go, 0);
                 const RingPos rp = ring_pos(seq, R.nslot);
-                if (seq >= R.nslot) mbar_wait(R.bar_empty + 8u * rp.slot, rp.parity ^ 1u);
+                if (seq >= R.nslot) mbar_wait(R.bar_empty + 8u * rp.slot, rp.parity ^ 1u);      // (every round in turn)
                 if (lane == 0) {                              // one bulk copy of up to 30 KiB per chunk
                     mbar_arrive_expect_tx(R.bar_full + 8u * rp.slot, (uint32_t)np * 1024u);
                     tma_bulk_g2s(R.base + rp.slot * R.slot_bytes, src + (size_t)p0 * 1024, (uint32_t)np * 1024u,
@@ -389,8 +404,7 @@ __device__ __forceinline__ void stage_gemm(const DevLin* lins, const DevStage& s
         zero_acc<MT>(acc, acc2);
         for (int p0 = 0; p0 < KB; p0 += cp, ++seq) {
             const int np = min(cp, KB - p0);
-            const RingPos rp = ring_pos(seq, R.nslot);
-            mbar_wait(R.bar_full + 8u * rp.slot, rp.parity);
+            const RingPos rp = ring_wait(R, seq, lane);
             chunk_mma<MT, PG_W, 2, 1>(R.base + rp.slot * R.slot_bytes, R.bar_empty + 8u * rp.slot, xq_s, w, 2 * np, 2 * p0,
                                       lane, acc, acc2);       // 15 arrivals (one per warp) hand the slot back
         }
@@ -426,11 +440,10 @@ __device__ __forceinline__ void stage_gemm_teams(const DevLin* lins, const DevSt
         const float beta = s_beta[l - st.lin_begin];
         int acc[2][MT][4], acc2[2][4];
         zero_acc<MT>(acc, acc2);
-        uint32_t cs = seq + (uint32_t)(n * nch);
+        uint32_t cs = seq + (uint32_t)(n * nch);             // ring chunks n * nch .. of this stage
         for (int p0 = 0; p0 < KB; p0 += cp, ++cs) {
             const int np = min(cp, KB - p0);
-            const RingPos rp = ring_pos(cs, R.nslot);
-            mbar_wait(R.bar_full + 8u * rp.slot, rp.parity);
+            const RingPos rp = ring_wait(R, cs, lane);
             chunk_mma<MT, PG_TW, 3, PG_TEAMS>(R.base + rp.slot * R.slot_bytes, R.bar_empty + 8u * rp.slot, xq_s, j, 2 * np,
                                               2 * p0, lane, acc, acc2);       // (the empty barrier counts 15: three arrivals per team warp)
         }
@@ -475,6 +488,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         fence_barrier_init();
         s_misc[0] = 0u;
         s_misc[1] = 0u;
+        for (int sl = 0; sl < PG_NSLOT_MAX; ++sl) reinterpret_cast<volatile unsigned*>(base_ptr + PG_OFF_GOT)[sl] = 0u;
     }
     if (tid < 16) s_rowmax[tid] = 0u;
     for (int i = tid; i < P.n_phases; i += PG_THREADS) s_info[i] = 0u;
@@ -511,6 +525,7 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
     R.nslot = min((uint32_t)PG_NSLOT_MAX, (base + (uint32_t)P.smem_bytes - R.base) / R.slot_bytes);
     R.bar_full = bar_full;
     R.bar_empty = bar_empty;
+    R.got = base + PG_OFF_GOT;
 
     if (tid >= PG_CONSUMERS) {
         // Weights never depend on the previous kernel on the stream: the ring starts filling under its tail.

@@ -56,8 +56,11 @@ struct DevProg {
     const DevLin* lins;
 };
 
+#ifndef VLA_PG_SLOT_PIECES
+#define VLA_PG_SLOT_PIECES 30
+#endif
 // ---- shared-memory map of program_kernel (one definition for the kernel and the host-side sizing)
-constexpr int PG_SLOT_PIECES = 30;                    // most 1 KiB pieces (32 channels x 128 k) per ring chunk
+constexpr int PG_SLOT_PIECES = VLA_PG_SLOT_PIECES;                    // most 1 KiB pieces (32 channels x 128 k) per ring chunk
 constexpr int PG_NSLOT_MAX = 12;
 constexpr int PG_NSLOT_MIN = 2;
 #ifndef VLA_PG_TEAMS
@@ -77,7 +80,8 @@ constexpr int PG_OFF_ALPHA = 208;                     // float4[16]: alpha_m, 1/
 constexpr int PG_OFF_BETA = 464;                      // float[16]
 constexpr int PG_OFF_ROWMAX = 528;                    // unsigned[16]
 constexpr int PG_OFF_MISC = 592;                      // unsigned[4]
-constexpr int PG_OFF_RED = 640;
+constexpr int PG_OFF_GOT = 608;                       // unsigned[12]: newest chunk seen to have landed, per ring slot
+constexpr int PG_OFF_RED = 704;
 constexpr int PG_OFF_INFO = PG_OFF_RED + PG_RED_INTS * 4;
 constexpr int PG_SMEM_LIMIT = 232448 - 128;           // 227 KB minus the alignment slack
 

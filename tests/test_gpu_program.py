@@ -164,6 +164,34 @@ def test_chained_stack_free_running(vla, oracle, M):
             assert np.array_equal(bits(st2.out[l][n]), ref[l][n]), "per-call route: layer %d %s differs" % (l, n)
 
 
+@pytest.mark.parametrize("M,K,N,nst", [(16, 8192, 2048, 16), (8, 6912, 1024, 16), (16, 6912, 2048, 16), (5, 8192, 1536, 12)])
+def test_team_mode_with_multi_chunk_granules(vla, oracle, M, K, N, nst):
+    """Granules longer than one ring slot (K = 6912: two chunks, K = 8192: three) in TEAM mode with as few as three ring
+    slots (M = 16 leaves the ring what 16*K bytes of activations do not take): `nst` independent stages share one
+    weight tensor and one activation matrix, so every group is ~9 CTAs with >= 3 granules each, and every team runs
+    several granules through its own slots.  (A team that waited two mbarrier phases ahead of a slot read stale chunks.)"""
+    w = synth.ternary_weights(N, K, 0.35, 4242 + K + N)
+    x_bits = synth.activations(M, K, 4243, outlier_frac=0.01)
+    beta = synth.weight_scale(4244)
+    packed = vla.pack_weights(dev(w))
+    beta_d = dev(np.array([beta], np.float32))
+    x = dev_bf16(x_bits)
+    outs = [torch.full((M, N), -7, dtype=torch.int32 if c % 2 else torch.bfloat16, device="cuda") for c in range(nst)]
+    stages = [dict(x=x, M=M, K=K, depends=0,
+                   linears=[dict(packed=packed, w_scale=beta_d, out=outs[c], N=N, out_dtype=2 if c % 2 else 1)]) for c in range(nst)]
+    prog = vla.compile_program(stages)
+    ref = oracle.ternary_linear(x_bits, w, beta)
+    for rep in range(2):
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        for c in range(nst):
+            if c % 2:
+                assert np.array_equal(outs[c].cpu().numpy(), ref["acc"]), "stage %d int32 (rep %d)" % (c, rep)
+            else:
+                assert np.array_equal(bits(outs[c]), ref["ybf16"]), "stage %d bf16 (rep %d)" % (c, rep)
+    vla.vla_program_release(prog)
+
+
 def test_program_errors(vla):
     p = make_point(vla, 8, 256, 256, 5, vla.VLA_BF16)
     bad_m = dict(stage_of(p), M=17)
