@@ -17,7 +17,9 @@
  *    and capturable in a CUDA graph, except vla_ternary_pack, which synchronises the stream.
  *  - Layouts: W logical [N,K] (row n = output channel, K contiguous); X [M,K] row-major;
  *    Y [M,N] row-major.
- *  - Shapes: M >= 1; K % 128 == 0; N % 128 == 0; K <= 65536 (else VLA_ERR_SHAPE).
+ *  - Shapes: M >= 1; K % 128 == 0; N % 128 == 0; K <= 65536 (else VLA_ERR_SHAPE; the decode scales the weights by 64,
+ *    and 64 * 127 * K < 2^31 holds up to K = 264 000).
+ *  - One device per call: every call works on the CURRENT device (cudaSetDevice); nothing is cached across devices.
  *  - Every pointer must be 16-byte aligned (VLA_ERR_ALIGN).
  *  - Inputs must be finite; NaN/Inf are not checked (result unspecified, memory-safe).
  *  - Arguments are validated on the host before any launch.  A non-zero status leaves the
@@ -54,8 +56,8 @@ typedef enum {
 
 typedef enum {
     VLA_PATH_AUTO = 0,      /* library chooses by M, and by (N,K) for 16 < M <= 32 (table in DESIGN.md 6d, measured) */
-    VLA_PATH_SMALL_ALU = 1, /* in-register decode + dp4a on the integer ALUs; M <= 16 */
-    VLA_PATH_SMALL_TC = 2,  /* in-register decode + warp-level int8 MMA; M <= 64 */
+    VLA_PATH_SMALL_ALU = 1, /* in-register decode + dp4a on the integer ALUs; M <= 16 (M = 17: VLA_ERR_SHAPE) */
+    VLA_PATH_SMALL_TC = 2,  /* in-register decode + warp-level int8 MMA; M <= 32 (M = 33: VLA_ERR_SHAPE) */
     VLA_PATH_LARGE = 3      /* TMA -> decode warps -> tcgen05.mma kind::i8 -> TMEM; any M */
 } vla_path;
 
@@ -72,7 +74,7 @@ size_t vla_ternary_workspace_bytes(int M, int N, int K, vla_path path);
  *   packed       packed_bytes >= vla_ternary_packed_bytes(N,K); layout is private to the library
  *                (tile-permuted 2-bit two's-complement codes), defined only by pack/unpack
  * SYNCHRONISES `stream`.  Returns VLA_ERR_VALUE if any element is outside {-1,0,+1}
- * (packed is then unspecified). */
+ * (packed is then unspecified), VLA_ERR_WORKSPACE if packed_bytes is too small. */
 vla_status vla_ternary_pack(const int8_t* w, int N, int K, void* packed, size_t packed_bytes, void* stream);
 
 /* Inverse of vla_ternary_pack: w[N,K] int8.  unpack(pack(W)) == W. */
@@ -128,7 +130,9 @@ vla_status vla_ternary_linear_host(const void* packed, const float* w_scale, con
  * A STAGE is one activation matrix x [M,K] bf16 (1 <= M <= 16, K % 128 == 0, K <= 8192) and n_linears
  * (1..16) ternary linears that all consume it, each with its own packed W [N,K], scale beta and output:
  * the per-output-group scales beta_g(n) of Eq. 4, e.g. q|k|v or gate|up.
- * Every stage runs Eq. 4 end to end: absmax int8 quant of x, int32 contraction, dequant to out_dtype.
+ * Every stage runs Eq. 4 end to end inside the one kernel: absmax int8 quant of x (fused: small stages are quantised by
+ * every CTA of the stage straight into shared memory, larger ones once per row and shared through the program buffer),
+ * int32 contraction, dequant to out_dtype.
  *   depends = 0   x does not depend on the stages since the last depends = 1 stage: the stage joins the
  *                 current PHASE, whose stages run concurrently on disjoint groups of SMs
  *   depends = 1   x is (part of) the output of EARLIER stages of this program: the stage opens a new
@@ -172,7 +176,12 @@ vla_status vla_program_build(const vla_prog_stage* stages /*host*/, int n_stages
 
 /* Runs a compiled program: ONE kernel launch, asynchronous on `stream`, capturable in a CUDA graph.
  * Returns VLA_ERR_VALUE if prog_dev was not produced by vla_program_build in this process.
- * Runs of the same program must not overlap in time (they share its counters and activations). */
+ * Runs of the same program must not overlap in time (they share its counters and activation scratch).
+ * The kernel is persistent (one CTA per SM) and, for programs with more than one phase or with cooperatively quantised
+ * stages, its CTAs wait for each other: vla_program_build sizes the grid so that all of them are resident on an
+ * otherwise idle device.  Do not run another persistent or SM-filling kernel concurrently with such a program (another
+ * stream, MPS, a green context with fewer SMs): a CTA that never becomes resident makes the others wait until the
+ * kernel's watchdog (~2 s of spinning) traps, which surfaces as VLA_ERR_CUDA on the next call, not as a hang. */
 vla_status vla_program_run(const void* prog_dev, void* stream);
 
 /* Host-buffer form of vla_program_run (the end-to-end call of a serving process): copies every `in` entry
@@ -193,15 +202,19 @@ vla_status vla_program_release(const void* prog_dev);
 /* The path VLA_PATH_AUTO resolves to for (M,N,K). */
 vla_path vla_ternary_auto_path(int M, int N, int K);
 
-/* Measurement aid (not on the hot path): issue `mmas_per_cta` back-to-back
+const char* vla_status_string(vla_status s);
+
+/* ---------------------------------------------------------------------------------------------------
+ * Instrumentation (benchmarks only; nothing below is on the hot path or needed to use the library).
+ * --------------------------------------------------------------------------------------------------- */
+
+/* Issue `mmas_per_cta` back-to-back
  * tcgen05.mma.cta_group::1.kind::i8 (M=128, N=256, K=32) per CTA on `ctas` CTAs with no loads,
  * and return the elapsed milliseconds through the HOST pointer ms_out.  Gives the box's INT8
  * tensor-pipe ceiling: ops = 2*128*256*32 * mmas_per_cta * ctas.  Synchronises the device. */
 vla_status vla_i8_mma_issue_probe(int ctas, int mmas_per_cta, float* ms_out /*host*/);
 
-const char* vla_status_string(vla_status s);
-
-/* Number of kernels this library has launched so far in this process (instrumentation for benchmarks). */
+/* Number of kernels this library has launched so far in this process. */
 unsigned long long vla_launch_count(void);
 
 #ifdef __cplusplus

@@ -53,8 +53,9 @@ class VlaError(RuntimeError):
 
 def _load():
     so = _build.SO
-    if not os.path.exists(so):
-        _build.build()          # needs nvcc; raises if the toolchain is missing -- no fallback
+    if not _build.is_current():
+        _build.build()          # missing, or built from other sources (a stale binary must never be loaded silently);
+                                # needs nvcc and raises if the toolchain is missing -- no fallback
     lib = ctypes.CDLL(so)
     vp, i, sz, st = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_int
     lib.vla_ternary_packed_bytes.restype = sz

@@ -2,6 +2,7 @@
 
     python -m paper_2606_08094_b200.build [--force] [--verbose]
 """
+import hashlib
 import os
 import subprocess
 import sys
@@ -14,14 +15,26 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--threads", "0"]
 
 
-def _newest_source_mtime():
-    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+STAMP = SO + ".srchash"
+
+
+def source_hash():
+    """sha256 over csrc/ and the public header: what the .so was built from (mtimes do not survive a copy)."""
+    paths = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC))
     paths.append(os.path.join(os.path.dirname(HERE), "include", "vla_ternary.h"))
-    return max(os.path.getmtime(p) for p in paths)
+    h = hashlib.sha256()
+    for p in paths:
+        h.update(os.path.basename(p).encode())
+        h.update(open(p, "rb").read())
+    return h.hexdigest()
+
+
+def is_current():
+    return os.path.exists(SO) and os.path.exists(STAMP) and open(STAMP).read().strip() == source_hash()
 
 
 def build(force=False, verbose=False):
-    if not force and os.path.exists(SO) and os.path.getmtime(SO) >= _newest_source_mtime():
+    if not force and is_current():
         return SO
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = SO + ".tmp%d" % os.getpid()
@@ -29,6 +42,8 @@ def build(force=False, verbose=False):
            *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
     subprocess.run(cmd, check=True)
     os.replace(tmp, SO)
+    with open(STAMP, "w") as f:
+        f.write(source_hash() + "\n")
     return SO
 
 

@@ -19,20 +19,13 @@ inline bool shape_ok(int N, int K) { return N >= 128 && K >= 128 && N % 128 == 0
 
 inline size_t round256(size_t b) { return (b + 255) / 256 * 256; }
 
-vla_status check_arch() {
-    static int cached_dev = -1;
-    static vla_status cached = VLA_ERR_ARCH;
-    int dev = -1;
-    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_ARCH; }
-    if (dev == cached_dev) return cached;
-    int major = 0;
-    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+vla_status check_arch() {                                  // per call: two cheap attribute queries, no cache to race on
+    int dev = -1, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
         cudaGetLastError();
         return VLA_ERR_ARCH;
     }
-    cached_dev = dev;
-    cached = (major == 10) ? VLA_OK : VLA_ERR_ARCH;
-    return cached;
+    return (major == 10) ? VLA_OK : VLA_ERR_ARCH;
 }
 
 inline vla_status from_cuda(cudaError_t e) {
@@ -72,7 +65,7 @@ const char* vla_status_string(vla_status s) {
     switch (s) {
         case VLA_OK: return "VLA_OK";
         case VLA_ERR_NULL: return "VLA_ERR_NULL: a required pointer is NULL";
-        case VLA_ERR_SHAPE: return "VLA_ERR_SHAPE: need M>=1, N%128==0, K%128==0, K<=65536, and M within the forced path's range";
+        case VLA_ERR_SHAPE: return "VLA_ERR_SHAPE: need M>=1, N%128==0, K%128==0, K<=65536; a forced path takes M<=16 (SMALL_ALU), M<=32 (SMALL_TC), any M (LARGE)";
         case VLA_ERR_ALIGN: return "VLA_ERR_ALIGN: pointers must be 16-byte aligned";
         case VLA_ERR_VALUE: return "VLA_ERR_VALUE: weight element outside {-1,0,+1}, or not a compiled program";
         case VLA_ERR_DTYPE: return "VLA_ERR_DTYPE: unknown vla_dtype or vla_path";
@@ -102,7 +95,7 @@ vla_path vla_ternary_auto_path(int M, int N, int K) {
 vla_status vla_ternary_pack(const int8_t* w, int N, int K, void* packed, size_t packed_bytes, void* stream) {
     if (!w || !packed) return VLA_ERR_NULL;
     if (!shape_ok(N, K)) return VLA_ERR_SHAPE;
-    if (packed_bytes < vla_ternary_packed_bytes(N, K)) return VLA_ERR_SHAPE;
+    if (packed_bytes < vla_ternary_packed_bytes(N, K)) return VLA_ERR_WORKSPACE;       // the documented code for a short buffer
     if (!aligned16(w) || !aligned16(packed)) return VLA_ERR_ALIGN;
     vla_status st = check_arch();
     if (st != VLA_OK) return st;

@@ -17,22 +17,10 @@
 //                tile's main loop through the second TMEM buffer
 #include <cuda.h>
 #include <cuda_bf16.h>
-#include <cstdlib>
 #include "common.cuh"
 #include "kernels.h"
 
 namespace vla {
-
-#ifdef VLA_LG_DEBUG
-// debug-only (never defined in the product build): switch pipeline pieces off to find the per-k-block bottleneck
-__device__ int g_lg_dbg = 0;
-__device__ long long g_lg_trace[4][512];
-#define LG_DBG(bit) (g_lg_dbg & (bit))
-#define LG_STAMP(role, n) do { if (blockIdx.x == 0 && (n) < 512) g_lg_trace[role][(n)] = clock64(); } while (0)
-#else
-#define LG_DBG(bit) 0
-#define LG_STAMP(role, n) do { } while (0)
-#endif
 
 constexpr int LG_THREADS = 15 * 32;
 constexpr int LG_SW = 6;                                // packed-weight stages (4 KiB each)
@@ -154,7 +142,6 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
                     const uint32_t s = it % ns;
                     mbar_wait(bar_full(s), (it / ns) & 1);
                     tc_fence_after();
-                    LG_STAMP(0, it);
 #pragma unroll
                     for (int kk = 0; kk < KS; ++kk) {
                         const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride + kk * LG_A_BYTES);
@@ -188,7 +175,6 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
                     for (int itx = 0; itx < 2; ++itx)
                         wv[kk][itx] = *reinterpret_cast<const uint4*>(wst + kk * LG_W_BYTES + ((i32 * 2 + (p ^ itx)) * 32 + g * 4 + t) * 16);
                 if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
-                if (threadIdx.x == 96) LG_STAMP(1, it);
 #pragma unroll
                 for (int kk = 0; kk < KS; ++kk) {
                     uint8_t* ast = pS + s * stride + kk * LG_A_BYTES;
@@ -210,7 +196,6 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
                     mbar_arrive(bar_empty_w(sw));
                     mbar_arrive(bar_full(s));
                 }
-                if (threadIdx.x == 96) LG_STAMP(2, it);
             }
         }
     } else {
@@ -234,15 +219,12 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
             __syncwarp();
             mbar_wait(bar_acc_full(ab), (ti >> 1) & 1);
             tc_fence_after();
-            if (threadIdx.x == 11 * 32) LG_STAMP(3, 2 * ti);
             const uint32_t t_addr = tmem_base + ab * 256u + ((uint32_t)(lq * 32) << 16);
             for (int c0 = 0; c0 < TN; c0 += 16) {
                 if (m0 + c0 >= M) break;
                 uint32_t r[16];
-                if (threadIdx.x == 11 * 32) LG_STAMP(3, 8 + 2 * (c0 >> 4));
                 tmem_ld_32x32b_x16(t_addr + (uint32_t)c0, r);
                 tmem_ld_wait();
-                if (threadIdx.x == 11 * 32) LG_STAMP(3, 9 + 2 * (c0 >> 4));
                 const int nrow = min(16, M - m0 - c0);
                 float sv[16];                                 // explicit ld.shared: cannot alias the stores below
 #pragma unroll
@@ -284,7 +266,6 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_acc_empty(ab));    // this TMEM buffer may be overwritten
-            if (threadIdx.x == 11 * 32) LG_STAMP(3, 2 * ti + 1);
         }
     }
     tc_fence_before();
@@ -296,16 +277,6 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static int env_ks() {
-    const char* v = std::getenv("VLA_TUNE_KS");                 // tuning aid: force the k blocks per stage (1 or 2)
-    return v ? std::atoi(v) : 0;
-}
-
-static int env_tn() {
-    const char* v = std::getenv("VLA_TUNE_TN");                 // tuning aid: force the token-tile width
-    return v ? std::atoi(v) : 0;
-}
 
 static EncodeTiledFn get_encode() {
     static EncodeTiledFn fn = nullptr;
@@ -345,15 +316,10 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     const int N = g.ct_begin[g.n] * TILE_N;                  // all channels of the group
     EncodeTiledFn enc = get_encode();
     if (!enc) return cudaErrorNotSupported;
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (sms <= 0) sms = 148;
-    }
-    static const int tune_tn = env_tn();
-    const int TN = tune_tn > 0 ? tune_tn : pick_tn(M, N, sms, (K / TILE_K) % 2 == 0);
+    int dev = 0, sms = 0;                                    // per call: a process may drive several devices
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+        return cudaErrorInvalidDevice;
+    const int TN = pick_tn(M, N, sms, (K / TILE_K) % 2 == 0);
 
     CUtensorMap tm;
     cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)M};
@@ -365,18 +331,15 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
 
-    static bool attr_set = false;
-    if (!attr_set) {
+    {   // function attributes are per device: set on every launch (cheap), no process-wide cache
         cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_large_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     const int ntiles = (N / TILE_N) * ((M + TN - 1) / TN);
     // narrow token tiles: two k blocks per stage (the MMAs of a 128 x TN x 32 step have a 31 ns floor for TN <= 112,
     // so four of them do not cover one full/empty handoff; eight do)
-    static const int tune_ks = env_ks();
-    const int KS = (tune_ks > 0) ? tune_ks : ((TN <= 160 && (K / TILE_K) % 2 == 0) ? 2 : 1);
+    const int KS = (TN <= 160 && (K / TILE_K) % 2 == 0) ? 2 : 1;
     const int stage = KS * (int)lg_stage_stride(TN);
     const int sw_bytes = LG_SW * KS * LG_W_BYTES;
     int NS = (LG_STAGE_REGION + LG_SW * LG_W_BYTES - sw_bytes) / stage;
@@ -457,10 +420,5 @@ cudaError_t run_i8_mma_probe(int ctas, int mmas_per_cta, float* ms_out) {
     cudaEventDestroy(b);
     return e;
 }
-
-#ifdef VLA_LG_DEBUG
-extern "C" int vla_debug_set_lg(int v) { return (int)cudaMemcpyToSymbol(g_lg_dbg, &v, sizeof(int)); }
-extern "C" int vla_debug_get_lg_trace(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_lg_trace, sizeof(g_lg_trace)); }
-#endif
 
 }  // namespace vla

@@ -15,7 +15,6 @@
 // weight stream of call i+1 overlaps the tail of call i (weights never depend on the previous kernel).
 #include <cooperative_groups.h>
 #include <cuda_bf16.h>
-#include <cstdlib>
 #include "common.cuh"
 #include "kernels.h"
 
@@ -182,19 +181,12 @@ __global__ void __launch_bounds__(SM_THREADS) gemm_small_kernel(
     }
 }
 
-static int env_int(const char* name, int dflt) {
-    const char* v = std::getenv(name);
-    return v ? std::atoi(v) : dflt;
-}
-
 template <int MTOK, bool USE_MMA>
 static cudaError_t launch_one(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,
                               int M, int N, int K, void* out, int out_dtype, cudaStream_t s) {
     const int n32 = N / BLK_N, kq = K / BLK_K;
-    static const int tune_ksplit = env_int("VLA_TUNE_KSPLIT", 0);
     int ksplit = 1;
-    if (tune_ksplit > 0) ksplit = tune_ksplit;
-    else while (n32 * ksplit < 296 && ksplit < 8 && kq / (ksplit * 2) >= 4) ksplit *= 2;
+    while (n32 * ksplit < 296 && ksplit < 8 && kq / (ksplit * 2) >= 4) ksplit *= 2;
     const int kq_per_cta = (kq + ksplit - 1) / ksplit;
 
     cudaLaunchConfig_t cfg = {};

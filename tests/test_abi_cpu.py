@@ -71,7 +71,7 @@ def test_host_validation_precedes_any_launch(vla):
     fake = 0x1000  # 16-byte aligned non-NULL "pointer"; never dereferenced because validation fails first
     assert L.vla_ternary_pack(None, 256, 256, fake, 16384, None) == vla.VLA_ERR_NULL
     assert L.vla_ternary_pack(fake, 100, 256, fake, 16384, None) == vla.VLA_ERR_SHAPE
-    assert L.vla_ternary_pack(fake, 256, 256, fake, 100, None) == vla.VLA_ERR_SHAPE
+    assert L.vla_ternary_pack(fake, 256, 256, fake, 100, None) == vla.VLA_ERR_WORKSPACE      # packed buffer too small
     assert L.vla_ternary_pack(fake + 4, 256, 256, fake, 16384, None) == vla.VLA_ERR_ALIGN
     assert L.vla_act_quant(None, 8, 256, fake, fake, None) == vla.VLA_ERR_NULL
     assert L.vla_act_quant(fake, 0, 256, fake, fake, None) == vla.VLA_ERR_SHAPE

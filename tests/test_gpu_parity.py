@@ -419,6 +419,104 @@ def test_grouped_large_gemm_per_group_scales(vla, oracle):
             assert np.array_equal(bf16_bits_of(out), ref["ybf16"])
 
 
+def test_grouped_full_size_ragged_mixed_dtypes(vla, oracle):
+    """The grouped tcgen05 launch at model size with a ragged token count (M = 545: one token past the prefill's 544) and
+    mixed output types: gate|up|k-like group, K = 2560, N = 6912 | 6912 | 640 (113 channel tiles over several waves, tiles
+    of three linears in one walk).  Rows are sampled for the oracle (its int32 contraction is exact per row)."""
+    M, K = 545, 2560
+    x_bits = synth.activations(M, K, 4343, outlier_frac=0.01)
+    x = dev_bf16(x_bits)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(x, M, K, xq, xs)
+    specs = [(6912, vla.VLA_BF16, 0.021), (6912, vla.VLA_F32, 0.3), (640, vla.VLA_I32, 0.07)]
+    lins, keep = [], []
+    for i, (N, dt, beta) in enumerate(specs):
+        w = synth.ternary_weights(N, K, 0.35, 950 + i)
+        beta_d = dev(np.array([beta], np.float32))
+        out = vla.empty_out(M, N, dt)
+        keep.append((w, beta_d, out, np.float32(beta), dt))
+        lins.append(dict(packed=vla.pack_weights(dev(w)), w_scale=beta_d, out=out, N=N, out_dtype=dt))
+    vla.vla_ternary_gemm_grouped(lins, xq, xs, M, K, vla.VLA_PATH_AUTO)
+    torch.cuda.synchronize()
+    rows = np.array([0, 1, 95, 96, 127, 128, 255, 256, 300, 511, 512, 543, 544])
+    for (w, beta_d, out, beta, dt) in keep:
+        ref = oracle.ternary_linear(np.ascontiguousarray(x_bits[rows]), w, beta)
+        got = out[torch.from_numpy(rows).cuda()]
+        if dt == vla.VLA_I32:
+            assert np.array_equal(got.cpu().numpy(), ref["acc"])
+        elif dt == vla.VLA_F32:
+            assert np.array_equal(got.cpu().numpy().view(np.uint32), ref["y32"].view(np.uint32))
+        else:
+            assert np.array_equal(bf16_bits_of(got.contiguous()), ref["ybf16"])
+
+
+def test_grouped_equal_groups_vs_oracle_group_vector(vla, oracle):
+    """Eq. 4's beta_g(n) in the oracle's own form: three equal output groups with a [G=3] scale vector (the branch pinned
+    by test_ternary_linear_bf16_with_three_output_groups_vs_exact) against ONE grouped launch of three linears."""
+    M, K, Ng = 77, 1280, 256
+    x_bits = synth.activations(M, K, 4444, outlier_frac=0.01)
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(x_bits), M, K, xq, xs)
+    w = synth.ternary_weights(3 * Ng, K, 0.35, 960)
+    betas = np.array([0.013, 0.4, 0.077], np.float32)
+    outs, lins, keep = [], [], []
+    for g in range(3):
+        out = vla.empty_out(M, Ng, vla.VLA_BF16)
+        bd = dev(betas[g:g + 1])
+        keep.append(bd)
+        outs.append(out)
+        lins.append(dict(packed=vla.pack_weights(dev(w[g * Ng:(g + 1) * Ng])), w_scale=bd, out=out, N=Ng, out_dtype=vla.VLA_BF16))
+    vla.vla_ternary_gemm_grouped(lins, xq, xs, M, K, vla.VLA_PATH_LARGE)
+    torch.cuda.synchronize()
+    ref = oracle.ternary_linear(x_bits, w, betas)
+    for g in range(3):
+        assert np.array_equal(bf16_bits_of(outs[g]), ref["ybf16"][:, g * Ng:(g + 1) * Ng]), "group %d" % g
+
+
+def test_longest_supported_k_saturating(vla):
+    """K = 65536, the largest K the ABI accepts: saturated activations (+-127) against sign-pattern weights, |acc| =
+    127 * 65536 (the decode's factor 64 leaves 64 * 127 * K < 2^31), on every path that takes this M."""
+    M, N, K = 4, 128, 65536
+    x = np.ones((M, K), np.float32)
+    x[1] = -1.0
+    x[2, ::2] = -1.0
+    x[3, ::3] = 0.5
+    w = np.ones((N, K), np.int8)
+    w[1::2] = -1
+    w[5, ::7] = 0
+    packed = vla.pack_weights(dev(w))
+    xq = torch.empty((M, K), dtype=torch.int8, device="cuda")
+    xs = torch.empty((M,), dtype=torch.float32, device="cuda")
+    vla.vla_act_quant(dev_bf16(synth._f32_to_bf16_bits(x)), M, K, xq, xs)
+    want = xq.cpu().numpy().astype(np.int64) @ w.T.astype(np.int64)
+    assert np.abs(want).max() == 127 * K
+    beta_d = dev(np.array([1.0], np.float32))
+    for path in paths_for(vla, M):
+        acc = run_gemm(vla, packed, beta_d, xq, xs, M, N, K, vla.VLA_I32, path).cpu().numpy()
+        assert np.array_equal(acc, want), "path %d" % path
+
+
+def test_forced_path_token_limits(vla):
+    """include/vla_ternary.h: VLA_PATH_SMALL_ALU takes M <= 16, VLA_PATH_SMALL_TC M <= 32; one more token is VLA_ERR_SHAPE."""
+    K, N = 256, 128
+    packed = vla.pack_weights(dev(synth.ternary_weights(N, K, 0.3, 3)))
+    beta_d = dev(np.array([0.05], np.float32))
+    for path, mmax in ((vla.VLA_PATH_SMALL_ALU, 16), (vla.VLA_PATH_SMALL_TC, 32)):
+        for M, ok in ((mmax, True), (mmax + 1, False)):
+            xq = torch.zeros((M, K), dtype=torch.int8, device="cuda")
+            xs = torch.ones((M,), dtype=torch.float32, device="cuda")
+            out = vla.empty_out(M, N, vla.VLA_F32)
+            if ok:
+                vla.vla_ternary_gemm(packed, beta_d, xq, xs, M, N, K, out, vla.VLA_F32, path, None, 0)
+            else:
+                with pytest.raises(vla.VlaError) as e:
+                    vla.vla_ternary_gemm(packed, beta_d, xq, xs, M, N, K, out, vla.VLA_F32, path, None, 0)
+                assert e.value.status == vla.VLA_ERR_SHAPE
+    torch.cuda.synchronize()
+
+
 @pytest.mark.parametrize("M,path_name", [(7, "small_tc"), (7, "small_alu"), (37, "large"), (200, "large")])
 def test_guard_bands_single_calls(vla, oracle, M, path_name):
     """Sentinel bytes around xq, alpha and the output survive act_quant + GEMM on every path (ragged M)."""

@@ -192,6 +192,53 @@ def test_team_mode_with_multi_chunk_granules(vla, oracle, M, K, N, nst):
     vla.vla_program_release(prog)
 
 
+def test_chained_stack_m544_grouped_tcgen05(vla, oracle):
+    """configs[3] at M=544, the launch configuration `bench.py --workload stack` times: 3 full-size layers through
+    Stack.run_stack_calls (activation quant + ONE grouped tcgen05 launch per stage: q|k|v as N=3840, gate|up as N=13824,
+    channel tiles crossing the linears' boundaries inside one persistent tile walk), free-running, every intermediate of
+    every layer bit-identical to the oracle's chain."""
+    from paper_2606_08094_b200.stack import Stack
+    layers, M = 3, synth.PREFILL_M
+    weights = [synth.stack_layer(l) for l in range(layers)]
+    x = synth.stack_input(M)
+    st = Stack(layers, M, weights=weights)
+    st.set_input(x)
+    st.alloc_call_workspace()
+    st.run_stack_calls()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()                               # and once more from a CUDA graph, as the bench runs it
+    with torch.cuda.graph(g):
+        st.run_stack_calls()
+    ref = oracle_stack(oracle, weights, x)
+    for rep in range(2):
+        for l in range(layers):
+            for n in ref[l]:
+                assert np.array_equal(bits(st.out[l][n]), ref[l][n]), "layer %d %s differs (rep %d)" % (l, n, rep)
+                st.out[l][n].zero_()
+        if rep == 0:
+            g.replay()
+            torch.cuda.synchronize()
+
+
+def test_full_depth_stack_m8_one_launch(vla, oracle):
+    """The launch `bench.py --workload stack` times at M=8: all 30 layers = 120 dependent phases, 210 linears, in ONE
+    persistent launch (descriptor tables near their capacity), free-running against the oracle's 30-layer chain."""
+    from paper_2606_08094_b200.stack import Stack
+    layers, M = synth.STACK_LAYERS, 8
+    weights = [synth.stack_layer(l) for l in range(layers)]
+    x = synth.stack_input(M)
+    st = Stack(layers, M, weights=weights)
+    st.set_input(x)
+    st.compile()
+    ref = oracle_stack(oracle, weights, x)
+    for rep in range(2):
+        st.run_program()
+        torch.cuda.synchronize()
+        for l in range(layers):
+            for n in ref[l]:
+                assert np.array_equal(bits(st.out[l][n]), ref[l][n]), "layer %d %s differs (rep %d)" % (l, n, rep)
+
+
 def test_program_errors(vla):
     p = make_point(vla, 8, 256, 256, 5, vla.VLA_BF16)
     bad_m = dict(stage_of(p), M=17)

@@ -260,6 +260,30 @@ def test_rescale_order_and_groups(oracle):
     assert (f32_bits(yg[:, 4:]) == f32_bits(acc[:, 4:].astype(np.float32) * (alpha * bg[1])[:, None])).all()
 
 
+def test_ternary_linear_bf16_with_three_output_groups_vs_exact(oracle):
+    """orc_ternary_linear's bf16 output with a [G=3] beta vector (oracle.cpp, the grouped branch): every group's
+    channels against tests/exact.py (exact rationals, own rounding), which knows nothing about groups -- it is called
+    once per group with that group's scalar beta."""
+    rng = np.random.default_rng(77)
+    M, K, N, G = 3, 16, 6, 3
+    x_bits = synth.activations(M, K, 991, outlier_frac=0.1)
+    w = rng.integers(-1, 2, (N, K)).astype(np.int8)
+    betas = np.array([0.0371, 0.5, 0.011], np.float32)
+    got = oracle.ternary_linear(x_bits, w, betas)
+    per = N // G
+    for g in range(G):
+        ex = exact.linear([list(map(int, r)) for r in x_bits], [list(map(int, r)) for r in w[g * per:(g + 1) * per]],
+                          Fraction(float(betas[g])))
+        for m in range(M):
+            for n in range(per):
+                assert int(got["acc"][m, g * per + n]) == ex["acc"][m][n]
+                assert int(f32_bits(got["y32"])[m, g * per + n]) == exact.fraction_to_f32_bits(ex["y32"][m][n])
+                assert int(got["ybf16"][m, g * per + n]) == exact.fraction_to_bf16_bits(ex["ybf16"][m][n])
+    # and it is NOT what a single scale would give
+    one = oracle.ternary_linear(x_bits, w, betas[:1])
+    assert not np.array_equal(one["ybf16"][:, per:], got["ybf16"][:, per:])
+
+
 def test_bf16_rne_matches_torch_and_ties(oracle):
     rng = np.random.default_rng(4)
     v = (rng.standard_normal(200000) * np.exp(rng.uniform(-20, 20, 200000))).astype(np.float32)
