@@ -122,3 +122,23 @@ def config4_point(M, shape_idx, zf_idx, dist_idx):
                     activations(max(SWEEP_M), K, _seed_x(4, shape_idx, dist_idx),
                                 dist=SWEEP_DISTS[dist_idx])[:M]),
                 out="f32")
+
+
+# ------------------------------------------------------------------ cached-conditioning attention
+ATTN_HEADS = (20, 5, 128)      # query heads, KV heads, head dim of BASELINE.json configs[3]
+ATTN_MC = PREFILL_M            # conditioning tokens: the 544-token prefix of configs[2]
+
+
+def attention_inputs(Mq, Mc, n_q_heads, n_kv_heads, d_k, seed, masked_frac=0.0, scale=1.0):
+    """bf16 bit patterns of Q [Mq, Hq*d], K_C / V_C [Mc, Hkv*d] (N(0, scale^2), stand-ins for the outputs of the q / k / v
+    linears on LIBERO observations, which are not available) and a visibility mask uint8 [Mq, Mc] (1 = visible; with
+    masked_frac > 0 a random subset of keys is masked per query row, at least one key stays visible), or None."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    q = _f32_to_bf16_bits(rng.standard_normal((Mq, n_q_heads * d_k), dtype=np.float32) * np.float32(scale))
+    kc = _f32_to_bf16_bits(rng.standard_normal((Mc, n_kv_heads * d_k), dtype=np.float32) * np.float32(scale))
+    vc = _f32_to_bf16_bits(rng.standard_normal((Mc, n_kv_heads * d_k), dtype=np.float32))
+    vis = None
+    if masked_frac > 0.0:
+        vis = (rng.random((Mq, Mc)) >= masked_frac).astype(np.uint8)
+        vis[np.arange(Mq), rng.integers(0, Mc, Mq)] = 1
+    return q, kc, vc, vis
