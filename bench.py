@@ -480,6 +480,11 @@ def run_gpu(args):
         if roof_tensor is not None:
             roof_tensor["traffic"] = ncu_traffic("gemm_large")
 
+    attn = None
+    if args.workload == "decode" and not args.no_vs_m:
+        import bench_workloads as bw
+        attn = bw.attention_points(pk)                        # SURVEY 8(f) NEXT-4, reported beside the hot path
+
     # ---- the oracle on this box's host cores, bounded sample
     from oracle import oracle as orc
     orc.build()
@@ -508,7 +513,7 @@ def run_gpu(args):
         "clocks": clocks, "gpu_launches": launches,
         "e2e": {"value": e2e_bytes / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": wl.h2d,
                 "d2h_bytes_per_step": wl.d2h, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
-        "roofline": roof, "roofline_tensor": roof_tensor, "cpu_baseline": cpu, "points": table, "vs_M": vs_m,
+        "roofline": roof, "roofline_tensor": roof_tensor, "cpu_baseline": cpu, "points": table, "vs_M": vs_m, "attention_next4": attn,
         "step_roofline_frac_hbm": value / pk["hbm_gbs"],
     }
     print(json.dumps(line))

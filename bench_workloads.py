@@ -345,3 +345,51 @@ def run_vs_m(pk, int8_probe_tops, Ms=None, shapes=None):
                   "peak_source": "MEASURED_PEAKS.json bf16_tflops x 2 (int8:bf16 nominal ratio)",
                   "int8_probe_tops": int8_probe_tops, "frac_of_probe": ach / int8_probe_tops}
     return pts, roof_t
+
+
+# ----------------------------------------------------------------------------- cached attention
+def attention_points(pk, cpu_seconds=1.0):
+    """vla_cached_attention (Eq. 2) at the configs[3] head shape (20 query / 5 KV heads x 128) over a
+    cached 544-token conditioning sequence, Mq in {8, 16} action queries per solver step, T steps per CUDA graph (K_C / V_C
+    are computed once and stay in L2: that is the point of the cache).  Returns a list of records: us per step, the
+    algorithmic bytes a step touches (Q + K_C + V_C + out) per second, GFLOP/s, and the oracle's time beside it."""
+    import torch
+    from paper_2606_08094_b200 import binding as vla, synth
+    from oracle import attention as att
+    dev = torch.device("cuda", torch.cuda.current_device())
+    Hq, Hkv, d = synth.ATTN_HEADS
+    Mc, T = synth.ATTN_MC, 64
+    recs = []
+    for Mq in (8, 16):
+        q, kc, vc, _ = synth.attention_inputs(Mq, Mc, Hq, Hkv, d, 8100 + Mq)
+        tb = lambda b: torch.from_numpy(np.ascontiguousarray(b).view(np.int16)).to(dev).view(torch.bfloat16)
+        qd, kd, vd = tb(q), tb(kc), tb(vc)
+        out = torch.empty((Mq, Hq * d), dtype=torch.bfloat16, device=dev)
+        nb = vla.vla_cached_attention_workspace_bytes(Mq, Mc, Hq, Hkv, d)
+        ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev)
+
+        def steps():
+            for _ in range(T):
+                vla.vla_cached_attention(qd, kd, vd, None, Mq, Mc, Hq, Hkv, d, out, vla.VLA_BF16, ws, nb)
+        steps()
+        torch.cuda.synchronize()
+        n0 = vla.vla_launch_count()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            steps()
+        launches = (vla.vla_launch_count() - n0) / T
+        sec = _time(torch, g.replay, 10) / T
+        by = 2 * (Mq * Hq * d + 2 * Mc * Hkv * d + Mq * Hq * d)
+        fl = 4.0 * Mq * Mc * d * Hq
+        t0 = time.perf_counter()
+        n = 0
+        while time.perf_counter() - t0 < cpu_seconds:
+            att.cached_attention(q, kc, vc, Hq, Hkv, d)
+            n += 1
+        cpu_us = (time.perf_counter() - t0) / n * 1e6
+        recs.append({"Mq": Mq, "Mc": Mc, "heads": "%dq/%dkv x %d" % (Hq, Hkv, d), "us_per_step": sec * 1e6,
+                     "launches_per_step": launches, "GBs": by / sec / 1e9, "GFLOPs": fl / sec / 1e9,
+                     "bound": "latency (1.4 MB of cached K_C/V_C from L2, 0.09 GFLOP)",
+                     "hbm_time_us_if_uncached": by / (pk["hbm_gbs"] * 1e9) * 1e6,
+                     "oracle_us_per_step": cpu_us, "oracle": "numpy float64, oracle/attention.py"})
+    return recs

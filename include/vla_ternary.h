@@ -199,6 +199,29 @@ vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in /*host*
 /* Forgets a compiled program (the caller then frees prog_dev). */
 vla_status vla_program_release(const void* prog_dev);
 
+/* ---------------------------------------------------------------------------------------------------
+ * Cached-conditioning cross-attention, Eq. 2 of the paper (section III-B), per head:
+ *
+ *     Attn(Q, K_C, V_C; M) = softmax(Q K_C^T / sqrt(d_k) + M) V_C          softmax over keys
+ *
+ * K_C = Z W_K and V_C = Z W_V are the cached projections of the conditioning sequence ("a cross-attention head caches
+ * K_C and V_C"): the caller computes them ONCE per observation (e.g. with vla_ternary_linear on the
+ * k / v weights) and passes the same buffers to every solver step; only q changes between steps.
+ *   q_bf16       [Mq, n_q_heads * d_k] bf16, row-major (the q linear's output: head h is columns [h*d_k, (h+1)*d_k))
+ *   kc_bf16      [Mc, n_kv_heads * d_k] bf16 (the k linear's output), vc_bf16 the same shape (the v linear's output)
+ *   visible_opt  NULL (every key visible) or [Mq, Mc] bytes: 1 = visible (M = 0), 0 = masked (M = -inf)
+ *   out          [Mq, n_q_heads * d_k] of out_dtype (VLA_F32 or VLA_BF16 with round-to-nearest-even)
+ *   workspace    >= vla_cached_attention_workspace_bytes(...) bytes (partial results of the key splits)
+ * Grouped-query heads: query head h reads KV head h / (n_q_heads / n_kv_heads).  A query row whose keys are all masked
+ * gives 0.  Shapes: d_k == 128, n_q_heads % n_kv_heads == 0 with at most 8 query heads per KV head, 1 <= Mq <= 4096,
+ * 1 <= Mc <= 65536 (else VLA_ERR_SHAPE).  Arithmetic: bf16 x bf16 products and all sums in fp32, probabilities kept to
+ * 2^-17 relative; the result is within 2e-5 * max|V_C| of the float64 value of Eq. 2.  Asynchronous on
+ * `stream`, capturable in a CUDA graph. */
+size_t vla_cached_attention_workspace_bytes(int Mq, int Mc, int n_q_heads, int n_kv_heads, int d_k);
+vla_status vla_cached_attention(const void* q_bf16, const void* kc_bf16, const void* vc_bf16, const uint8_t* visible_opt,
+                                int Mq, int Mc, int n_q_heads, int n_kv_heads, int d_k, void* out, vla_dtype out_dtype,
+                                void* workspace, size_t workspace_bytes, void* stream);
+
 /* The path VLA_PATH_AUTO resolves to for (M,N,K). */
 vla_path vla_ternary_auto_path(int M, int N, int K);
 

@@ -26,6 +26,7 @@ EXPORTS = [
     "vla_act_quant", "vla_ternary_gemm", "vla_ternary_linear", "vla_ternary_linear_host",
     "vla_ternary_host_workspace_bytes",
     "vla_ternary_auto_path", "vla_i8_mma_issue_probe", "vla_status_string", "vla_launch_count",
+    "vla_cached_attention", "vla_cached_attention_workspace_bytes",
     "vla_ternary_gemm_grouped", "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_run_host", "vla_program_release",
 ]
 
@@ -97,6 +98,10 @@ def _load():
     lib.vla_program_run_host.argtypes = [vp, ctypes.POINTER(vla_copy), i, ctypes.POINTER(vla_copy), i, vp]
     lib.vla_program_release.restype = st
     lib.vla_program_release.argtypes = [vp]
+    lib.vla_cached_attention_workspace_bytes.restype = sz
+    lib.vla_cached_attention_workspace_bytes.argtypes = [i, i, i, i, i]
+    lib.vla_cached_attention.restype = st
+    lib.vla_cached_attention.argtypes = [vp, vp, vp, vp, i, i, i, i, i, vp, i, vp, sz, vp]
     return lib
 
 
@@ -251,6 +256,17 @@ def vla_program_run_host(prog_dev, copies_in, copies_out, stream=None):
     """copies_in / copies_out: ctypes arrays from make_copies.  Synchronises the stream."""
     _check(_lib.vla_program_run_host(_ptr(prog_dev), copies_in, len(copies_in), copies_out, len(copies_out),
                                      _stream(stream)), "vla_program_run_host")
+
+
+def vla_cached_attention_workspace_bytes(Mq, Mc, n_q_heads, n_kv_heads, d_k):
+    return int(_lib.vla_cached_attention_workspace_bytes(Mq, Mc, n_q_heads, n_kv_heads, d_k))
+
+
+def vla_cached_attention(q_bf16, kc_bf16, vc_bf16, visible_opt, Mq, Mc, n_q_heads, n_kv_heads, d_k, out, out_dtype,
+                         workspace=None, workspace_bytes=0, stream=None):
+    _check(_lib.vla_cached_attention(_ptr(q_bf16), _ptr(kc_bf16), _ptr(vc_bf16), _ptr(visible_opt), Mq, Mc, n_q_heads,
+                                     n_kv_heads, d_k, _ptr(out), out_dtype, _ptr(workspace), workspace_bytes,
+                                     _stream(stream)), "vla_cached_attention")
 
 
 def vla_program_release(prog_dev):

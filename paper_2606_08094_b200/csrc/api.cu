@@ -210,6 +210,45 @@ vla_status vla_ternary_linear_host(const void* packed, const float* w_scale, con
     return from_cuda(e);
 }
 
+// ---------------------------------------------------------------- cached-conditioning attention (Eq. 2)
+static bool attn_shape_ok(int Mq, int Mc, int Hq, int Hkv, int d_k) {
+    return Mq >= 1 && Mq <= 4096 && Mc >= 1 && Mc <= 65536 && d_k == 128 && Hkv >= 1 && Hq >= Hkv && Hq % Hkv == 0 &&
+           Hq / Hkv <= 8 && Hq <= 1024;
+}
+static int current_sms() {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return 148;                                           // (sizes only; the launch itself reports the error)
+    }
+    return sms > 0 ? sms : 148;
+}
+
+size_t vla_cached_attention_workspace_bytes(int Mq, int Mc, int n_q_heads, int n_kv_heads, int d_k) {
+    if (!attn_shape_ok(Mq, Mc, n_q_heads, n_kv_heads, d_k)) return 0;
+    // sized for the most splits any device takes (one per 64-key tile), so the answer does not depend on the device
+    return round256((size_t)((Mc + 63) / 64) * n_q_heads * Mq * (128 + 2) * sizeof(float));
+}
+
+vla_status vla_cached_attention(const void* q_bf16, const void* kc_bf16, const void* vc_bf16, const uint8_t* visible_opt,
+                                int Mq, int Mc, int n_q_heads, int n_kv_heads, int d_k, void* out, vla_dtype out_dtype,
+                                void* workspace, size_t workspace_bytes, void* stream) {
+    if (!q_bf16 || !kc_bf16 || !vc_bf16 || !out) return VLA_ERR_NULL;
+    if (out_dtype != VLA_F32 && out_dtype != VLA_BF16) return VLA_ERR_DTYPE;
+    if (!attn_shape_ok(Mq, Mc, n_q_heads, n_kv_heads, d_k)) return VLA_ERR_SHAPE;
+    if (!aligned16(q_bf16) || !aligned16(kc_bf16) || !aligned16(vc_bf16) || !aligned16(out)) return VLA_ERR_ALIGN;
+    vla_status st = check_arch();
+    if (st != VLA_OK) return st;
+    const int sms = current_sms();
+    const size_t need = vla::attention_workspace_bytes(Mq, Mc, n_q_heads, n_kv_heads, sms);
+    if (need > 0) {
+        if (!workspace || workspace_bytes < need) return VLA_ERR_WORKSPACE;
+        if (!aligned16(workspace)) return VLA_ERR_ALIGN;
+    }
+    return from_cuda(vla::launch_attention(q_bf16, kc_bf16, vc_bf16, visible_opt, Mq, Mc, n_q_heads, n_kv_heads, out,
+                                           (int)out_dtype, reinterpret_cast<float*>(workspace), sms, (cudaStream_t)stream));
+}
+
 unsigned long long vla_launch_count(void) { return vla::launch_count(); }
 
 vla_status vla_i8_mma_issue_probe(int ctas, int mmas_per_cta, float* ms_out) {

@@ -35,5 +35,9 @@ struct DevProg;
 cudaError_t launch_program(const DevProg& prog, int grid, int max_m, cudaStream_t s);
 cudaError_t program_max_ctas_per_sm(int max_m, int smem_bytes, int* out);      // co-residency of the persistent grid
 cudaError_t run_i8_mma_probe(int ctas, int mmas_per_cta, float* ms_out);
+// cached-conditioning cross-attention (attention.cu): d_k = 128, out_dtype 0 fp32 / 1 bf16
+size_t attention_workspace_bytes(int Mq, int Mc, int Hq, int Hkv, int sms);
+cudaError_t launch_attention(const void* q, const void* kc, const void* vc, const uint8_t* visible, int Mq, int Mc, int Hq,
+                             int Hkv, void* out, int out_dtype, float* workspace, int sms, cudaStream_t s);
 
 }  // namespace vla
