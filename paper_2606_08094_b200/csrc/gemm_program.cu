@@ -10,11 +10,14 @@
 //                        griddepcontrol.wait (weights never depend on the previous kernel) and never waits on
 //                        activations, so HBM stays busy across launch, stage and phase boundaries.
 //   warps 0-14 (consumers) per stage:
-//     1. activation quant, Eq. 4 lines 1-2, FUSED INTO THE PROLOGUE: every CTA of the stage's group reads the bf16
-//        rows itself (L2 hits after the first CTA), takes the row absmax, and quantises straight into shared memory
-//        in mma.m16n8k32 B-fragment order.  No CTA ever waits for another CTA's quantised activations: there is no
-//        int8 round trip through global memory and no flag (the caller's optional xq / alpha outputs are written by
-//        the group's first CTA on the side).
+//     1. activation quant, Eq. 4 lines 1-2, FUSED INTO THE KERNEL (quant_rows): a SMALL stage (<= 1440 sixteen-element
+//        tasks, e.g. M = 8 x K = 2560) is quantised by every CTA of its group for itself, from the bf16 rows straight
+//        into shared memory in mma.m16n8k32 B-fragment order -- no int8 round trip, no flag, nothing to wait for.  A
+//        LARGER stage is quantised cooperatively: row r once, by CTA r mod c of the stage's group, into the stage's
+//        scratch (already in fragment order), published with one release per CTA; every CTA of the group then pulls the
+//        finished fragments with one bulk copy.  Either way the weight ring is never gated on activations.
+//        The quantiser is an exact shortcut of the two true divisions (bracketed FMA, true-division patch for the rare
+//        element whose bracket holds a rounding boundary): bit-identical to quant.cuh / the oracle.
 //     2. GEMM: packed words from the ring are decoded in registers (2 ALU ops per 4 weights, common.cuh) into A
 //        fragments, B fragments come from shared memory, int32 accumulation on the warp-level int8 MMA.  Either
 //        three TEAMS of five warps work on three granules at once (each team's warps split the k blocks of its
@@ -24,8 +27,9 @@
 // Work unit: a GRANULE = 32 output channels x all of K of one linear (one contiguous run of 8*K bytes).  The stages
 // of one PHASE are independent, so they run CONCURRENTLY on disjoint CTA groups sized by the program compiler
 // (api_program.cu); granule gi of a stage goes to CTA (gi mod group size) of its group.
-// The only grid-wide synchronisation left is between dependent phases:
-//   bp[p] = CTAs that finished phase p   (a dependent phase's CTAs wait for bp[p-1] == gridDim.x before reading x)
+// Counters in the program buffer (re-zeroed by the last CTA of every launch):
+//   bp[p]  = CTAs that finished phase p      (a dependent phase's CTAs wait for bp[p-1] == gridDim.x before reading x)
+//   cnt[s] = rows of cooperative stage s in its scratch   (the stage's group waits for cnt[s] == M_s before its bulk copy)
 // Every sum is an exact integer sum and the quantiser reproduces the two true divisions of Eq. 4 bit for bit, so the
 // result is bit-identical to the per-call kernels and to the oracle.
 #include <cuda_bf16.h>
@@ -49,7 +53,6 @@ static_assert(PG_TEAMS * PG_TW == PG_W, "teams must cover the consumer warps");
 #else
 #define PG_STAMP(k) do { } while (0)
 #endif
-#define PG_STAMPP(k, p) PG_STAMP(((k) - 2) + 2 + 6 * ((p) & 3) + 2)
 
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" :: "n"(PG_CONSUMERS) : "memory"); }
 __device__ __forceinline__ void team_bar(int team) {
@@ -258,9 +261,7 @@ __device__ __forceinline__ void quant_rows(const DevProg& P, const DevStage& st,
                 }
             }
         }
-        PG_STAMP(26);
         consumer_bar();
-        PG_STAMP(27);
         if (tid < 16) {                                      // per row: alpha_m and the bracketing reciprocals
             const float alpha = alpha_of(__uint_as_float(s_rowmax[tid]));
             const float inv = __frcp_rn(alpha);
@@ -272,7 +273,6 @@ __device__ __forceinline__ void quant_rows(const DevProg& P, const DevStage& st,
             }
         }
         consumer_bar();
-        PG_STAMP(28);
 #pragma unroll
         for (int i = 0; i < PG_QNB; ++i) {
             const int f = tid + i * PG_CONSUMERS;
@@ -286,7 +286,6 @@ __device__ __forceinline__ void quant_rows(const DevProg& P, const DevStage& st,
                 if (write_out && st.xq_out) *reinterpret_cast<uint4*>(st.xq_out + (size_t)row * K + c * 16) = q;
             }
         }
-        PG_STAMP(29);
     }
 }
 
@@ -550,13 +549,12 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
         if (s >= 0) {                                        // this CTA runs stage s in phase p
             const DevStage& st = stages[s];
             const int count = st.cta_count, rank = cta - st.cta_begin;
-            PG_STAMPP(6, p);
             if (p > 0) {                                     // a phase starts only after every earlier phase has completed
                                                               // (vla_ternary.h: x of ANY of its stages may be an earlier phase's output)
                 if (tid == 0) spin_until(P.bp + (p - 1), (unsigned)G);
                 consumer_bar();
             }
-            PG_STAMPP(2, p);
+            PG_STAMP(2);
             // the stage's scales beta -> shared memory (one L2 round trip per stage instead of one per granule)
             // (loaded now, stored after the quantisation: a cold scale costs a DRAM round trip that must not delay this
             // warp's activation loads)
@@ -601,12 +599,9 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
                 }
             }
             if (tid >= 32 && tid < 32 + st.n_lin) s_beta[tid - 32] = beta_r;
-#ifdef VLA_PROG_STAMPS
-            if ((tid & 31) == 0 && P.stamps) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.stamps[(148 + blockIdx.x) * 32 + (tid >> 5)] = t_; }
-#endif
             consumer_bar();                                  // fragments and scales are complete
             if (tid < 16) s_rowmax[tid] = 0u;                // (the next stage's atomics come after its own barriers)
-            PG_STAMPP(3, p);
+            PG_STAMP(3);
             const bool teams = prog_team_mode(st.granules, count);
             if (MAXMT == 1 || st.M <= 8) {
                 if (teams) stage_gemm_teams<1>(lins, st, rank, count, tid, R, red, xq_s, s_beta, s_scale, seq, gcount);
@@ -616,12 +611,11 @@ __global__ void __launch_bounds__(PG_THREADS, 1) program_kernel(const __grid_con
                 else stage_gemm<MAXMT>(lins, st, rank, count, tid, R, red, xq_s, s_beta, s_scale, seq, gcount);
             }
             consumer_bar();                                  // everybody is done with xq_s / s_beta / s_scale of this stage
-            PG_STAMPP(4, p);
+            PG_STAMP(4);
         }
         if (info & INFO_PUBLISH) {                           // end of a phase that a later phase reads from
             consumer_bar();                                  // every output store of this CTA precedes the release
             if (tid == 0) red_release_gpu(P.bp + p, 1u);
-            PG_STAMPP(5, p);
         }
     }
     if (!go_sent && tid == 0) mbar_arrive(bar_go);           // (a CTA without a stage: its producer has nothing to copy)
