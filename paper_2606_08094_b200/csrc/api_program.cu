@@ -17,15 +17,35 @@
 #endif
 #ifndef VLA_PG_START0
 #define VLA_PG_START0 3300.0
+#endif
+#ifndef VLA_PG_START1
 #define VLA_PG_START1 2.5
-#define VLA_PG_START_COOP 10000.0
-#define VLA_PG_T1A 400.0
-#define VLA_PG_T1B 45.0
+#endif
+#ifndef VLA_PG_START_COOP
+#define VLA_PG_START_COOP 9000.0
+#endif
+#ifndef VLA_PG_T1A
+#define VLA_PG_T1A 200.0
+#endif
+#ifndef VLA_PG_T1B
+#define VLA_PG_T1B 55.0
+#endif
+#ifndef VLA_PG_T2A
 #define VLA_PG_T2A 700.0
+#endif
+#ifndef VLA_PG_T2B
 #define VLA_PG_T2B 75.0
+#endif
+#ifndef VLA_PG_F1A
 #define VLA_PG_F1A 954.0
+#endif
+#ifndef VLA_PG_F1B
 #define VLA_PG_F1B 50.0
+#endif
+#ifndef VLA_PG_F2A
 #define VLA_PG_F2A 1212.0
+#endif
+#ifndef VLA_PG_F2B
 #define VLA_PG_F2B 75.0
 #endif
 
