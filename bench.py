@@ -542,6 +542,8 @@ def run_extra(args):
     pk = peaks()
     if args.workload == "stack":
         return bw.run_stack(args, pk, ClockSampler(0))
+    if args.workload == "dispatch":
+        return bw.run_dispatch(args, pk, ClockSampler(0))
     return bw.run_sweep(args, pk, ClockSampler(0), int8_probe_tops(vla))
 
 
@@ -550,7 +552,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=4000)
     ap.add_argument("--warmup", type=int, default=16)
-    ap.add_argument("--workload", choices=["decode", "prefill", "stack", "sweep"], default="decode")
+    ap.add_argument("--workload", choices=["decode", "prefill", "stack", "sweep", "dispatch"], default="decode")
     ap.add_argument("--quick", action="store_true", help="sweep: one zero fraction and one distribution only")
     ap.add_argument("--sweep-m", default="", help="sweep: comma-separated M values (default: 1,2,4,...,4096)")
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
@@ -560,10 +562,10 @@ def main():
     ap.add_argument("--no-vs-m", action="store_true", help="skip the vs-M block (both halves of the metric)")
     args = ap.parse_args()
     if args.impl == "reference":
-        if args.workload in ("stack", "sweep"):
+        if args.workload in ("stack", "sweep", "dispatch"):
             args.workload = "decode"
         return run_reference(args)
-    if args.workload in ("stack", "sweep"):
+    if args.workload in ("stack", "sweep", "dispatch"):
         return run_extra(args)
     return run_gpu(args)
 

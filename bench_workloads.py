@@ -251,6 +251,52 @@ def run_sweep(args, pk, clock_sampler, int8_probe_tops):
     return 0
 
 
+# ----------------------------------------------------------------------------- row a6: forced paths side by side (ncu target)
+def run_dispatch(args, pk, clock_sampler):
+    """Row a6 evidence: the kernels the dispatcher chooses between, forced, on the same pre-quantised inputs over cold
+    packed weights -- dp4a (VLA_PATH_SMALL_ALU) vs IMMA (VLA_PATH_SMALL_TC) at M in {8, 16}, IMMA vs tcgen05
+    (VLA_PATH_LARGE) at M in {17, 24, 32}.  Few eager launches per point (3 timed), so that an
+    `ncu --metrics ... -k regex:gemm_` pass over this command stays short; profiles/r02_dispatch_ncu.md is that pass."""
+    import torch
+    from paper_2606_08094_b200 import binding as vla, synth
+    dev = torch.device("cuda", 0)
+    l2 = torch.cuda.get_device_properties(dev).L2_cache_size
+    flush = torch.empty(2 * l2, dtype=torch.uint8, device=dev)
+    rows = []
+    clock_sampler.start()
+    for si, (K, N) in enumerate(synth.MODEL_SHAPES):
+        w = synth.ternary_weights(N, K, 0.35, 4900 + si)
+        packed = vla.pack_weights(torch.from_numpy(w).to(dev))
+        beta = torch.tensor([0.05], dtype=torch.float32, device=dev)
+        for M, paths in ((8, ("SMALL_ALU", "SMALL_TC")), (16, ("SMALL_ALU", "SMALL_TC")),
+                         (17, ("SMALL_TC", "LARGE")), (24, ("SMALL_TC", "LARGE")), (32, ("SMALL_TC", "LARGE"))):
+            xq = torch.randint(-127, 128, (M, K), dtype=torch.int8, device=dev)
+            xs = torch.rand(M, device=dev) + 0.01
+            out = torch.empty((M, N), dtype=torch.bfloat16, device=dev)
+            row = {"M": M, "K": K, "N": N, "auto": int(vla.vla_ternary_auto_path(M, N, K))}
+            for name in paths:
+                path = getattr(vla, "VLA_PATH_" + name)
+                us = []
+                for _ in range(4):                                  # first one is the warm-up
+                    flush.fill_(1)                                   # weights leave L2
+                    e0, e1 = _events(torch)
+                    e0.record()
+                    vla.vla_ternary_gemm(packed, beta, xq, xs, M, N, K, out, vla.VLA_BF16, path, None, 0)
+                    e1.record()
+                    e1.synchronize()
+                    us.append(e0.elapsed_time(e1) * 1e3)
+                row[name + "_us"] = float(np.median(us[1:]))
+            rows.append(row)
+        del packed
+    clocks = clock_sampler.stop()
+    print(json.dumps({"metric": "ternary GEMM TOPS & HBM GB/s vs M; fraction of INT8/HBM roofline (1 B200)",
+                      "value": None, "unit": "us per forced-path launch (eager, cold weights, includes launch overhead)",
+                      "n_gpus": 1, "steps": 3, "warmup": 1, "higher_is_better": False, "data": "synthetic",
+                      "config": {"workload": "row a6 dispatch evidence: forced paths on the four model shapes"},
+                      "clocks": clocks, "dispatch": rows}))
+    return 0
+
+
 # ----------------------------------------------------------------------------- the metric "vs M" (default bench.py line)
 VS_M_SHAPES = [(2560, 2560), (2560, 640), (2560, 6912), (6912, 2560), (8192, 8192)]
 VS_M_M = [1, 8, 16, 64, 512, 544, 1024, 4096]
