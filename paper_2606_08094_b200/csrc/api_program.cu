@@ -10,6 +10,8 @@
 #include <vector>
 #include "kernels.h"
 #include "program.h"
+#include "lprogram.h"
+#include "gemm_large.cuh"
 
 // partition model constants (SM cycles; see vla_program_build).  Compile-time defaults, overridable for calibration.
 #ifndef VLA_PROG_GATE
@@ -55,16 +57,62 @@ using vla::DevLin;
 using vla::DevProg;
 using vla::DevStage;
 
-struct ProgInfo { int grid; int n_stages; int max_m; DevProg header; };
+struct ProgInfo { int grid; int n_stages; int max_m; DevProg header; bool large; vla::DevLProg lheader; };
 std::mutex g_mu;
 std::unordered_map<const void*, ProgInfo> g_programs;
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline size_t round256(size_t b) { return (b + 255) / 256 * 256; }
 
+// LARGE programs (every stage has M > 16 tokens): the persistent tcgen05 kernel of gemm_lprog.cu
+bool is_large(const vla_prog_stage* st) { return st[0].M > 16; }
+
+vla_status check_large(const vla_prog_stage* st, int n) {
+    for (int s = 0; s < n; ++s) {
+        const vla_prog_stage& a = st[s];
+        if (!a.x_bf16 || !a.linears) return VLA_ERR_NULL;
+        if (a.M <= 16 || a.M > 32768 || a.K < 128 || a.K % 128 != 0 || a.K > 8192) return VLA_ERR_SHAPE;
+        if (a.n_linears < 1 || a.n_linears > 8) return VLA_ERR_SHAPE;
+        if (a.depends != 0 && a.depends != 1) return VLA_ERR_SHAPE;
+        if (!aligned16(a.x_bf16) || (a.xq_opt && !aligned16(a.xq_opt)) || (a.x_scale_opt && !aligned16(a.x_scale_opt)))
+            return VLA_ERR_ALIGN;
+        for (int j = 0; j < a.n_linears; ++j) {
+            const vla_prog_linear& l = a.linears[j];
+            if (l.out_dtype < 0 || l.out_dtype > 2) return VLA_ERR_DTYPE;
+            if (!l.packed || !l.out || (l.out_dtype != VLA_I32 && !l.w_scale)) return VLA_ERR_NULL;
+            if (l.N < 128 || l.N % 128 != 0) return VLA_ERR_SHAPE;
+            if (!aligned16(l.packed) || !aligned16(l.out) || (reinterpret_cast<uintptr_t>(l.w_scale) & 3u)) return VLA_ERR_ALIGN;
+        }
+    }
+    return VLA_OK;
+}
+
+struct LLayout { size_t off_stages, off_counters, off_xq[2], off_xs[2], total; };
+
+LLayout llayout_of(const vla_prog_stage* st, int n) {
+    LLayout L{};
+    size_t max_xq = 0, max_m = 0;
+    for (int s = 0; s < n; ++s) {
+        max_xq = std::max(max_xq, (size_t)st[s].M * (size_t)st[s].K);
+        max_m = std::max(max_m, (size_t)st[s].M);
+    }
+    size_t o = round256(sizeof(vla::DevLProg));
+    L.off_stages = o;   o += round256(sizeof(vla::LpStage) * (size_t)n);
+    L.off_counters = o; o += round256(sizeof(unsigned) * (2 * (size_t)n + 1));
+    for (int b = 0; b < 2; ++b) { L.off_xq[b] = o; o += round256(max_xq); }
+    for (int b = 0; b < 2; ++b) { L.off_xs[b] = o; o += round256(4 * max_m); }
+    L.total = o;
+    return L;
+}
+
 vla_status check_stages(const vla_prog_stage* st, int n) {
     if (!st) return VLA_ERR_NULL;
     if (n < 1 || n > 4096) return VLA_ERR_SHAPE;
+    {                                                         // one kind per program: all stages small, or all large
+        const bool large = is_large(st);
+        for (int s = 1; s < n; ++s) if ((st[s].M > 16) != large) return VLA_ERR_SHAPE;
+        if (large) return check_large(st, n);
+    }
     for (int s = 0; s < n; ++s) {
         const vla_prog_stage& a = st[s];
         if (!a.x_bf16 || !a.linears) return VLA_ERR_NULL;
@@ -115,12 +163,99 @@ Layout layout_of(const vla_prog_stage* st, int n) {
     return L;
 }
 
+
+vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_dev, size_t prog_bytes, void* stream) {
+    using vla::LpStage;
+    using vla::DevLProg;
+    const LLayout L = llayout_of(stages, n_stages);
+    if (prog_bytes < L.total) return VLA_ERR_WORKSPACE;
+    int dev = 0, sms = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return VLA_ERR_ARCH;
+    }
+    if (major != 10 || sms < 1) return VLA_ERR_ARCH;
+    uint8_t* base = reinterpret_cast<uint8_t*>(prog_dev);
+    std::vector<uint8_t> host(L.off_xq[0] + 64, 0);
+    // LpStage is 64-byte aligned (tensor maps): place the table at a 64-byte aligned HOST address with the same offsets
+    uint8_t* h = host.data() + ((64 - (reinterpret_cast<uintptr_t>(host.data()) & 63u)) & 63u);
+    DevLProg* P = reinterpret_cast<DevLProg*>(h);
+    LpStage* S = reinterpret_cast<LpStage*>(h + L.off_stages);
+    P->magic = vla::LPROG_MAGIC;
+    P->n_stages = n_stages;
+    P->qdone = reinterpret_cast<unsigned*>(base + L.off_counters);
+    P->gdone = P->qdone + n_stages;
+    P->done = P->gdone + n_stages;
+    P->stages = reinterpret_cast<const LpStage*>(base + L.off_stages);
+    int KS = 2, max_tiles = 1, prev_user[2] = {-1, -1};
+    uint32_t x_tile = 0;
+    for (int s = 0; s < n_stages; ++s) {
+        const vla_prog_stage& a = stages[s];
+        LpStage& d = S[s];
+        int n_total = 0;
+        d.grp.n = a.n_linears;
+        d.grp.ct_begin[0] = 0;
+        for (int j = 0; j < a.n_linears; ++j) {
+            const vla_prog_linear& l = a.linears[j];
+            d.grp.packed[j] = reinterpret_cast<const uint8_t*>(l.packed);
+            d.grp.beta[j] = l.w_scale;
+            d.grp.out[j] = l.out;
+            d.grp.N[j] = l.N;
+            d.grp.dtype[j] = l.out_dtype;
+            d.grp.ct_begin[j + 1] = d.grp.ct_begin[j] + l.N / 128;
+            n_total += l.N;
+        }
+        d.x = reinterpret_cast<const uint4*>(a.x_bf16);
+        d.M = a.M;
+        d.K = a.K;
+        d.TN = vla::lg_pick_tn(a.M, n_total, sms, (a.K / 128) % 2 == 0);
+        if (vla::lg_pick_ks(d.TN, a.K) != 2) KS = 1;
+        x_tile = std::max(x_tile, ((uint32_t)d.TN * 128u + 1023u) & ~1023u);
+        d.tiles_n = n_total / 128;
+        d.ntiles = d.tiles_n * ((a.M + d.TN - 1) / d.TN);
+        max_tiles = std::max(max_tiles, d.ntiles);
+        d.inv_nvec = (uint32_t)((0x100000000ull + (unsigned)(a.K / 8) - 1u) / (unsigned)(a.K / 8));
+        const int b = s & 1;                                  // scratch pair of the stage
+        d.xq = a.xq_opt ? a.xq_opt : reinterpret_cast<int8_t*>(base + L.off_xq[b]);
+        d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + L.off_xs[b]);
+        d.wait_stage = std::max((s > 0 && a.depends) ? s - 1 : -1, prev_user[b]);
+        prev_user[b] = s;
+        d.pad = 0;
+        if (vla::lg_encode_x_map(d.tmap, d.xq, a.M, a.K, d.TN) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+    }
+    const int stride = KS * (vla::LG_A_BYTES + (int)x_tile);
+    const int sw_bytes = vla::LG_SW * KS * vla::LG_W_BYTES;
+    int NS = (vla::LG_STAGE_REGION + vla::LG_SW * vla::LG_W_BYTES - sw_bytes) / stride;
+    if (NS > vla::LG_NS_MAX) NS = vla::LG_NS_MAX;
+    if (NS < 2) return VLA_ERR_SHAPE;
+    P->KS = KS;
+    P->NS = NS;
+    P->x_tile = x_tile;
+    P->smem_bytes = NS * stride + sw_bytes + vla::LG_SCALE_BYTES + 1024 + 8 * vla::LG_NBAR + 16 + vla::LP_EXTRA_SMEM;
+    int grid = max_tiles < sms ? max_tiles : sms;
+    {   // the CTAs wait for each other: all of them must be resident at once
+        int per_sm = 0;
+        if (vla::lprogram_max_ctas_per_sm(KS, P->smem_bytes, &per_sm) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+        if (per_sm < 1) return VLA_ERR_CUDA;
+        if (grid > per_sm * sms) grid = per_sm * sms;
+    }
+    cudaStream_t cs = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(prog_dev, h, L.off_xq[0], cudaMemcpyHostToDevice, cs);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
+    if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_programs[prog_dev] = ProgInfo{grid, n_stages, 0, DevProg{}, true, *P};
+    return VLA_OK;
+}
+
 }  // namespace
 
 extern "C" {
 
 size_t vla_program_bytes(const vla_prog_stage* stages, int n_stages) {
     if (check_stages(stages, n_stages) != VLA_OK) return 0;
+    if (is_large(stages)) return llayout_of(stages, n_stages).total;
     return layout_of(stages, n_stages).total;
 }
 
@@ -129,6 +264,7 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     if (st != VLA_OK) return st;
     if (!prog_dev) return VLA_ERR_NULL;
     if (reinterpret_cast<uintptr_t>(prog_dev) & 255u) return VLA_ERR_ALIGN;
+    if (is_large(stages)) return build_large(stages, n_stages, prog_dev, prog_bytes, stream);
     const Layout L = layout_of(stages, n_stages);
     if (prog_bytes < L.total) return VLA_ERR_WORKSPACE;
     int dev = 0, sms = 0, major = 0;
@@ -309,7 +445,7 @@ vla_status vla_program_build(const vla_prog_stage* stages, int n_stages, void* p
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     std::lock_guard<std::mutex> lk(g_mu);
-    g_programs[prog_dev] = ProgInfo{grid, n_stages, max_m, *P};
+    g_programs[prog_dev] = ProgInfo{grid, n_stages, max_m, *P, false, vla::DevLProg{}};
     return VLA_OK;
 }
 
@@ -322,7 +458,8 @@ vla_status vla_program_run(const void* prog_dev, void* stream) {
         if (it == g_programs.end()) return VLA_ERR_VALUE;
         info = it->second;
     }
-    cudaError_t e = vla::launch_program(info.header, info.grid, info.max_m, (cudaStream_t)stream);
+    cudaError_t e = info.large ? vla::launch_lprogram(info.lheader, info.grid, (cudaStream_t)stream)
+                               : vla::launch_program(info.header, info.grid, info.max_m, (cudaStream_t)stream);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     return VLA_OK;
 }

@@ -149,6 +149,24 @@ __device__ __forceinline__ void mma_m16n8k32_s8(int (&c)[4], uint32_t a0, uint32
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// ---------------------------------------------------------------- grid-wide counters of the persistent kernels
+__device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// A CTA that never becomes resident (the grid is sized for co-residency at build time, but the device may be shared)
+// would make this spin forever: after ~2 s the kernel traps, so a hang becomes a launch error (VLA_ERR_CUDA).
+__device__ __forceinline__ void spin_until(const unsigned* p, unsigned target) {
+    const long long t0 = clock64();
+    while (ld_acquire_gpu(p) < target) {
+        if (clock64() - t0 > (1ll << 32)) __trap();
+    }
+}
+__device__ __forceinline__ void red_release_gpu(unsigned* p, unsigned v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+
 // ---------------------------------------------------------------- dequant epilogue, Eq. 4 line 3
 // canonical order (reading R6): s = alpha_m * beta (one fp32 multiply), y = (float)acc * s.
 __device__ __forceinline__ float dequant(int acc, float s) { return __fmul_rn(__int2float_rn(acc), s); }

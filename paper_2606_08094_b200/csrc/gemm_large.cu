@@ -18,27 +18,10 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include "common.cuh"
+#include "gemm_large.cuh"
 #include "kernels.h"
 
 namespace vla {
-
-constexpr int LG_THREADS = 15 * 32;
-constexpr int LG_SW = 6;                                // packed-weight stages (4 KiB each)
-constexpr int LG_NS_MAX = 8;                            // {decoded A, X} stages
-constexpr int LG_A_BYTES = TILE_N * TILE_K;             // 16384 decoded int8
-constexpr int LG_W_BYTES = TILE_BYTES;                  // 4096 packed
-constexpr int LG_STAGE_REGION = 192 * 1024;             // 4 stages at TN = 256, 6 at TN = 96
-constexpr int LG_SCALE_BYTES = 4 * 256 * 4;             // per epilogue warp: alpha_m * beta of the tile's tokens
-constexpr int LG_NBAR = 2 * LG_SW + 2 * LG_NS_MAX + 4;
-constexpr int LG_FIXED_SMEM = LG_SW * LG_W_BYTES + LG_SCALE_BYTES + 1024 /*align*/ + 8 * LG_NBAR + 16;
-
-__host__ __device__ inline uint32_t lg_stage_stride(int TN) { return LG_A_BYTES + (((uint32_t)TN * TILE_K + 1023u) & ~1023u); }
-
-__device__ __forceinline__ uint4 lds128_nv(uint32_t addr) {
-    uint4 r;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
-    return r;
-}
 
 // KS = k blocks (of 128) per pipeline stage: 2 for token tiles <= 160 (eight MMAs per full/empty handoff), else 1.
 template <int KS>
@@ -295,7 +278,7 @@ static EncodeTiledFn get_encode() {
 // Measured on B200 (profiles/): a k block costs ~540 cycles at TN = 96 and ~610 at TN = 256 -- the shared-memory
 // traffic of decode + operand fetch dominates, not the 2*TN cycles of the MMAs -- so cycles ~ 500 + 0.42*TN.
 // Ties go to the wider tile (fewer re-decodes of the same weights).
-static int pick_tn(int M, int N, int sms, bool k_even) {
+int lg_pick_tn(int M, int N, int sms, bool k_even) {
     int best = 16;
     double best_cost = 1e30;
     for (int tn = 16; tn <= 256; tn += 16) {
@@ -311,25 +294,32 @@ static int pick_tn(int M, int N, int sms, bool k_even) {
     return best;
 }
 
-cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const float* x_scale, int M, int K,
-                                      cudaStream_t s) {
-    const int N = g.ct_begin[g.n] * TILE_N;                  // all channels of the group
+// tensor map of the int8 activations xq [M,K]: box = [128 k, TN tokens], SWIZZLE_128B (operand B of the MMA)
+cudaError_t lg_encode_x_map(void* tmap_out, const int8_t* xq, int M, int K, int TN) {
     EncodeTiledFn enc = get_encode();
     if (!enc) return cudaErrorNotSupported;
-    int dev = 0, sms = 0;                                    // per call: a process may drive several devices
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-        return cudaErrorInvalidDevice;
-    const int TN = pick_tn(M, N, sms, (K / TILE_K) % 2 == 0);
-
-    CUtensorMap tm;
     cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)M};
     cuuint64_t gstr[1] = {(cuuint64_t)K};
     cuuint32_t box[2] = {(cuuint32_t)TILE_K, (cuuint32_t)TN};
     cuuint32_t estr[2] = {1, 1};
-    CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, (void*)xq, gdim, gstr, box, estr,
+    CUresult r = enc(reinterpret_cast<CUtensorMap*>(tmap_out), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, (void*)xq, gdim, gstr, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const float* x_scale, int M, int K,
+                                      cudaStream_t s) {
+    const int N = g.ct_begin[g.n] * TILE_N;                  // all channels of the group
+    int dev = 0, sms = 0;                                    // per call: a process may drive several devices
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+        return cudaErrorInvalidDevice;
+    const int TN = lg_pick_tn(M, N, sms, (K / TILE_K) % 2 == 0);
+    CUtensorMap tm;
+    {
+        const cudaError_t e = lg_encode_x_map(&tm, xq, M, K, TN);
+        if (e != cudaSuccess) return e;
+    }
 
     {   // function attributes are per device: set on every launch (cheap), no process-wide cache
         cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
@@ -339,7 +329,7 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     const int ntiles = (N / TILE_N) * ((M + TN - 1) / TN);
     // narrow token tiles: two k blocks per stage (the MMAs of a 128 x TN x 32 step have a 31 ns floor for TN <= 112,
     // so four of them do not cover one full/empty handoff; eight do)
-    const int KS = (TN <= 160 && (K / TILE_K) % 2 == 0) ? 2 : 1;
+    const int KS = lg_pick_ks(TN, K);
     const int stage = KS * (int)lg_stage_stride(TN);
     const int sw_bytes = LG_SW * KS * LG_W_BYTES;
     int NS = (LG_STAGE_REGION + LG_SW * LG_W_BYTES - sw_bytes) / stage;

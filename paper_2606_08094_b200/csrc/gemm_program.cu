@@ -59,19 +59,6 @@ __device__ __forceinline__ void team_bar(int team) {
     asm volatile("bar.sync %0, %1;" :: "r"(2 + team), "n"(PG_TW * 32) : "memory");
 }
 
-__device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned* p) {
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-// A CTA that never becomes resident (the grid is sized for co-residency at build time, but the device may be shared)
-// would make this spin forever: after ~2 s the kernel traps, so a hang becomes a launch error (VLA_ERR_CUDA).
-__device__ __forceinline__ void spin_until(const unsigned* p, unsigned target) {
-    const long long t0 = clock64();
-    while (ld_acquire_gpu(p) < target) {
-        if (clock64() - t0 > (1ll << 32)) __trap();
-    }
-}
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 r;
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr) : "memory");
@@ -92,9 +79,6 @@ __device__ __forceinline__ void red_shared_add(uint32_t addr, int v) {
     asm volatile("red.shared.add.s32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
 }
 // publish: every store this CTA made before the preceding consumer_bar() becomes visible before the count does
-__device__ __forceinline__ void red_release_gpu(unsigned* p, unsigned v) {
-    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
-}
 // non-volatile form: the compiler may interleave it with the decode of the next block
 __device__ __forceinline__ void mma_m16n8k32_s8_nv(int (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
                                                    uint32_t b0, uint32_t b1) {

@@ -82,6 +82,21 @@ __device__ __forceinline__ uint4 quant16(uint4 a, uint4 b, float4 sc) {      // 
     if (diff != 0u) o = quant16_patch(a, b, sc, o);          // rare: a rounding boundary is too close
     return o;
 }
+// the same for one vector of 8 (stand-alone act_quant kernel)
+static __device__ __noinline__ uint2 quant8_patch(uint4 a, float4 sc, uint2 o) {
+    o.x = patch2(a.y, patch2(a.x, o.x, 0, sc), 16, sc);
+    o.y = patch2(a.w, patch2(a.z, o.y, 0, sc), 16, sc);
+    return o;
+}
+__device__ __forceinline__ uint2 quant8_fast(uint4 a, float4 sc) {
+    const float2 ilo = make_float2(sc.y, sc.y), ihi = make_float2(sc.z, sc.z);
+    uint32_t diff = 0;
+    uint2 o;
+    o.x = quant4_fast(a.x, a.y, ilo, ihi, diff);
+    o.y = quant4_fast(a.z, a.w, ilo, ihi, diff);
+    if (diff != 0u) o = quant8_patch(a, sc, o);
+    return o;
+}
 // absmax of 8 bf16 as a packed pair of 15-bit magnitudes (bf16 magnitudes order like unsigned integers)
 __device__ __forceinline__ uint32_t absmax8_packed(uint4 v, uint32_t m) {
     m = __vmaxu2(m, v.x & 0x7FFF7FFFu);
@@ -90,6 +105,9 @@ __device__ __forceinline__ uint32_t absmax8_packed(uint4 v, uint32_t m) {
     m = __vmaxu2(m, v.w & 0x7FFF7FFFu);
     return m;
 }
+
+// the larger half of a packed absmax pair as fp32
+__device__ __forceinline__ float absmax_unpack(uint32_t m) { return fmaxf(bf16lo(m), bf16hi(m)); }
 
 // {alpha, 1/alpha * (1 - 2^-19), 1/alpha * (1 + 2^-19), -}
 __device__ __forceinline__ float4 quant_scales_of_alpha(float alpha) {

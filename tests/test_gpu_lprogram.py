@@ -1,0 +1,155 @@
+"""GPU parity tests (-m gpu) of LARGE programs (vla_program_build / vla_program_run with M > 16 tokens per stage): the
+persistent tcgen05 kernel of csrc/gemm_lprog.cu -- activation quant fused into the launch (rows quantised cooperatively
+by the CTAs, grid-wide counters), stages chained without leaving the kernel -- against the CPU oracle.  Every output is
+compared element by element and is bit-identical (canonical operation order, R1, R6).
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_08094_b200 import synth
+from test_gpu_program import bits, check_point, dev, dev_bf16, make_point, oracle_stack, stage_of, vla  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("M,K,N", [(17, 128, 128), (32, 256, 256), (100, 640, 384), (200, 2560, 640), (544, 2560, 2560),
+                                   (545, 6912, 2560), (1000, 2560, 6912), (2500, 1024, 256), (333, 8192, 128)])
+@pytest.mark.parametrize("dtype", [0, 1, 2])
+def test_single_stage_large_program(vla, oracle, M, K, N, dtype):
+    """one linear per program: token tiles of 32..256, one and two k blocks per pipeline stage, ragged M, one to several
+    waves of tiles, 1..28 rows per CTA in the fused quantiser (several rounds), every output type; also the optional
+    xq / alpha outputs"""
+    p = make_point(vla, M, K, N, 9100 + M + K + N, dtype, want_xq=True)
+    prog = vla.compile_program([stage_of(p)])
+    vla.vla_program_run(prog)
+    torch.cuda.synchronize()
+    check_point(vla, oracle, p)
+    vla.vla_program_release(prog)
+
+
+def test_grouped_stage_mixed_dtypes_scratch_activations(vla, oracle):
+    """one stage, three linears with their own beta and output type (Eq. 4's per-output-group scales), ragged M=545,
+    quantised activations kept in the program's scratch (no xq_opt)"""
+    M, K = 545, 2560
+    x = synth.activations(M, K, 9301, outlier_frac=0.01)
+    lins, refs = [], []
+    for j, (N, dt) in enumerate([(2560, vla.VLA_BF16), (640, vla.VLA_F32), (640, vla.VLA_I32)]):
+        p = make_point(vla, M, K, N, 9310 + j, dt)
+        p["x_bits"], p["x"] = x, None
+        lins.append(p)
+    xd = dev_bf16(x)
+    stage = dict(x=xd, M=M, K=K, depends=0,
+                 linears=[dict(packed=p["packed"], w_scale=p["beta_d"], out=p["out"], N=p["N"], out_dtype=p["dtype"]) for p in lins])
+    prog = vla.compile_program([stage])
+    for rep in range(3):
+        for p in lins:
+            p["out"].fill_(-5)
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        for p in lins:
+            check_point(vla, oracle, p)
+    vla.vla_program_release(prog)
+
+
+def test_independent_stages_alternate_scratch_and_rerun(vla, oracle):
+    """seven independent stages of different M, K, N in one launch (the two scratch pairs alternate; the token tile and the
+    reserved X tile differ per stage), run three times and once from a CUDA graph: the counters reset themselves"""
+    shapes = [(64, 2560, 640), (544, 640, 1280), (200, 6912, 256), (17, 256, 128), (1024, 1280, 384), (96, 8192, 256),
+              (300, 384, 2560)]
+    pts = [make_point(vla, M, K, N, 9400 + i, [1, 0, 2][i % 3]) for i, (M, K, N) in enumerate(shapes)]
+    prog = vla.compile_program([stage_of(p) for p in pts])
+    for rep in range(3):
+        for p in pts:
+            p["out"].fill_(-3)
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        for p in pts:
+            check_point(vla, oracle, p)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        vla.vla_program_run(prog)
+        vla.vla_program_run(prog)
+    for p in pts:
+        p["out"].fill_(-3)
+    g.replay()
+    torch.cuda.synchronize()
+    for p in pts:
+        check_point(vla, oracle, p)
+    vla.vla_program_release(prog)
+
+
+def test_chained_stack_m544_one_launch(vla, oracle):
+    """configs[3] at M=544 as ONE launch: 3 full-size layers = 12 dependent stages (q|k|v as one N=3840 group, gate|up as
+    N=13824), quantisation fused, free-running; every intermediate of every layer bit-identical to the oracle's chain.
+    Run twice (stale activations of the first run are still in the scratch and in L2 during the second)."""
+    from paper_2606_08094_b200.stack import Stack
+    layers, M = 3, synth.PREFILL_M
+    weights = [synth.stack_layer(l) for l in range(layers)]
+    x = synth.stack_input(M)
+    st = Stack(layers, M, weights=weights)
+    st.set_input(x)
+    st.compile()
+    ref = oracle_stack(oracle, weights, x)
+    for rep in range(2):
+        st.run_program()
+        torch.cuda.synchronize()
+        for l in range(layers):
+            for n in ref[l]:
+                assert np.array_equal(bits(st.out[l][n]), ref[l][n]), "layer %d %s differs (rep %d)" % (l, n, rep)
+                st.out[l][n].zero_()
+
+
+def test_chained_large_program_changing_inputs(vla, oracle):
+    """a dependent pair (stage 1 reads stage 0's bf16 output) re-run with NEW inputs in the same buffers: a stale row in an
+    SM's L1 or a stale alpha would show"""
+    M, K, N1, N2 = 130, 640, 1280, 256
+    a = make_point(vla, M, K, N1, 9500, vla.VLA_BF16)
+    b = make_point(vla, M, N1, N2, 9510, vla.VLA_F32)
+    st0 = stage_of(a)
+    st1 = dict(stage_of(b), x=a["out"], depends=1)
+    prog = vla.compile_program([st0, st1])
+    for rep in range(3):
+        x = synth.activations(M, K, 9520 + rep, outlier_frac=0.01)
+        a["x"].copy_(dev_bf16(x))
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        r0 = oracle.ternary_linear(x, a["w"], a["beta"])
+        assert np.array_equal(bits(a["out"]), r0["ybf16"])
+        r1 = oracle.ternary_linear(r0["ybf16"], b["w"], b["beta"])
+        assert np.array_equal(b["out"].cpu().numpy().view(np.uint32), r1["y32"].view(np.uint32))
+    vla.vla_program_release(prog)
+
+
+def test_large_program_guard_bands(vla, oracle):
+    """nothing is written outside [M,N] / [M,K] / [M]: outputs and the optional xq / alpha live inside guarded buffers"""
+    M, K, N = 77, 384, 256
+    p = make_point(vla, M, K, N, 9600, vla.VLA_F32)
+    G = 512
+    out = torch.full((M * N + 2 * G,), 1234.5, dtype=torch.float32, device="cuda")
+    xq = torch.full((M * K + 2 * G,), 55, dtype=torch.int8, device="cuda")
+    xs = torch.full((M + 2 * G,), -9.0, dtype=torch.float32, device="cuda")
+    p["out"] = out[G:G + M * N].view(M, N)
+    p["xq"] = xq[G:G + M * K].view(M, K)
+    p["xs"] = xs[G:G + M]
+    prog = vla.compile_program([stage_of(p)])
+    vla.vla_program_run(prog)
+    torch.cuda.synchronize()
+    check_point(vla, oracle, p)
+    for t, v in ((out, 1234.5), (xq, 55), (xs, -9.0)):
+        n = t.numel()
+        inner = {id(out): M * N, id(xq): M * K, id(xs): M}[id(t)]
+        assert bool((t[:G] == v).all()) and bool((t[G + inner:n] == v).all())
+    vla.vla_program_release(prog)
+
+
+def test_large_program_errors(vla):
+    small = make_point(vla, 8, 256, 256, 5, vla.VLA_BF16)
+    large = make_point(vla, 64, 256, 256, 6, vla.VLA_BF16)
+    assert vla.vla_program_bytes([stage_of(small), stage_of(large)]) == 0          # one kind per program
+    assert vla.vla_program_bytes([dict(stage_of(large), M=32769)]) == 0
+    assert vla.vla_program_bytes([dict(stage_of(large), K=8192 + 128)]) == 0
+    nine = stage_of(large)
+    nine["linears"] = nine["linears"] * 9
+    assert vla.vla_program_bytes([nine]) == 0                                      # at most 8 linears per large stage
+    assert vla.vla_program_bytes([stage_of(large)]) > 0

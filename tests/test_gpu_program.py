@@ -241,8 +241,10 @@ def test_full_depth_stack_m8_one_launch(vla, oracle):
 
 def test_program_errors(vla):
     p = make_point(vla, 8, 256, 256, 5, vla.VLA_BF16)
-    bad_m = dict(stage_of(p), M=17)
+    bad_m = dict(stage_of(p), M=0)
     assert vla.vla_program_bytes([bad_m]) == 0
+    mixed = [stage_of(p), dict(stage_of(p), M=17)]      # M > 16 is a LARGE program (test_gpu_lprogram.py): one kind per program
+    assert vla.vla_program_bytes(mixed) == 0
     bad_k = dict(stage_of(p), K=8192 + 128)
     assert vla.vla_program_bytes([bad_k]) == 0
     with pytest.raises(vla.VlaError) as e:

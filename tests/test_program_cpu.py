@@ -29,10 +29,21 @@ def test_program_bytes_counts_tables_counters_and_cooperative_scratch(vla):
     assert one + 8 * 6912 <= two < one + 8 * 6912 + 1024
 
 
-@pytest.mark.parametrize("bad", [dict(M=0), dict(M=17), dict(K=100), dict(K=8192 + 128), dict(N=100), dict(N=0),
+@pytest.mark.parametrize("bad", [dict(M=0), dict(M=32769), dict(M=64, n=9), dict(M=64, K=8192 + 128), dict(K=100), dict(K=8192 + 128), dict(N=100), dict(N=0),
                                  dict(depends=2), dict(n=0), dict(n=17), dict(dtype=3)])
 def test_invalid_stage_gives_zero_bytes(vla, bad):
     assert vla.vla_program_bytes([stage(**bad)]) == 0
+
+
+def test_one_kind_per_program_and_large_program_bytes(vla):
+    """stages with M > 16 tokens form a LARGE program (persistent tcgen05 kernel): not mixable with small stages; its
+    buffer holds the stage table (tensor map + group per stage), the counters and two {int8 [M,K], alpha [M]} scratch pairs"""
+    assert vla.vla_program_bytes([stage(M=8), stage(M=64)]) == 0
+    assert vla.vla_program_bytes([stage(M=64), stage(M=16)]) == 0
+    one = vla.vla_program_bytes([stage(M=544)])
+    assert one % 256 == 0 and 2 * 544 * 2560 <= one < 2 * 544 * 2560 + 16384
+    two = vla.vla_program_bytes([stage(M=544), stage(M=100, K=6912, depends=1, n=2)])
+    assert 2 * 544 * 2560 <= two < 2 * 544 * 2560 + 16384 and two > one
 
 
 def test_descriptor_capacity_is_enforced(vla):
