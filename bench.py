@@ -52,7 +52,7 @@ def workload_name(workload):
     """`config.workload` of the JSON line -- the same string for the B200 arm and the reference arm."""
     if workload == "decode":
         return "configs[1] decode: 4 BitNet-2B linears x M in {1,8,16}, fused quant, bf16 out (B200 arm: one persistent program launch per step)"
-    return "configs[2] prefill: 4 BitNet-2B linears at M=544, fused quant, fp32 out"
+    return "configs[2] prefill: 4 BitNet-2B linears at M=544, fused quant, fp32 out (B200 arm: one persistent tcgen05 program launch per step)"
 
 
 def out_elem_bytes(workload):
@@ -293,9 +293,10 @@ class GpuWorkload:
                 xq=torch.empty((M, K), dtype=torch.int8, device=device),
                 xs=torch.empty((M,), dtype=torch.float32, device=device),
                 ws=torch.empty(ws_bytes, dtype=torch.uint8, device=device), ws_bytes=ws_bytes))
-        # decode: the 12 points of a step are one compiled program per ring position (one persistent launch)
+        # the points of a step are one compiled program per ring position: ONE persistent launch per step
+        # (decode: program_kernel, M <= 16; prefill: lprog_kernel, tcgen05, activation quant fused into the launch)
         self.programs = []
-        if workload == "decode":
+        if workload in ("decode", "prefill"):
             for step in range(self.rev_steps):
                 stages = [dict(x=b["x"], M=b["M"], K=b["K"], depends=0,
                                linears=[dict(packed=self.ring[b["si"]][self.slot(step, pi)], w_scale=self.beta[b["si"]],
@@ -316,7 +317,7 @@ class GpuWorkload:
     def launch_point(self, pi, step, mode="linear"):
         b, vla = self.buf[pi], self.vla
         packed = self.ring[b["si"]][self.slot(step, pi)]
-        if mode == "linear":          # the whole hot path: quant fused into the call
+        if mode in ("linear", "calls"):   # the whole hot path as single calls: quant kernel + GEMM kernel per linear
             vla.vla_ternary_linear(packed, self.beta[b["si"]], b["x"], b["M"], b["N"], b["K"], b["out"], self.out_dtype,
                                    vla.VLA_PATH_AUTO, b["xq"], b["xs"], b["ws"], b["ws_bytes"])
         elif mode == "gemm":          # the dominant kernel alone, on pre-quantised activations
@@ -375,6 +376,7 @@ def run_gpu(args):
     for s in range(max(args.warmup, 3)):
         wl.launch_step(s)
         if args.workload != "decode":
+            wl.launch_step(s, "calls")
             wl.launch_step(s, "gemm")
     torch.cuda.synchronize()
 
@@ -424,18 +426,12 @@ def run_gpu(args):
 
     # ---- roofline of the dominant kernel (the GEMM), timed alone on pre-quantised activations, cold ring
     pk = peaks()
-    if args.workload != "decode":
-        g_gemm, n_gemm = wl.capture(list(range(rev)), "gemm")
-        time_replays(torch, [g_gemm] * 2)
-        reps_g = max(3, min(200, int(2e5 / max(1, n_gemm))))
-        gemm_ms = time_replays(torch, [g_gemm] * reps_g) / reps_g
-        per_launch_s = gemm_ms * 1e-3 / n_gemm
+    # the dominant (only) kernel of the step is the persistent program kernel: one launch = one step
+    g_one, n_one = wl.capture(list(range(rev)))
+    time_replays(torch, [g_one] * 2)
+    reps = max(3, min(200, int(4000 / max(1, rev))))
+    per_launch_s = time_replays(torch, [g_one] * reps) * 1e-3 / (reps * n_one)
     if args.workload == "decode":
-        # the dominant (only) kernel of the step is the persistent program kernel: one launch = one step
-        g_one, n_one = wl.capture(list(range(rev)))
-        time_replays(torch, [g_one] * 2)
-        reps = max(3, min(200, int(4000 / max(1, rev))))
-        per_launch_s = time_replays(torch, [g_one] * reps) * 1e-3 / (reps * n_one)
         alg = float(wl.step_bytes)                            # algorithmic bytes of one launch
         achieved = alg / per_launch_s / 1e9
         roof = {"bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
@@ -444,17 +440,29 @@ def run_gpu(args):
                 "alg_bytes_per_launch": alg, "us_per_launch": per_launch_s * 1e6,
                 "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
     else:
-        alg = wl.step_ops / len(wl.buf)
+        alg = float(wl.step_ops)                              # one launch = the four linears of the step, Eq. 4 end to end
         achieved = alg / per_launch_s / 1e12
         peak_i8 = pk["bf16_tflops"] * 2.0                     # int8 : bf16 = 4.5 : 2.25 nominal
+        probe = int8_probe_tops(vla)                          # tcgen05.mma.kind::i8 issue-rate ceiling of this box
         roof = {"bound": "tensor", "achieved": achieved, "peak": peak_i8, "unit": "TOP/s",
-                "frac": achieved / peak_i8, "traffic": ncu_traffic("gemm_large"),
-                "kernel": "gemm_large_kernel", "peak_source": pk["source"] + " bf16_tflops x 2 (int8:bf16 nominal ratio)",
+                "frac": achieved / peak_i8, "traffic": ncu_traffic("lprog_kernel"),
+                "kernel": "lprog_kernel", "peak_source": pk["source"] + " bf16_tflops x 2 (int8:bf16 nominal ratio)",
                 "alg_ops_per_launch": alg, "us_per_launch": per_launch_s * 1e6,
-                "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS}
-        probe = int8_probe_tops(vla)
-        roof["int8_probe_tops"] = probe                       # tcgen05.mma.kind::i8 issue-rate ceiling of this box
-        roof["frac_of_probe"] = achieved / probe
+                "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS, "int8_probe_tops": probe,
+                "frac_of_probe": achieved / probe}
+        # beside it: the same step as single calls (quant kernel + GEMM kernel per linear, CUDA graph + PDL), and the GEMM
+        # kernel alone on pre-quantised activations
+        g_calls, n_calls = wl.capture(list(range(rev)), "calls")
+        time_replays(torch, [g_calls] * 2)
+        calls_s = time_replays(torch, [g_calls] * 20) * 1e-3 / (20 * rev)
+        g_gemm, n_gemm = wl.capture(list(range(rev)), "gemm")
+        time_replays(torch, [g_gemm] * 2)
+        gemm_s = time_replays(torch, [g_gemm] * 20) * 1e-3 / (20 * n_gemm)
+        a_g = wl.step_ops / len(wl.buf) / gemm_s / 1e12
+        roof["single_calls"] = {"us_per_step": calls_s * 1e6, "launches_per_step": n_calls // rev,
+                                "TOPS": wl.step_ops / calls_s / 1e12, "frac": wl.step_ops / calls_s / 1e12 / peak_i8}
+        roof["gemm_only"] = {"kernel": "gemm_large_kernel", "us_per_launch": gemm_s * 1e6, "achieved": a_g,
+                             "frac": a_g / peak_i8, "frac_of_probe": a_g / probe, "traffic": ncu_traffic("gemm_large")}
 
     # ---- per-point table (the metric is "vs M"): each point alone, whole hot path, cold ring
     table = []
@@ -478,7 +486,9 @@ def run_gpu(args):
         import bench_workloads as bw
         vs_m, roof_tensor = bw.run_vs_m(pk, int8_probe_tops(vla))
         if roof_tensor is not None:
-            roof_tensor["traffic"] = ncu_traffic("gemm_large")
+            roof_tensor["traffic"] = ncu_traffic("lprog_kernel_x%d" % 12)
+            if roof_tensor.get("gemm_only"):
+                roof_tensor["gemm_only"]["traffic"] = ncu_traffic("gemm_large")
 
     attn = None
     if args.workload == "decode" and not args.no_vs_m:
@@ -509,7 +519,7 @@ def run_gpu(args):
                    "value_is": ("algorithmic HBM GB/s of the configs[1] decode step (the M <= 16 half of the metric); both halves "
                                 "per (shape, M) are in vs_M, the dominant kernel of the M >= 512 half in roofline_tensor")
                    if args.workload == "decode" else "algorithmic HBM GB/s of the configs[2] prefill step; TOPS beside it",
-                   "launch": ("CUDA graphs of %d program launches" if args.workload == "decode" else "CUDA graphs of %d steps + PDL") % rev, "parallelism": "replicas" if world > 1 else "single"},
+                   "launch": "CUDA graphs of %d program launches" % rev, "parallelism": "replicas" if world > 1 else "single"},
         "clocks": clocks, "gpu_launches": launches,
         "e2e": {"value": e2e_bytes / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": wl.h2d,
                 "d2h_bytes_per_step": wl.d2h, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},

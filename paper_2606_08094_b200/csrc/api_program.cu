@@ -87,7 +87,11 @@ vla_status check_large(const vla_prog_stage* st, int n) {
     return VLA_OK;
 }
 
-struct LLayout { size_t off_stages, off_counters, off_xq[2], off_xs[2], total; };
+#ifndef VLA_LP_NSCRATCH
+#define VLA_LP_NSCRATCH 4
+#endif
+constexpr int LP_NSCRATCH = VLA_LP_NSCRATCH;      // {int8 [M,K], alpha [M]} scratch sets: the quantiser runs up to three stages ahead
+struct LLayout { size_t off_stages, off_counters, off_xq[LP_NSCRATCH], off_xs[LP_NSCRATCH], off_stamps, total; };
 
 LLayout llayout_of(const vla_prog_stage* st, int n) {
     LLayout L{};
@@ -99,8 +103,11 @@ LLayout llayout_of(const vla_prog_stage* st, int n) {
     size_t o = round256(sizeof(vla::DevLProg));
     L.off_stages = o;   o += round256(sizeof(vla::LpStage) * (size_t)n);
     L.off_counters = o; o += round256(sizeof(unsigned) * (2 * (size_t)n + 1));
-    for (int b = 0; b < 2; ++b) { L.off_xq[b] = o; o += round256(max_xq); }
-    for (int b = 0; b < 2; ++b) { L.off_xs[b] = o; o += round256(4 * max_m); }
+    for (int b = 0; b < LP_NSCRATCH; ++b) { L.off_xq[b] = o; o += round256(max_xq); }
+    for (int b = 0; b < LP_NSCRATCH; ++b) { L.off_xs[b] = o; o += round256(4 * max_m); }
+#ifdef VLA_LP_STAMPS
+    L.off_stamps = o;   o += round256(sizeof(unsigned long long) * 8 * 160 * (size_t)n);
+#endif
     L.total = o;
     return L;
 }
@@ -188,7 +195,14 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
     P->gdone = P->qdone + n_stages;
     P->done = P->gdone + n_stages;
     P->stages = reinterpret_cast<const LpStage*>(base + L.off_stages);
-    int KS = 2, max_tiles = 1, prev_user[2] = {-1, -1};
+#ifdef VLA_LP_STAMPS
+    P->stamps = reinterpret_cast<unsigned long long*>(base + L.off_stamps);
+    fprintf(stderr, "lprog stamps at offset %zu\n", L.off_stamps);
+#else
+    P->stamps = nullptr;
+#endif
+    int KS = 2, max_tiles = 1, prev_user[LP_NSCRATCH];
+    for (int b = 0; b < LP_NSCRATCH; ++b) prev_user[b] = -1;
     uint32_t x_tile = 0;
     for (int s = 0; s < n_stages; ++s) {
         const vla_prog_stage& a = stages[s];
@@ -216,7 +230,7 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         d.ntiles = d.tiles_n * ((a.M + d.TN - 1) / d.TN);
         max_tiles = std::max(max_tiles, d.ntiles);
         d.inv_nvec = (uint32_t)((0x100000000ull + (unsigned)(a.K / 8) - 1u) / (unsigned)(a.K / 8));
-        const int b = s & 1;                                  // scratch pair of the stage
+        const int b = s % LP_NSCRATCH;                        // scratch set of the stage
         d.xq = a.xq_opt ? a.xq_opt : reinterpret_cast<int8_t*>(base + L.off_xq[b]);
         d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + L.off_xs[b]);
         d.wait_stage = std::max((s > 0 && a.depends) ? s - 1 : -1, prev_user[b]);
@@ -244,6 +258,11 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
     cudaError_t e = cudaMemcpyAsync(prog_dev, h, L.off_xq[0], cudaMemcpyHostToDevice, cs);
     if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+#ifdef VLA_LP_STAMPS
+    for (int s = 0; s < n_stages && s < 16; ++s)
+        fprintf(stderr, "lstage %d: M=%d K=%d TN=%d tiles %d (n %d) wait %d | KS %d NS %d x_tile %u grid %d\n", s, S[s].M, S[s].K,
+                S[s].TN, S[s].ntiles, S[s].tiles_n, S[s].wait_stage, KS, NS, x_tile, grid);
+#endif
     std::lock_guard<std::mutex> lk(g_mu);
     g_programs[prog_dev] = ProgInfo{grid, n_stages, 0, DevProg{}, true, *P};
     return VLA_OK;

@@ -1,7 +1,7 @@
 // gemm_lprog.cu -- LARGE programs: a list of stages with M > 16 tokens, each Eq. 4 end to end,
 // in ONE persistent tcgen05 launch (lprogram.h).  The per-stage work is gemm_large_kernel's (same tiles, same warp
 // roles, same pipeline); what is new is that the launch does not end between stages:
-//   * activation quant is FUSED: before a stage's tiles, the eight decode warps of every CTA quantise the rows
+//   * activation quant is FUSED: dedicated quantiser warps of every CTA (after gemm_large_kernel's 15) quantise the rows
 //     r = blockIdx.x, += gridDim.x of x into the stage's int8 matrix and its alpha vector (quant.cuh's exact fast
 //     quantiser), then the CTA counts itself in qdone[s]; the X producer (TMA) and the epilogue warps start the stage when
 //     qdone[s] == gridDim.x.  The packed weights of the stage are already streaming (they depend on nothing).
@@ -18,68 +18,129 @@
 
 namespace vla {
 
-constexpr int LP_QT = 256;                               // quantising threads: the eight decode warps
-constexpr int LP_QV = 6;                                 // vectors of 8 bf16 a thread holds per round
+#ifndef VLA_LP_QG
+#define VLA_LP_QG 1
+#endif
+#ifndef VLA_LP_QW
+#define VLA_LP_QW 8
+#endif
+#ifndef VLA_LP_QV
+#define VLA_LP_QV 6
+#endif
+constexpr int LP_QG = VLA_LP_QG;                         // quantiser groups (after the 15 warps of gemm_large_kernel): group i
+                                                         // takes the stages s = i (mod LP_QG), so LP_QG latency chains overlap
+constexpr int LP_QW = VLA_LP_QW;                         // warps per group
+constexpr int LP_QT = 32 * LP_QW;
+constexpr int LP_QV = VLA_LP_QV;                         // vectors of 8 bf16 a thread has in flight
+constexpr int LP_THREADS = LG_THREADS + LP_QG * LP_QT;
 constexpr int LP_QROWS = 16;                             // most rows per round
-static_assert(LP_EXTRA_SMEM == LP_QROWS * 4 + LP_QROWS * 16, "lprogram.h");
+static_assert(LP_QG == 1 && LP_EXTRA_SMEM == LP_QROWS * 4 + LP_QROWS * 16, "lprogram.h");
+
+#ifdef VLA_LP_STAMPS
+__device__ __forceinline__ unsigned long long lp_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+#define LP_STAMP(k) do { P.stamps[((size_t)sidx * gridDim.x + blockIdx.x) * 8 + (k)] = lp_now(); } while (0)
+#else
+#define LP_STAMP(k) do { } while (0)
+#endif
 
 __device__ __forceinline__ void lp_bar(int id, int threads) {
     asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(threads) : "memory");
 }
 
-// rows blockIdx.x, += gridDim.x of the stage's x -> int8 + alpha.  Flat tasks of one 8-element vector; a round covers as
-// many rows as fit LP_QT * LP_QV vectors, the vectors stay in registers between the absmax and the quantisation.
-__device__ __forceinline__ void lp_quant_stage(const LpStage& st, int tid, unsigned* s_rowmax, float4* s_scale) {
-    const int grid = (int)gridDim.x, cta = (int)blockIdx.x, nvec = st.K >> 3;
-    const int R = st.M > cta ? (st.M - cta + grid - 1) / grid : 0;
-    const int G = min(LP_QROWS, (LP_QT * LP_QV) / nvec);
-    uint2* __restrict__ xq = reinterpret_cast<uint2*>(st.xq);
-    for (int i0 = 0; i0 < R; i0 += G) {
-        const int g = min(G, R - i0), ntask = g * nvec;
+// rows blockIdx.x, += gridDim.x of the stage's x -> int8 + alpha, LP_QROWS rows at a time.  Flat tasks of one 8-element
+// vector over the chunk's rows, two streaming passes: absmax (loads only), then quantise (the same vectors again, now L2
+// hits).  Nothing is held in registers between the passes, so a chunk is two latency chains whatever K and M are.
+struct LpQuantArgs {           // the quantiser's view of a stage, read from the table BEFORE it waits for the stage's inputs
+    const uint4* x;
+    uint2* xq;
+    float* xs;
+    int M, nvec, wait_stage;
+    unsigned inv_nvec;
+};
+__device__ __forceinline__ LpQuantArgs lp_quant_args(const LpStage& st) {
+    LpQuantArgs a;
+    a.x = st.x; a.xq = reinterpret_cast<uint2*>(st.xq); a.xs = st.xs;
+    a.M = st.M; a.nvec = st.K >> 3; a.wait_stage = st.wait_stage; a.inv_nvec = st.inv_nvec;
+    return a;
+}
+
+__device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, int tid, int bar_id, unsigned* s_rowmax, float4* s_scale,
+                                               unsigned long long* dbg) {
+    const int grid = (int)gridDim.x, cta = (int)blockIdx.x, nvec = a.nvec, M = a.M;
+    const unsigned inv_nvec = a.inv_nvec;
+    const uint4* __restrict__ x = a.x;
+    uint2* __restrict__ xq = a.xq;
+    float* __restrict__ xs = a.xs;
+    const int R = M > cta ? (M - cta + grid - 1) / grid : 0;
+    for (int i0 = 0; i0 < R; i0 += LP_QROWS) {
+        const int g = min(LP_QROWS, R - i0), ntask = g * nvec;
         if (tid < LP_QROWS) s_rowmax[tid] = 0u;
-        lp_bar(2, LP_QT);
+        lp_bar(bar_id, LP_QT);
+        const bool held = ntask <= LP_QT * LP_QV;                     // one round: the vectors stay in registers
         uint4 v[LP_QV];
         int rl[LP_QV];
-        size_t at[LP_QV];
+        for (int f0 = 0; f0 < ntask; f0 += LP_QT * LP_QV) {           // pass 1: row absmax
 #pragma unroll
-        for (int j = 0; j < LP_QV; ++j) {
-            const int f = tid + j * LP_QT;
-            rl[j] = -1;
-            at[j] = 0;
-            v[j] = make_uint4(0, 0, 0, 0);
-            if (f < ntask) {
-                rl[j] = (int)__umulhi((unsigned)f, st.inv_nvec);
-                at[j] = (size_t)(cta + (i0 + rl[j]) * grid) * nvec + (f - rl[j] * nvec);
-                v[j] = __ldcg(st.x + at[j]);             // L2: another SM may have written it earlier in this launch
+            for (int j = 0; j < LP_QV; ++j) {
+                const int f = f0 + tid + j * LP_QT;
+                rl[j] = -1;
+                v[j] = make_uint4(0, 0, 0, 0);
+                if (f < ntask) {
+                    rl[j] = (int)__umulhi((unsigned)f, inv_nvec);
+                    v[j] = __ldcg(x + ((unsigned)(cta + (i0 + rl[j]) * grid) * (unsigned)nvec + (unsigned)(f - rl[j] * nvec)));   // L2: written by other SMs
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < LP_QV; ++j) {
+                uint32_t m = absmax8_packed(v[j], 0u);
+                m = max(m & 0xFFFFu, m >> 16);
+                const int r0 = __shfl_sync(0xFFFFFFFFu, rl[j], 0);
+                if (__all_sync(0xFFFFFFFFu, rl[j] == r0)) {
+                    m = __reduce_max_sync(0xFFFFFFFFu, m);
+                    if ((tid & 31) == 0 && r0 >= 0) atomicMax(s_rowmax + r0, m);
+                } else if (rl[j] >= 0) {
+                    atomicMax(s_rowmax + rl[j], m);
+                }
             }
         }
-#pragma unroll
-        for (int j = 0; j < LP_QV; ++j) {
-            uint32_t m = absmax8_packed(v[j], 0u);
-            m = max(m & 0xFFFFu, m >> 16);
-            const int r0 = __shfl_sync(0xFFFFFFFFu, rl[j], 0);
-            if (__all_sync(0xFFFFFFFFu, rl[j] == r0)) {
-                m = __reduce_max_sync(0xFFFFFFFFu, m);
-                if ((tid & 31) == 0 && r0 >= 0) atomicMax(s_rowmax + r0, m);
-            } else if (rl[j] >= 0) {
-                atomicMax(s_rowmax + rl[j], m);
-            }
-        }
-        lp_bar(2, LP_QT);
+#ifdef VLA_LP_STAMPS
+        if (tid == 0 && i0 == 0) dbg[6] = lp_now();
+#endif
+        lp_bar(bar_id, LP_QT);
         if (tid < g) {
             const float alpha = alpha_of(bf16lo(s_rowmax[tid]));
             s_scale[tid] = quant_scales_of_alpha(alpha);
-            st.xs[cta + (i0 + tid) * grid] = alpha;
+            xs[cta + (i0 + tid) * grid] = alpha;
         }
-        lp_bar(2, LP_QT);
+        lp_bar(bar_id, LP_QT);
+        for (int f0 = 0; f0 < ntask; f0 += LP_QT * LP_QV) {           // pass 2: quantise
 #pragma unroll
-        for (int j = 0; j < LP_QV; ++j)
-            if (rl[j] >= 0) xq[at[j]] = quant8_fast(v[j], s_scale[rl[j]]);
+            for (int j = 0; j < LP_QV; ++j) {
+                const int f = f0 + tid + j * LP_QT;
+                if (!held) {
+                    rl[j] = -1;
+                    if (f < ntask) {
+                        rl[j] = (int)__umulhi((unsigned)f, inv_nvec);
+                        v[j] = __ldcg(x + ((unsigned)(cta + (i0 + rl[j]) * grid) * (unsigned)nvec + (unsigned)(f - rl[j] * nvec)));
+                    }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < LP_QV; ++j) {
+                const int f = f0 + tid + j * LP_QT;
+                if (rl[j] >= 0)
+                    xq[(unsigned)(cta + (i0 + rl[j]) * grid) * (unsigned)nvec + (unsigned)(f - rl[j] * nvec)] = quant8_fast(v[j], s_scale[rl[j]]);
+            }
+        }
     }
 }
 
 template <int KS>
-__global__ void __launch_bounds__(LG_THREADS, 1) lprog_kernel(const __grid_constant__ DevLProg P) {
+__global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_constant__ DevLProg P) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
@@ -159,6 +220,7 @@ __global__ void __launch_bounds__(LG_THREADS, 1) lprog_kernel(const __grid_const
                 tma_prefetch_desc(st.tmap);
                 if (!waited) { pdl_wait(); waited = true; }   // the counters are re-zeroed by the previous run's last CTA
                 spin_until(P.qdone + sidx, grid);
+                LP_STAMP(2);
                 asm volatile("fence.proxy.async.global;" ::: "memory");       // generic-proxy stores -> TMA reads
                 for (int tile = blockIdx.x; tile < ntiles; tile += grid) {
                     const int m0 = (tile / tiles_n) * TN;
@@ -190,6 +252,7 @@ __global__ void __launch_bounds__(LG_THREADS, 1) lprog_kernel(const __grid_const
                         const uint32_t s = it % ns;
                         mbar_wait(bar_full(s), (it / ns) & 1);
                         tc_fence_after();
+                        if (kb == 0 && tile == (int)blockIdx.x) LP_STAMP(3);
 #pragma unroll
                         for (int kk = 0; kk < KS; ++kk) {
                             const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride + kk * LG_A_BYTES);
@@ -201,24 +264,19 @@ __global__ void __launch_bounds__(LG_THREADS, 1) lprog_kernel(const __grid_const
                         mma_commit(bar_empty(s));
                     }
                     mma_commit(bar_acc_full(ab));
+                    LP_STAMP(4);
                 }
             }
         }
     } else if (warp <= 10) {
-        // ---------------- decode warps: fused quant of the stage, then the stage's weight tiles ----------------
+        // ---------------- decode warps ----------------
         const int dgrp = (warp - 3) >> 2;
-        const int d = (threadIdx.x - 96) & 127, qt = (int)threadIdx.x - 96;
+        const int d = (threadIdx.x - 96) & 127;
         const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
         const int g = 2 * q + p;
         uint32_t it = 0;
-        pdl_wait();                                           // x of the first stages may be the previous kernel's output
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpStage& st = stages[sidx];
-            if (qt == 0 && st.wait_stage >= 0) spin_until(P.gdone + st.wait_stage, grid);
-            lp_bar(2, LP_QT);
-            lp_quant_stage(st, qt, s_rowmax, s_scale);
-            lp_bar(2, LP_QT);                                 // every row of this CTA is stored ...
-            if (qt == 0) red_release_gpu(P.qdone + sidx, 1u); // ... and published
             const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
             for (int tile = blockIdx.x; tile < ntiles; tile += grid) {
                 for (int kb = 0; kb < num_kb; kb += KS, ++it) {
@@ -257,7 +315,7 @@ __global__ void __launch_bounds__(LG_THREADS, 1) lprog_kernel(const __grid_const
                 }
             }
         }
-    } else {
+    } else if (warp <= 14) {
         // ---------------- epilogue warps ----------------
         const int lq = warp & 3;
         float* sc = pScale + lq * 256;
@@ -268,8 +326,8 @@ __global__ void __launch_bounds__(LG_THREADS, 1) lprog_kernel(const __grid_const
             const LpStage& st = stages[sidx];
             const int tiles_n = st.tiles_n, ntiles = st.ntiles, TN = st.TN, M = st.M, nlin = st.grp.n;
             if ((int)blockIdx.x < ntiles) {
-                if (lane == 0) spin_until(P.qdone + sidx, grid);              // alpha of every row is stored
-                __syncwarp();
+                if (threadIdx.x == 11 * 32) spin_until(P.qdone + sidx, grid); // alpha of every row is stored
+                lp_bar(3, 128);
             }
             const float* __restrict__ x_scale = st.xs;
             for (int tile = blockIdx.x; tile < ntiles; tile += grid, ++ti) {
@@ -335,7 +393,30 @@ __global__ void __launch_bounds__(LG_THREADS, 1) lprog_kernel(const __grid_const
                 if (lane == 0) mbar_arrive(bar_acc_empty(ab));
             }
             lp_bar(3, 128);                                   // the four epilogue warps have stored the CTA's tiles of the stage
-            if (threadIdx.x == 11 * 32) red_release_gpu(P.gdone + sidx, 1u);
+            if (threadIdx.x == 11 * 32) { LP_STAMP(5); red_release_gpu(P.gdone + sidx, 1u); }
+        }
+    }
+    else {
+        // ---------------- quantiser groups: run ahead of the GEMM as far as the stages' dependencies allow ----------------
+        const int qg = ((int)threadIdx.x - LG_THREADS) / LP_QT, qt = ((int)threadIdx.x - LG_THREADS) % LP_QT;
+        const int bar_id = 4 + qg;
+        pdl_wait();                                           // x of the first stages may be the previous kernel's output
+        if (qg < P.n_stages) {
+            LpQuantArgs next = lp_quant_args(stages[qg]);
+            for (int sidx = qg; sidx < P.n_stages; sidx += LP_QG) {
+                const LpQuantArgs st = next;
+                if (sidx + LP_QG < P.n_stages) next = lp_quant_args(stages[sidx + LP_QG]);   // its loads fly during this stage's work
+                if (qt == 0 && st.wait_stage >= 0) spin_until(P.gdone + st.wait_stage, grid);
+                lp_bar(bar_id, LP_QT);
+                if (qt == 0) LP_STAMP(0);
+#ifdef VLA_LP_STAMPS
+                lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, P.stamps + ((size_t)sidx * gridDim.x + blockIdx.x) * 8);
+#else
+                lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, nullptr);
+#endif
+                lp_bar(bar_id, LP_QT);                        // every row of this CTA is stored ...
+                if (qt == 0) { LP_STAMP(1); red_release_gpu(P.qdone + sidx, 1u); }      // ... and published
+            }
         }
     }
     tc_fence_before();
@@ -357,11 +438,11 @@ cudaError_t lprogram_max_ctas_per_sm(int KS, int smem_bytes, int* out) {
     if (KS == 2) {
         e = cudaFuncSetAttribute(lprog_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
         if (e != cudaSuccess) return e;
-        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, lprog_kernel<2>, LG_THREADS, (size_t)smem_bytes);
+        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, lprog_kernel<2>, LP_THREADS, (size_t)smem_bytes);
     }
     e = cudaFuncSetAttribute(lprog_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, lprog_kernel<1>, LG_THREADS, (size_t)smem_bytes);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, lprog_kernel<1>, LP_THREADS, (size_t)smem_bytes);
 }
 
 cudaError_t launch_lprogram(const DevLProg& prog, int grid, cudaStream_t s) {
@@ -371,7 +452,7 @@ cudaError_t launch_lprogram(const DevLProg& prog, int grid, cudaStream_t s) {
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(LG_THREADS);
+    cfg.blockDim = dim3(LP_THREADS);
     cfg.dynamicSmemBytes = (size_t)prog.smem_bytes;
     cfg.stream = s;
     cudaLaunchAttribute at[1];

@@ -193,8 +193,7 @@ __device__ __forceinline__ void quant_rows(const DevProg& P, const DevStage& st,
         consumer_bar();
         if (tid < 16) {                                      // per row: alpha_m and the bracketing reciprocals
             const float alpha = alpha_of(__uint_as_float(s_rowmax[tid]));
-            const float inv = __frcp_rn(alpha);
-            s_scale[tid] = make_float4(alpha, __fmul_rn(inv, 1.0f - 1.9073486328125e-06f), __fmul_rn(inv, 1.0f + 1.9073486328125e-06f), 0.0f);
+            s_scale[tid] = quant_scales_of_alpha(alpha);
             const int j = (tid - first) / step;              // is row tid one of this round's rows?
             if (tid >= first && tid < M && (tid - first) % step == 0 && j >= j0 && j < j0 + rpr) {
                 if (TO_GLOBAL) alpha_g[tid] = alpha;

@@ -10,7 +10,7 @@
 namespace vla {
 
 constexpr uint32_t LPROG_MAGIC = 0x564C414Cu;   // "VLAL"
-constexpr int LP_EXTRA_SMEM = 16 * 4 + 16 * 16;  // quantiser scratch behind gemm_large's layout: row absmax [16] + scales float4 [16]
+constexpr int LP_EXTRA_SMEM = 16 * 4 + 16 * 16;   // quantiser scratch behind gemm_large's layout: row absmax [16], scales float4 [16]
 
 struct alignas(64) LpStage {
     unsigned char tmap[128];   // CUtensorMap of xq [M,K] int8: box [128 k, TN tokens], SWIZZLE_128B
@@ -37,6 +37,7 @@ struct DevLProg {
     unsigned* gdone;           // [n_stages] CTAs that have stored their tiles of stage s         (target gridDim.x)
     unsigned* done;            // [1]        CTAs past their last counter access; the last one re-zeroes the counters
     const LpStage* stages;
+    unsigned long long* stamps; // debug builds only (VLA_LP_STAMPS): [n_stages][grid][8] globaltimer stamps
 };
 
 cudaError_t launch_lprogram(const DevLProg& prog, int grid, cudaStream_t s);

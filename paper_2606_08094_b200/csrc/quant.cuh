@@ -35,66 +35,69 @@ __device__ __forceinline__ uint2 quant8(uint4 v, float alpha) {
 
 __device__ __forceinline__ float alpha_of(float absmax) { return __fdiv_rn(fmaxf(absmax, 1e-5f), 127.0f); }
 
-// ---------------------------------------------------------------- exact fast quantiser (program kernel)
-// Exact shortcut for  a = rint(x / alpha)  (quant.cuh's q1, two true divisions):  with  inv = RN(1 / alpha),
-// the products x * inv * (1 -+ 2^-19) bracket fl(x / alpha) (which is x / alpha within 2^-24 relative), and an FMA with
-// 1.5 * 2^23 rounds each of them to the nearest integer, ties to even, exactly.  rint(fl(.)) is monotone, so when both
-// ends give the same integer it IS the result; when they differ (a rounding boundary inside the bracket: < 5e-4 of the
-// elements) the 16 elements are redone with the true-division quantiser.  |x / alpha| <= 127 (1 + 2^-23): no clamp.
-// Two elements per instruction: fma.rn.f32x2.
-__device__ __forceinline__ uint32_t quant4_fast(uint32_t u0, uint32_t u1, float2 ilo, float2 ihi, uint32_t& diff) {
+// ---------------------------------------------------------------- exact fast quantiser (persistent kernels)
+// Exact shortcut for  a = rint(x / alpha)  (q1 above: two true divisions):  with  inv = RN(1 / alpha), the products
+// x * inv * (1 -+ 2^-19) bracket fl(x / alpha) (which is x / alpha within 2^-24 relative), and an FMA with 1.5 * 2^23 rounds
+// each of them to the nearest integer, ties to even, exactly.  rint(fl(.)) is monotone, so when both ends give the same
+// integer it IS the result; when they differ (a rounding boundary inside the bracket) that ELEMENT is redone with q1.
+// |x / alpha| <= 127 (1 + 2^-23): no clamp.  Two elements per instruction: fma.rn.f32x2.
+// How often: on bf16 data ~1 % of all 8-element vectors have such an element (measured) -- with 8-bit mantissas x / alpha
+// is often an exact rational tie k + 1/2 -- so almost every warp takes the rare branch for one or two lanes per round.  The
+// branch therefore has to be SHORT: the low bytes of both bracket ends are packed (PRMT) and XORed, a non-zero byte marks
+// the element, and only marked elements run q1 (~40 instructions).  (Re-scanning all elements of the vector with scalar
+// FMAs, as the first version did, cost 1.5 us per stage of the large programs and 1.6 us per phase of the M=8 stack.)
+__device__ __forceinline__ uint32_t quant4_fast(uint32_t u0, uint32_t u1, float2 ilo, float2 ihi, uint32_t& dw) {
     const float2 MAGIC = make_float2(12582912.0f, 12582912.0f);
     const float2 x01 = make_float2(bf16lo(u0), bf16hi(u0)), x23 = make_float2(bf16lo(u1), bf16hi(u1));
     const float2 a01 = __ffma2_rn(x01, ilo, MAGIC), b01 = __ffma2_rn(x01, ihi, MAGIC);
     const float2 a23 = __ffma2_rn(x23, ilo, MAGIC), b23 = __ffma2_rn(x23, ihi, MAGIC);
-    const uint32_t a0 = __float_as_uint(a01.x), a1 = __float_as_uint(a01.y), a2 = __float_as_uint(a23.x), a3 = __float_as_uint(a23.y);
-    diff |= (a0 ^ __float_as_uint(b01.x)) | (a1 ^ __float_as_uint(b01.y));
-    diff |= (a2 ^ __float_as_uint(b23.x)) | (a3 ^ __float_as_uint(b23.y));
     // the int8 result is the low byte of each sum (0x4B400000 + r)
-    return __byte_perm(__byte_perm(a0, a1, 0x0040), __byte_perm(a2, a3, 0x0040), 0x5410);
+    const uint32_t wa = __byte_perm(__byte_perm(__float_as_uint(a01.x), __float_as_uint(a01.y), 0x0040),
+                                    __byte_perm(__float_as_uint(a23.x), __float_as_uint(a23.y), 0x0040), 0x5410);
+    const uint32_t wb = __byte_perm(__byte_perm(__float_as_uint(b01.x), __float_as_uint(b01.y), 0x0040),
+                                    __byte_perm(__float_as_uint(b23.x), __float_as_uint(b23.y), 0x0040), 0x5410);
+    dw = wa ^ wb;                                        // adjacent integers differ in their low byte
+    return wa;
 }
-// Rare path (a rounding boundary inside an element's bracket): redo exactly those elements with the true-division
-// quantiser of quant.cuh.  One out-of-line copy; the fast path is inlined per task.
-__device__ __forceinline__ uint32_t patch2(uint32_t u, uint32_t o2, int shift, float4 sc) {
-    const float MAGIC = 12582912.0f;
-    const float x0 = bf16lo(u), x1 = bf16hi(u);
-    if (__float_as_uint(__fmaf_rn(x0, sc.y, MAGIC)) != __float_as_uint(__fmaf_rn(x0, sc.z, MAGIC)))
-        o2 = (o2 & ~(0xFFu << shift)) | (q1(x0, sc.x) << shift);
-    if (__float_as_uint(__fmaf_rn(x1, sc.y, MAGIC)) != __float_as_uint(__fmaf_rn(x1, sc.z, MAGIC)))
-        o2 = (o2 & ~(0xFF00u << shift)) | (q1(x1, sc.x) << (shift + 8));
-    return o2;
-}
-static __device__ __noinline__ uint4 quant16_patch(uint4 a, uint4 b, float4 sc, uint4 o) {
-    o.x = patch2(a.y, patch2(a.x, o.x, 0, sc), 16, sc);
-    o.y = patch2(a.w, patch2(a.z, o.y, 0, sc), 16, sc);
-    o.z = patch2(b.y, patch2(b.x, o.z, 0, sc), 16, sc);
-    o.w = patch2(b.w, patch2(b.z, o.w, 0, sc), 16, sc);
-    return o;
+// redo the elements marked in dw (non-zero byte e = element e of {u0 lo, u0 hi, u1 lo, u1 hi}) with the true divisions
+__device__ __forceinline__ uint32_t fix4(uint32_t w, uint32_t dw, uint32_t u0, uint32_t u1, float alpha) {
+    while (dw != 0u) {
+        const int e = (__ffs((int)dw) - 1) >> 3;
+        const uint32_t u = (e & 2) ? u1 : u0;
+        const float x = (e & 1) ? bf16hi(u) : bf16lo(u);
+        const uint32_t m = 0xFFu << (8 * e);
+        w = (w & ~m) | (q1(x, alpha) << (8 * e));
+        dw &= ~m;
+    }
+    return w;
 }
 __device__ __forceinline__ uint4 quant16(uint4 a, uint4 b, float4 sc) {      // sc = {alpha, inv_lo, inv_hi, -}
     const float2 ilo = make_float2(sc.y, sc.y), ihi = make_float2(sc.z, sc.z);
-    uint32_t diff = 0;
+    uint32_t d0, d1, d2, d3;
     uint4 o;
-    o.x = quant4_fast(a.x, a.y, ilo, ihi, diff);
-    o.y = quant4_fast(a.z, a.w, ilo, ihi, diff);
-    o.z = quant4_fast(b.x, b.y, ilo, ihi, diff);
-    o.w = quant4_fast(b.z, b.w, ilo, ihi, diff);
-    if (diff != 0u) o = quant16_patch(a, b, sc, o);          // rare: a rounding boundary is too close
+    o.x = quant4_fast(a.x, a.y, ilo, ihi, d0);
+    o.y = quant4_fast(a.z, a.w, ilo, ihi, d1);
+    o.z = quant4_fast(b.x, b.y, ilo, ihi, d2);
+    o.w = quant4_fast(b.z, b.w, ilo, ihi, d3);
+    if ((d0 | d1 | d2 | d3) != 0u) {                         // rare per lane, common per warp: keep it short
+        o.x = fix4(o.x, d0, a.x, a.y, sc.x);
+        o.y = fix4(o.y, d1, a.z, a.w, sc.x);
+        o.z = fix4(o.z, d2, b.x, b.y, sc.x);
+        o.w = fix4(o.w, d3, b.z, b.w, sc.x);
+    }
     return o;
 }
-// the same for one vector of 8 (stand-alone act_quant kernel)
-static __device__ __noinline__ uint2 quant8_patch(uint4 a, float4 sc, uint2 o) {
-    o.x = patch2(a.y, patch2(a.x, o.x, 0, sc), 16, sc);
-    o.y = patch2(a.w, patch2(a.z, o.y, 0, sc), 16, sc);
-    return o;
-}
+// the same for one vector of 8
 __device__ __forceinline__ uint2 quant8_fast(uint4 a, float4 sc) {
     const float2 ilo = make_float2(sc.y, sc.y), ihi = make_float2(sc.z, sc.z);
-    uint32_t diff = 0;
+    uint32_t d0, d1;
     uint2 o;
-    o.x = quant4_fast(a.x, a.y, ilo, ihi, diff);
-    o.y = quant4_fast(a.z, a.w, ilo, ihi, diff);
-    if (diff != 0u) o = quant8_patch(a, sc, o);
+    o.x = quant4_fast(a.x, a.y, ilo, ihi, d0);
+    o.y = quant4_fast(a.z, a.w, ilo, ihi, d1);
+    if ((d0 | d1) != 0u) {
+        o.x = fix4(o.x, d0, a.x, a.y, sc.x);
+        o.y = fix4(o.y, d1, a.z, a.w, sc.x);
+    }
     return o;
 }
 // absmax of 8 bf16 as a packed pair of 15-bit magnitudes (bf16 magnitudes order like unsigned integers)
@@ -110,9 +113,15 @@ __device__ __forceinline__ uint32_t absmax8_packed(uint4 v, uint32_t m) {
 __device__ __forceinline__ float absmax_unpack(uint32_t m) { return fmaxf(bf16lo(m), bf16hi(m)); }
 
 // {alpha, 1/alpha * (1 - 2^-19), 1/alpha * (1 + 2^-19), -}
+// A power-of-two alpha (absmax = 127 * 2^j: one bf16 mantissa in 128, so ~1 % of all rows) makes x / alpha EXACT, and with
+// 8-bit bf16 mantissas a large share of its elements are exact ties k + 1/2, which a bracket of non-zero width can never
+// decide: every vector of such a row would take the slow patch (measured: 2 % of all vectors, 1.5 us per stage).  There
+// 1 / alpha is exact too, so x * (1/alpha) + MAGIC rounds the exact quotient, ties to even: the bracket collapses to a point.
 __device__ __forceinline__ float4 quant_scales_of_alpha(float alpha) {
     const float inv = __frcp_rn(alpha);
-    return make_float4(alpha, __fmul_rn(inv, 1.0f - 1.9073486328125e-06f), __fmul_rn(inv, 1.0f + 1.9073486328125e-06f), 0.0f);
+    const bool dyadic = (__float_as_uint(alpha) & 0x007FFFFFu) == 0u;
+    return make_float4(alpha, dyadic ? inv : __fmul_rn(inv, 1.0f - 1.9073486328125e-06f),
+                       dyadic ? inv : __fmul_rn(inv, 1.0f + 1.9073486328125e-06f), 0.0f);
 }
 
 }  // namespace vla
