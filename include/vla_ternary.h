@@ -118,6 +118,23 @@ vla_status vla_ternary_linear_host(const void* packed, const float* w_scale, con
                                    int M, int N, int K, void* out_host, vla_dtype out_dtype, vla_path path,
                                    void* workspace, size_t workspace_bytes, void* stream);
 
+/* vla_ternary_linear for callers that CANNOT ALLOCATE device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the scratch of the call -- the quantised activations [M,K] int8 and their
+ * scales [M] fp32 -- lives in a fixed array inside the library (csrc/no_alloc.cu; every GPU that loads the library holds
+ * its VLA_STATIC_MAX_MK + 4 * VLA_STATIC_MAX_M bytes until the process exits), so there is no workspace argument and the
+ * call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine).  Same arithmetic, same kernels and
+ * the same result, bit for bit, as vla_ternary_linear.
+ *   limit   M * K <= VLA_STATIC_MAX_MK and M <= VLA_STATIC_MAX_M, else VLA_ERR_WORKSPACE (use vla_ternary_linear with
+ *           a workspace of your own for larger problems); other errors as vla_ternary_linear
+ *   sharing every call on a device uses the SAME array, which keeps the last call's contents (nothing in it has to be
+ *           cleared: each call overwrites what it reads).  Calls that overlap on the GPU -- different streams, graphs
+ *           replayed concurrently -- race on it: issue them on one stream, or order them with events.
+ * Asynchronous on `stream`, capturable. */
+#define VLA_STATIC_MAX_MK 8388608   /* 8 MiB of int8 activations, e.g. M = 1024 at K = 8192, M = 1213 at K = 6912 */
+#define VLA_STATIC_MAX_M 16384
+vla_status vla_ternary_linear_static(const void* packed, const float* w_scale, const void* x_bf16,
+                                     int M, int N, int K, void* out, vla_dtype out_dtype, vla_path path, void* stream);
+
 /* ---------------------------------------------------------------------------------------------------
  * Programs: a whole list of small-M ternary linears in ONE persistent launch.
  *

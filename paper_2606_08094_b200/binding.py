@@ -24,7 +24,7 @@ _TORCH_DTYPE = {VLA_F32: torch.float32, VLA_BF16: torch.bfloat16, VLA_I32: torch
 EXPORTS = [
     "vla_ternary_packed_bytes", "vla_ternary_workspace_bytes", "vla_ternary_pack", "vla_ternary_unpack",
     "vla_act_quant", "vla_ternary_gemm", "vla_ternary_linear", "vla_ternary_linear_host",
-    "vla_ternary_host_workspace_bytes",
+    "vla_ternary_host_workspace_bytes", "vla_ternary_linear_static",
     "vla_ternary_auto_path", "vla_i8_mma_issue_probe", "vla_status_string", "vla_launch_count",
     "vla_cached_attention", "vla_cached_attention_workspace_bytes",
     "vla_ternary_gemm_grouped", "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_run_host", "vla_program_release",
@@ -73,6 +73,8 @@ def _load():
     lib.vla_ternary_gemm.argtypes = [vp, vp, vp, vp, i, i, i, vp, i, i, vp, sz, vp]
     lib.vla_ternary_linear.restype = st
     lib.vla_ternary_linear.argtypes = [vp, vp, vp, i, i, i, vp, i, i, vp, vp, vp, sz, vp]
+    lib.vla_ternary_linear_static.restype = st
+    lib.vla_ternary_linear_static.argtypes = [vp, vp, vp, i, i, i, vp, i, i, vp]
     lib.vla_ternary_linear_host.restype = st
     lib.vla_ternary_linear_host.argtypes = [vp, vp, vp, i, i, i, vp, i, i, vp, sz, vp]
     lib.vla_ternary_host_workspace_bytes.restype = sz
@@ -177,6 +179,15 @@ def vla_ternary_linear(packed, w_scale, x_bf16, M, N, K, out, out_dtype, path=VL
     _check(_lib.vla_ternary_linear(_ptr(packed), _ptr(w_scale), _ptr(x_bf16), M, N, K, _ptr(out), out_dtype, path,
                                    _ptr(xq_opt), _ptr(x_scale_opt), _ptr(workspace), workspace_bytes,
                                    _stream(stream)), "vla_ternary_linear")
+
+
+VLA_STATIC_MAX_MK, VLA_STATIC_MAX_M = 8388608, 16384
+
+
+def vla_ternary_linear_static(packed, w_scale, x_bf16, M, N, K, out, out_dtype, path=VLA_PATH_AUTO, stream=None):
+    """vla_ternary_linear with its scratch in a fixed array inside the library: allocates nothing (include/vla_ternary.h)."""
+    _check(_lib.vla_ternary_linear_static(_ptr(packed), _ptr(w_scale), _ptr(x_bf16), M, N, K, _ptr(out), out_dtype, path,
+                                          _stream(stream)), "vla_ternary_linear_static")
 
 
 def vla_ternary_host_workspace_bytes(M, N, K, out_dtype, path=VLA_PATH_AUTO):

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libvlaternary.so")
-SOURCES = ["api.cu", "pack.cu", "act_quant.cu", "gemm_small.cu", "gemm_large.cu", "gemm_program.cu", "gemm_lprog.cu", "api_program.cu", "attention.cu"]
+SOURCES = ["api.cu", "pack.cu", "act_quant.cu", "gemm_small.cu", "gemm_large.cu", "gemm_program.cu", "gemm_lprog.cu", "api_program.cu", "attention.cu", "no_alloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--threads", "0"]
 
