@@ -486,7 +486,10 @@ def run_gpu(args):
         import bench_workloads as bw
         vs_m, roof_tensor = bw.run_vs_m(pk, int8_probe_tops(vla))
         if roof_tensor is not None:
-            roof_tensor["traffic"] = ncu_traffic("lprog_kernel_x%d" % 12)
+            t1 = ncu_traffic("lprog_kernel")                # DRAM bytes of the captured ONE-step launch (--workload prefill)
+            nstep = max(1, int(round(roof_tensor["us_per_launch"] / roof_tensor["us_per_step"])))
+            roof_tensor["traffic"] = None if t1 is None else t1 * nstep
+            roof_tensor["traffic_source"] = "DRAM bytes per step of the captured one-step launch x %d steps per launch" % nstep
             if roof_tensor.get("gemm_only"):
                 roof_tensor["gemm_only"]["traffic"] = ncu_traffic("gemm_large")
 
