@@ -136,7 +136,7 @@ vla_status vla_ternary_linear_static(const void* packed, const float* w_scale, c
                                      int M, int N, int K, void* out, vla_dtype out_dtype, vla_path path, void* stream);
 
 /* ---------------------------------------------------------------------------------------------------
- * Programs: a whole list of small-M ternary linears in ONE persistent launch.
+ * Programs: a whole list of ternary linears -- all small-M (decode) or all large-M (prefill) -- in ONE persistent launch.
  *
  * "graphs and buffers persist across same-shape requests ... GPU graph capture" removes
  * dispatch overhead.  On B200 one launch costs more than ten times the HBM time of a BitNet-2B weight
@@ -144,7 +144,7 @@ vla_status vla_ternary_linear_static(const void* packed, const float* w_scale, c
  * persistent kernel (csrc/gemm_program.cu) that streams the packed weights of every stage back to back
  * and synchronises only where a stage reads what an earlier stage wrote.
  *
- * A STAGE is one activation matrix x [M,K] bf16 (1 <= M <= 16, K % 128 == 0, K <= 8192) and n_linears
+ * A STAGE is one activation matrix x [M,K] bf16 (small programs: 1 <= M <= 16; K % 128 == 0, K <= 8192) and n_linears
  * (1..16) ternary linears that all consume it, each with its own packed W [N,K], scale beta and output:
  * the per-output-group scales beta_g(n) of Eq. 4, e.g. q|k|v or gate|up.
  * Every stage runs Eq. 4 end to end inside the one kernel: absmax int8 quant of x (fused: small stages are quantised by
@@ -154,6 +154,14 @@ vla_status vla_ternary_linear_static(const void* packed, const float* w_scale, c
  *                 current PHASE, whose stages run concurrently on disjoint groups of SMs
  *   depends = 1   x is (part of) the output of EARLIER stages of this program: the stage opens a new
  *                 phase, which starts only after every earlier phase has completed on the whole grid
+ *
+ * LARGE programs (csrc/gemm_lprog.cu): if the stages have M > 16 tokens (17 <= M <= 32768, K <= 8192, 1..8 linears per
+ * stage; ALL stages of a program are of one kind, else VLA_ERR_SHAPE) the program runs on the tcgen05 / TMEM kernel
+ * instead: every CTA quantises a share of the rows of x into int8 scratch inside the program buffer (or into xq_opt /
+ * x_scale_opt), the CTAs meet on a grid-wide counter, and the stage's 128-channel x token tiles are walked as in
+ * VLA_PATH_LARGE; the launch does not end between stages.  Stages run in list order; depends = 1 makes a stage's
+ * quantisation wait until EVERY earlier stage has stored its outputs, depends = 0 lets it run ahead (its x must not be
+ * written by this program).  Results are bit-identical to vla_ternary_linear.
  * All pointers inside the descriptors are DEVICE pointers, 16-byte aligned, and must stay valid for as
  * long as the program is run.  The descriptor arrays themselves are HOST memory.
  */
@@ -182,8 +190,9 @@ typedef struct {
 vla_status vla_ternary_gemm_grouped(const vla_prog_linear* lins /*host*/, int n_linears, const int8_t* xq,
                                     const float* x_scale, int M, int K, vla_path path, void* stream);
 
-/* Device bytes a compiled program needs (descriptor tables, barrier counters, quantised activations);
- * a multiple of 256.  0 if any stage is invalid. */
+/* Device bytes a compiled program needs (descriptor tables, barrier counters, quantised activations: for a large
+ * program four int8 [M,K] + alpha [M] scratch sets of its largest stage); a multiple of 256.  0 if any stage is invalid
+ * or small and large stages are mixed. */
 size_t vla_program_bytes(const vla_prog_stage* stages /*host*/, int n_stages);
 
 /* Compiles `stages` into prog_dev (device memory, >= vla_program_bytes, 256-byte aligned).
