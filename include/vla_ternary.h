@@ -191,7 +191,7 @@ vla_status vla_ternary_gemm_grouped(const vla_prog_linear* lins /*host*/, int n_
                                     const float* x_scale, int M, int K, vla_path path, void* stream);
 
 /* Device bytes a compiled program needs (descriptor tables, barrier counters, quantised activations: for a large
- * program four int8 [M,K] + alpha [M] scratch sets of its largest stage); a multiple of 256.  0 if any stage is invalid
+ * program eight int8 [M,K] + alpha [M] scratch sets of its largest stage); a multiple of 256.  0 if any stage is invalid
  * or small and large stages are mixed. */
 size_t vla_program_bytes(const vla_prog_stage* stages /*host*/, int n_stages);
 

@@ -32,7 +32,7 @@ constexpr int LP_QG = VLA_LP_QG;                         // quantiser groups (af
 constexpr int LP_QW = VLA_LP_QW;                         // warps per group
 constexpr int LP_QT = 32 * LP_QW;
 constexpr int LP_QV = VLA_LP_QV;                         // vectors of 8 bf16 a thread has in flight
-constexpr int LP_THREADS = LG_THREADS + LP_QG * LP_QT;
+constexpr int LP_THREADS = LG_THREADS + LP_QG * LP_QT + 32;         // + the publisher warp
 constexpr int LP_QROWS = 16;                             // most rows per round
 static_assert(LP_QG == 1 && LP_EXTRA_SMEM == LP_QROWS * 4 + LP_QROWS * 16, "lprogram.h");
 
@@ -47,6 +47,12 @@ __device__ __forceinline__ unsigned long long lp_now() {
 #define LP_STAMP(k) do { } while (0)
 #endif
 
+// Tile t of a stage runs on CTA (t + rot) mod grid: `rot` continues the round robin where the previous stage's tiles ended,
+// so that the CTAs a short stage leaves idle are the first to start the next one (independent stages overlap).
+__device__ __forceinline__ int lp_first_tile(const LpStage& st, unsigned grid) {
+    const int b = (int)blockIdx.x, r = st.rot;
+    return b >= r ? b - r : b + (int)grid - r;
+}
 __device__ __forceinline__ void lp_bar(int id, int threads) {
     asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(threads) : "memory");
 }
@@ -166,6 +172,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(p_tail);
     unsigned* s_rowmax = reinterpret_cast<unsigned*>(p_tail + 16);
     float4* s_scale = reinterpret_cast<float4*>(p_tail + 16 + LP_QROWS * 4);
+    const uint32_t s_qcount = tmem_slot + 8u;                // quantiser warps that have stored a stage, summed over the stages
+    const uint32_t s_gok = tmem_slot + 12u;                  // stages the publisher has cleared for the quantiser
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const unsigned grid = gridDim.x;
@@ -176,6 +184,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         for (int s = 0; s < LG_NS_MAX; ++s) { mbar_init(bar_full(s), 5); mbar_init(bar_empty(s), 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(bar_acc_full(s), 1); mbar_init(bar_acc_empty(s), 4); }
         fence_barrier_init();
+        asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 8u), "r"(0u) : "memory");
+        asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 12u), "r"(0u) : "memory");
     }
     if (warp == 2) tmem_alloc(tmem_slot, 512u);
     tc_fence_before();
@@ -192,7 +202,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
             for (int sidx = 0; sidx < P.n_stages; ++sidx) {
                 const LpStage& st = stages[sidx];
                 const int num_kb = st.K / TILE_K, tiles_n = st.tiles_n, ntiles = st.ntiles, nlin = st.grp.n;
-                for (int tile = blockIdx.x; tile < ntiles; tile += grid) {
+                for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid) {
                     const int ct = tile % tiles_n;
                     int li = 0;
                     for (int j = 1; j < nlin; ++j) if (ct >= st.grp.ct_begin[j]) li = j;
@@ -216,13 +226,13 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
             for (int sidx = 0; sidx < P.n_stages; ++sidx) {
                 const LpStage& st = stages[sidx];
                 const int num_kb = st.K / TILE_K, tiles_n = st.tiles_n, ntiles = st.ntiles, TN = st.TN;
-                if ((int)blockIdx.x >= ntiles) continue;
+                if (lp_first_tile(st, grid) >= ntiles) continue;
                 tma_prefetch_desc(st.tmap);
                 if (!waited) { pdl_wait(); waited = true; }   // the counters are re-zeroed by the previous run's last CTA
                 spin_until(P.qdone + sidx, grid);
                 LP_STAMP(2);
                 asm volatile("fence.proxy.async.global;" ::: "memory");       // generic-proxy stores -> TMA reads
-                for (int tile = blockIdx.x; tile < ntiles; tile += grid) {
+                for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid) {
                     const int m0 = (tile / tiles_n) * TN;
                     for (int kb = 0; kb < num_kb; kb += KS, ++it) {
                         const uint32_t s = it % ns;
@@ -243,7 +253,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                 const LpStage& st = stages[sidx];
                 const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
                 const uint32_t idesc = umma_idesc_i8(TILE_N, st.TN);
-                for (int tile = blockIdx.x; tile < ntiles; tile += grid, ++ti) {
+                for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid, ++ti) {
                     const uint32_t ab = ti & 1;
                     if (ti >= 2) mbar_wait(bar_acc_empty(ab), ((ti >> 1) & 1) ^ 1);
                     tc_fence_after();
@@ -252,7 +262,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                         const uint32_t s = it % ns;
                         mbar_wait(bar_full(s), (it / ns) & 1);
                         tc_fence_after();
-                        if (kb == 0 && tile == (int)blockIdx.x) LP_STAMP(3);
+                        if (kb == 0 && tile == lp_first_tile(st, grid)) LP_STAMP(3);
 #pragma unroll
                         for (int kk = 0; kk < KS; ++kk) {
                             const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride + kk * LG_A_BYTES);
@@ -278,7 +288,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpStage& st = stages[sidx];
             const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
-            for (int tile = blockIdx.x; tile < ntiles; tile += grid) {
+            for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid) {
                 for (int kb = 0; kb < num_kb; kb += KS, ++it) {
                     if ((int)(it & 1u) != dgrp) continue;
                     const uint32_t sw = it % LG_SW, s = it % ns;
@@ -325,12 +335,12 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpStage& st = stages[sidx];
             const int tiles_n = st.tiles_n, ntiles = st.ntiles, TN = st.TN, M = st.M, nlin = st.grp.n;
-            if ((int)blockIdx.x < ntiles) {
+            if (lp_first_tile(st, grid) < ntiles) {
                 if (threadIdx.x == 11 * 32) spin_until(P.qdone + sidx, grid); // alpha of every row is stored
                 lp_bar(3, 128);
             }
             const float* __restrict__ x_scale = st.xs;
-            for (int tile = blockIdx.x; tile < ntiles; tile += grid, ++ti) {
+            for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid, ++ti) {
                 const int ct = tile % tiles_n, m0 = (tile / tiles_n) * TN;
                 int li = 0;
                 for (int j = 1; j < nlin; ++j) if (ct >= st.grp.ct_begin[j]) li = j;
@@ -396,26 +406,62 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
             if (threadIdx.x == 11 * 32) { LP_STAMP(5); red_release_gpu(P.gdone + sidx, 1u); }
         }
     }
-    else {
-        // ---------------- quantiser groups: run ahead of the GEMM as far as the stages' dependencies allow ----------------
-        const int qg = ((int)threadIdx.x - LG_THREADS) / LP_QT, qt = ((int)threadIdx.x - LG_THREADS) % LP_QT;
-        const int bar_id = 4 + qg;
+    else if (warp < 15 + LP_QW) {
+        // ---------------- quantiser warps: run ahead of the GEMM as far as the stages' dependencies allow ----------------
+        const int qt = (int)threadIdx.x - LG_THREADS;
+        const int bar_id = 4;
         pdl_wait();                                           // x of the first stages may be the previous kernel's output
-        if (qg < P.n_stages) {
-            LpQuantArgs next = lp_quant_args(stages[qg]);
-            for (int sidx = qg; sidx < P.n_stages; sidx += LP_QG) {
-                const LpQuantArgs st = next;
-                if (sidx + LP_QG < P.n_stages) next = lp_quant_args(stages[sidx + LP_QG]);   // its loads fly during this stage's work
-                if (qt == 0 && st.wait_stage >= 0) spin_until(P.gdone + st.wait_stage, grid);
-                lp_bar(bar_id, LP_QT);
-                if (qt == 0) LP_STAMP(0);
+        LpQuantArgs next = lp_quant_args(stages[0]);
+        for (int sidx = 0; sidx < P.n_stages; ++sidx) {
+            const LpQuantArgs st = next;
+            if (sidx + 1 < P.n_stages) next = lp_quant_args(stages[sidx + 1]);       // its loads fly during this stage's work
+            if (qt == 0 && st.wait_stage >= 0) {                // cleared by the publisher warp, usually during the last stage
+                const long long t0 = clock64();
+                unsigned ok;
+                do {
+                    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(ok) : "r"(s_gok) : "memory");
+                    if (clock64() - t0 > (1ll << 32)) __trap();
+                } while (ok <= (unsigned)sidx);
+            }
+            lp_bar(bar_id, LP_QT);
+            if (qt == 0) LP_STAMP(0);
 #ifdef VLA_LP_STAMPS
-                lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, P.stamps + ((size_t)sidx * gridDim.x + blockIdx.x) * 8);
+            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, P.stamps + ((size_t)sidx * gridDim.x + blockIdx.x) * 8);
 #else
-                lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, nullptr);
+            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, nullptr);
 #endif
-                lp_bar(bar_id, LP_QT);                        // every row of this CTA is stored ...
-                if (qt == 0) { LP_STAMP(1); red_release_gpu(P.qdone + sidx, 1u); }      // ... and published
+            // this warp's rows of the stage are stored: tell the publisher warp and go on with the next stage -- the
+            // gpu-scope release (a fence that waits for the stores, ~1 us) is the publisher's, off this chain
+            __syncwarp();
+            if (lane == 0) asm volatile("red.release.cta.shared::cta.add.u32 [%0], 1;" :: "r"(s_qcount) : "memory");
+        }
+    } else {
+        // ---------------- publisher: the quantiser's grid-scope hand-offs, off its chain ----------------
+        // (1) counts the CTA in qdone[s] once all quantiser warps have stored stage s;  (2) clears stage s+1 for the
+        // quantiser (s_gok = stages cleared) once gdone[wait_stage(s+1)] == grid -- polled WHILE the quantiser works on stage
+        // s, except where stage s+1 waits for stage s itself (depends = 1): then qdone[s] has to be published first.
+        if (lane == 0) {
+            pdl_wait();                                       // the counters are re-zeroed by the previous run's last CTA
+            auto clear_stage = [&](int t) {                   // stage t may start quantising
+                const int w = stages[t].wait_stage;
+                if (w >= 0) spin_until(P.gdone + w, grid);
+                asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" :: "r"(s_gok), "r"((unsigned)t + 1u) : "memory");
+            };
+            clear_stage(0);
+            for (int sidx = 0; sidx < P.n_stages; ++sidx) {
+                const bool has_next = sidx + 1 < P.n_stages;
+                const bool next_needs_me = has_next && stages[sidx + 1].wait_stage >= sidx;
+                if (has_next && !next_needs_me) clear_stage(sidx + 1);
+                const unsigned want = (unsigned)LP_QW * (unsigned)(sidx + 1);
+                const long long t0 = clock64();
+                unsigned have;
+                do {
+                    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(have) : "r"(s_qcount) : "memory");
+                    if (clock64() - t0 > (1ll << 32)) __trap();
+                } while (have < want);
+                LP_STAMP(1);
+                red_release_gpu(P.qdone + sidx, 1u);          // cumulative: covers the quantiser warps' stores observed above
+                if (next_needs_me) clear_stage(sidx + 1);
             }
         }
     }

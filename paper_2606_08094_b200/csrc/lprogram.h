@@ -16,14 +16,14 @@ struct alignas(64) LpStage {
     unsigned char tmap[128];   // CUtensorMap of xq [M,K] int8: box [128 k, TN tokens], SWIZZLE_128B
     LgGroup grp;               // the linears that consume x (per-output-group scales), as one [sum N, K] tile walk
     const uint4* x;            // bf16 [M,K]
-    int8_t* xq;                // int8 [M,K]: the caller's xq_opt, else one of the program's two scratch buffers
+    int8_t* xq;                // int8 [M,K]: the caller's xq_opt, else one of the program's scratch sets
     float* xs;                 // alpha [M]: the caller's x_scale_opt, else scratch
     int M, K, TN;
     int wait_stage;            // quantisation of this stage starts after gdone[wait_stage] == grid (-1: at once):
                                // the previous stage if depends = 1, and the last stage that used the same scratch
     int tiles_n, ntiles;       // channel tiles of the group, tiles of the stage
     uint32_t inv_nvec;         // ceil(2^32 / (K/8)): f / (K/8) == umulhi(f, inv_nvec) for the quantiser's task index
-    int pad;
+    int rot;                   // tile t runs on CTA (t + rot) mod grid
 };
 
 struct DevLProg {

@@ -37,13 +37,13 @@ def test_invalid_stage_gives_zero_bytes(vla, bad):
 
 def test_one_kind_per_program_and_large_program_bytes(vla):
     """stages with M > 16 tokens form a LARGE program (persistent tcgen05 kernel): not mixable with small stages; its
-    buffer holds the stage table (tensor map + group per stage), the counters and four {int8 [M,K], alpha [M]} scratch sets"""
+    buffer holds the stage table (tensor map + group per stage), the counters and eight {int8 [M,K], alpha [M]} scratch sets"""
     assert vla.vla_program_bytes([stage(M=8), stage(M=64)]) == 0
     assert vla.vla_program_bytes([stage(M=64), stage(M=16)]) == 0
     one = vla.vla_program_bytes([stage(M=544)])
-    assert one % 256 == 0 and 4 * 544 * 2560 <= one < 4 * 544 * 2560 + 32768
+    assert one % 256 == 0 and 8 * 544 * 2560 <= one < 8 * 544 * 2560 + 65536
     two = vla.vla_program_bytes([stage(M=544), stage(M=100, K=6912, depends=1, n=2)])
-    assert 4 * 544 * 2560 <= two < 4 * 544 * 2560 + 32768 and two > one
+    assert 8 * 544 * 2560 <= two < 8 * 544 * 2560 + 65536 and two > one
 
 
 def test_descriptor_capacity_is_enforced(vla):
