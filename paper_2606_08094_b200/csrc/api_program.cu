@@ -279,10 +279,29 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
     int NS = (vla::LG_STAGE_REGION + vla::LG_SW * vla::LG_W_BYTES - sw_bytes) / stride;
     if (NS > vla::LG_NS_MAX) NS = vla::LG_NS_MAX;
     if (NS < 2) return VLA_ERR_SHAPE;
+    // Row buffer of the fused quantiser: room for the rows a CTA quantises per stage (at most 16 at a time), taken from the
+    // shared memory the pipeline stages leave free; the pipeline gives up stages (down to 3, or 2 with two k blocks per
+    // stage) until at least that many rows, and in any case one row, fit.
+    const int smem_limit = 232448 - 64;
+    auto fixed_bytes = [&](int ns) { return ns * stride + sw_bytes + vla::LG_SCALE_BYTES + 1024 + 8 * vla::LG_NBAR + 16 + vla::LP_EXTRA_SMEM; };
+    int want = 0, one_row = 0;
+    for (int s = 0; s < n_stages; ++s) {
+        const int rows = std::min(16, (S[s].M + std::min(sms, S[s].M) - 1) / std::min(sms, S[s].M));
+        want = std::max(want, rows * S[s].K * 2);
+        one_row = std::max(one_row, S[s].K * 2);
+    }
+    const int ns_floor = KS == 2 ? 2 : 3;
+    while (NS > ns_floor && smem_limit - fixed_bytes(NS) < want) --NS;
+    while (NS > 2 && smem_limit - fixed_bytes(NS) < one_row) --NS;
+    int qbuf = std::min(want, smem_limit - fixed_bytes(NS));
+    qbuf &= ~127;
+    if (qbuf < one_row) return VLA_ERR_SHAPE;
     P->KS = KS;
     P->NS = NS;
     P->x_tile = x_tile;
-    P->smem_bytes = NS * stride + sw_bytes + vla::LG_SCALE_BYTES + 1024 + 8 * vla::LG_NBAR + 16 + vla::LP_EXTRA_SMEM;
+    P->qbuf_bytes = (uint32_t)qbuf;
+    P->pad = 0;
+    P->smem_bytes = fixed_bytes(NS) + qbuf;
     // with the round robin continued across stages (rot), a stage with fewer tiles than SMs leaves the other CTAs to the next
     // stage: size the grid for the whole program, not for its widest stage
     long long all_tiles = 0;

@@ -24,17 +24,17 @@ namespace vla {
 #ifndef VLA_LP_QW
 #define VLA_LP_QW 8
 #endif
-#ifndef VLA_LP_QV
-#define VLA_LP_QV 6
-#endif
 constexpr int LP_QG = VLA_LP_QG;                         // quantiser groups (after the 15 warps of gemm_large_kernel): group i
                                                          // takes the stages s = i (mod LP_QG), so LP_QG latency chains overlap
 constexpr int LP_QW = VLA_LP_QW;                         // warps per group
 constexpr int LP_QT = 32 * LP_QW;
-constexpr int LP_QV = VLA_LP_QV;                         // vectors of 8 bf16 a thread has in flight
+#ifndef VLA_LP_QU
+#define VLA_LP_QU 1
+#endif
+constexpr int LP_QU = VLA_LP_QU;                                 // vectors of 8 bf16 a quantiser thread handles per loop trip
 constexpr int LP_THREADS = LG_THREADS + LP_QG * LP_QT + 32;         // + the publisher warp
 constexpr int LP_QROWS = 16;                             // most rows per round
-static_assert(LP_QG == 1 && LP_EXTRA_SMEM == LP_QROWS * 4 + LP_QROWS * 16, "lprogram.h");
+static_assert(LP_QG == 1 && LP_EXTRA_SMEM >= LP_QROWS * 4 + LP_QROWS * 16 + 16 + 128, "lprogram.h");
 
 #ifdef VLA_LP_STAMPS
 __device__ __forceinline__ unsigned long long lp_now() {
@@ -57,9 +57,11 @@ __device__ __forceinline__ void lp_bar(int id, int threads) {
     asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(threads) : "memory");
 }
 
-// rows blockIdx.x, += gridDim.x of the stage's x -> int8 + alpha, LP_QROWS rows at a time.  Flat tasks of one 8-element
-// vector over the chunk's rows, two streaming passes: absmax (loads only), then quantise (the same vectors again, now L2
-// hits).  Nothing is held in registers between the passes, so a chunk is two latency chains whatever K and M are.
+// rows blockIdx.x, += gridDim.x of the stage's x -> int8 + alpha.  The rows are STAGED IN SHARED MEMORY: one bulk copy (TMA)
+// per row, all rows of a chunk in flight at once (as many rows as fit the program's row buffer, at most LP_QROWS), then the
+// absmax pass and the quantising pass both read shared memory.  x is read from L2 / DRAM exactly once, no registers are
+// held across the passes, and the memory parallelism no longer depends on how many 16-byte loads a thread can keep in
+// flight (the register-held form took 10-11 us per stage at K = 6912, 3 us at K = 2560: DESIGN.md 6c).
 struct LpQuantArgs {           // the quantiser's view of a stage, read from the table BEFORE it waits for the stage's inputs
     const uint4* x;
     uint2* xq;
@@ -75,47 +77,53 @@ __device__ __forceinline__ LpQuantArgs lp_quant_args(const LpStage& st) {
 }
 
 __device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, int tid, int bar_id, unsigned* s_rowmax, float4* s_scale,
+                                               uint32_t qbuf, uint32_t qbuf_bytes, uint32_t bar_q, uint32_t& q_parity,
                                                unsigned long long* dbg) {
     const int grid = (int)gridDim.x, cta = (int)blockIdx.x, nvec = a.nvec, M = a.M;
     const unsigned inv_nvec = a.inv_nvec;
+    const uint32_t row_bytes = (uint32_t)nvec * 16u;
     const uint4* __restrict__ x = a.x;
     uint2* __restrict__ xq = a.xq;
     float* __restrict__ xs = a.xs;
     const int R = M > cta ? (M - cta + grid - 1) / grid : 0;
-    for (int i0 = 0; i0 < R; i0 += LP_QROWS) {
-        const int g = min(LP_QROWS, R - i0), ntask = g * nvec;
+    const int rows_per_chunk = min(LP_QROWS, (int)(qbuf_bytes / row_bytes));
+    for (int i0 = 0; i0 < R; i0 += rows_per_chunk) {
+        const int g = min(rows_per_chunk, R - i0), ntask = g * nvec;
         if (tid < LP_QROWS) s_rowmax[tid] = 0u;
-        lp_bar(bar_id, LP_QT);
-        const bool held = ntask <= LP_QT * LP_QV;                     // one round: the vectors stay in registers
-        uint4 v[LP_QV];
-        int rl[LP_QV];
-        for (int f0 = 0; f0 < ntask; f0 += LP_QT * LP_QV) {           // pass 1: row absmax
-#pragma unroll
-            for (int j = 0; j < LP_QV; ++j) {
-                const int f = f0 + tid + j * LP_QT;
-                rl[j] = -1;
-                v[j] = make_uint4(0, 0, 0, 0);
-                if (f < ntask) {
-                    rl[j] = (int)__umulhi((unsigned)f, inv_nvec);
-                    v[j] = __ldcg(x + ((unsigned)(cta + (i0 + rl[j]) * grid) * (unsigned)nvec + (unsigned)(f - rl[j] * nvec)));   // L2: written by other SMs
-                }
-            }
-#pragma unroll
-            for (int j = 0; j < LP_QV; ++j) {
-                uint32_t m = absmax8_packed(v[j], 0u);
-                m = max(m & 0xFFFFu, m >> 16);
-                const int r0 = __shfl_sync(0xFFFFFFFFu, rl[j], 0);
-                if (__all_sync(0xFFFFFFFFu, rl[j] == r0)) {
-                    m = __reduce_max_sync(0xFFFFFFFFu, m);
-                    if ((tid & 31) == 0 && r0 >= 0) atomicMax(s_rowmax + r0, m);
-                } else if (rl[j] >= 0) {
-                    atomicMax(s_rowmax + rl[j], m);
-                }
-            }
+        lp_bar(bar_id, LP_QT);                                        // (also: everybody is done reading the previous chunk)
+        if (tid == 0) {
+            mbar_arrive_expect_tx(bar_q, (uint32_t)g * row_bytes);
+            for (int j = 0; j < g; ++j)
+                tma_bulk_g2s(qbuf + (uint32_t)j * row_bytes, x + (size_t)(cta + (i0 + j) * grid) * nvec, row_bytes, bar_q);
         }
+        mbar_wait(bar_q, q_parity);
+        q_parity ^= 1u;
 #ifdef VLA_LP_STAMPS
         if (tid == 0 && i0 == 0) dbg[6] = lp_now();
 #endif
+        for (int f0 = tid; (f0 & ~31) < ntask; f0 += LP_QT * LP_QU) { // pass 1: row absmax (LP_QU independent vectors a trip;
+                                                                      // warp-uniform trip count: full-mask shuffles inside)
+            uint4 v[LP_QU];
+#pragma unroll
+            for (int u = 0; u < LP_QU; ++u) {
+                const int f = f0 + u * LP_QT;
+                v[u] = f < ntask ? lds128_nv(qbuf + (uint32_t)f * 16u) : make_uint4(0, 0, 0, 0);
+            }
+#pragma unroll
+            for (int u = 0; u < LP_QU; ++u) {
+                const int f = f0 + u * LP_QT;
+                const int r = f < ntask ? (int)__umulhi((unsigned)f, inv_nvec) : -1;
+                uint32_t m = absmax8_packed(v[u], 0u);
+                m = max(m & 0xFFFFu, m >> 16);
+                const int r0 = __shfl_sync(0xFFFFFFFFu, r, 0);
+                if (__all_sync(0xFFFFFFFFu, r == r0)) {
+                    m = __reduce_max_sync(0xFFFFFFFFu, m);
+                    if ((tid & 31) == 0 && r0 >= 0) atomicMax(s_rowmax + r0, m);
+                } else if (r >= 0) {
+                    atomicMax(s_rowmax + r, m);
+                }
+            }
+        }
         lp_bar(bar_id, LP_QT);
         if (tid < g) {
             const float alpha = alpha_of(bf16lo(s_rowmax[tid]));
@@ -123,23 +131,20 @@ __device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, int tid, in
             xs[cta + (i0 + tid) * grid] = alpha;
         }
         lp_bar(bar_id, LP_QT);
-        for (int f0 = 0; f0 < ntask; f0 += LP_QT * LP_QV) {           // pass 2: quantise
+        for (int f0 = tid; (f0 & ~31) < ntask; f0 += LP_QT * LP_QU) { // pass 2: quantise
+            uint4 v[LP_QU];
 #pragma unroll
-            for (int j = 0; j < LP_QV; ++j) {
-                const int f = f0 + tid + j * LP_QT;
-                if (!held) {
-                    rl[j] = -1;
-                    if (f < ntask) {
-                        rl[j] = (int)__umulhi((unsigned)f, inv_nvec);
-                        v[j] = __ldcg(x + ((unsigned)(cta + (i0 + rl[j]) * grid) * (unsigned)nvec + (unsigned)(f - rl[j] * nvec)));
-                    }
-                }
+            for (int u = 0; u < LP_QU; ++u) {
+                const int f = f0 + u * LP_QT;
+                v[u] = f < ntask ? lds128_nv(qbuf + (uint32_t)f * 16u) : make_uint4(0, 0, 0, 0);
             }
 #pragma unroll
-            for (int j = 0; j < LP_QV; ++j) {
-                const int f = f0 + tid + j * LP_QT;
-                if (rl[j] >= 0)
-                    xq[(unsigned)(cta + (i0 + rl[j]) * grid) * (unsigned)nvec + (unsigned)(f - rl[j] * nvec)] = quant8_fast(v[j], s_scale[rl[j]]);
+            for (int u = 0; u < LP_QU; ++u) {
+                const int f = f0 + u * LP_QT;
+                if (f < ntask) {
+                    const int r = (int)__umulhi((unsigned)f, inv_nvec);
+                    xq[(unsigned)(cta + (i0 + r) * grid) * (unsigned)nvec + (unsigned)(f - r * nvec)] = quant8_fast(v[u], s_scale[r]);
+                }
             }
         }
     }
@@ -174,6 +179,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     float4* s_scale = reinterpret_cast<float4*>(p_tail + 16 + LP_QROWS * 4);
     const uint32_t s_qcount = tmem_slot + 8u;                // quantiser warps that have stored a stage, summed over the stages
     const uint32_t s_gok = tmem_slot + 12u;                  // stages the publisher has cleared for the quantiser
+    const uint32_t bar_q = tmem_slot + 16u + LP_QROWS * 20u;  // the quantiser's row copies have landed
+    const uint32_t qbuf = (bar_q + 16u + 127u) & ~127u;       // row buffer of the quantiser, P.qbuf_bytes
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const unsigned grid = gridDim.x;
@@ -183,6 +190,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         for (int s = 0; s < LG_SW; ++s) { mbar_init(bar_full_w(s), 1); mbar_init(bar_empty_w(s), 4); }
         for (int s = 0; s < LG_NS_MAX; ++s) { mbar_init(bar_full(s), 5); mbar_init(bar_empty(s), 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(bar_acc_full(s), 1); mbar_init(bar_acc_empty(s), 4); }
+        mbar_init(tmem_slot + 16u + LP_QROWS * 20u, 1);
         fence_barrier_init();
         asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 8u), "r"(0u) : "memory");
         asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 12u), "r"(0u) : "memory");
@@ -412,6 +420,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         const int bar_id = 4;
         pdl_wait();                                           // x of the first stages may be the previous kernel's output
         LpQuantArgs next = lp_quant_args(stages[0]);
+        uint32_t q_parity = 0u;
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpQuantArgs st = next;
             if (sidx + 1 < P.n_stages) next = lp_quant_args(stages[sidx + 1]);       // its loads fly during this stage's work
@@ -422,13 +431,14 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                     asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(ok) : "r"(s_gok) : "memory");
                     if (clock64() - t0 > (1ll << 32)) __trap();
                 } while (ok <= (unsigned)sidx);
+                asm volatile("fence.proxy.async.global;" ::: "memory");       // x written by other SMs -> this CTA's bulk copies
             }
             lp_bar(bar_id, LP_QT);
             if (qt == 0) LP_STAMP(0);
 #ifdef VLA_LP_STAMPS
-            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, P.stamps + ((size_t)sidx * gridDim.x + blockIdx.x) * 8);
+            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, qbuf, P.qbuf_bytes, bar_q, q_parity, P.stamps + ((size_t)sidx * gridDim.x + blockIdx.x) * 8);
 #else
-            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, nullptr);
+            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, qbuf, P.qbuf_bytes, bar_q, q_parity, nullptr);
 #endif
             // this warp's rows of the stage are stored: tell the publisher warp and go on with the next stage -- the
             // gpu-scope release (a fence that waits for the stores, ~1 us) is the publisher's, off this chain

@@ -10,7 +10,8 @@
 namespace vla {
 
 constexpr uint32_t LPROG_MAGIC = 0x564C414Cu;   // "VLAL"
-constexpr int LP_EXTRA_SMEM = 16 * 4 + 16 * 16;   // quantiser scratch behind gemm_large's layout: row absmax [16], scales float4 [16]
+constexpr int LP_EXTRA_SMEM = 512;   // behind gemm_large's layout: quantiser row absmax [16], scales float4 [16], its mbarrier, and the
+                                     // alignment slack of its row buffer (DevLProg::qbuf_bytes more bytes follow)
 
 struct alignas(64) LpStage {
     unsigned char tmap[128];   // CUtensorMap of xq [M,K] int8: box [128 k, TN tokens], SWIZZLE_128B
@@ -33,6 +34,8 @@ struct DevLProg {
     int NS;                    // {decoded A, X} pipeline stages
     uint32_t x_tile;           // bytes reserved per X tile (the widest token tile of the program, 1 KiB aligned)
     int smem_bytes;
+    uint32_t qbuf_bytes;       // row buffer of the quantiser (shared memory): holds min(16, qbuf_bytes / (2 K)) rows of x
+    int pad;
     unsigned* qdone;           // [n_stages] CTAs that have quantised their rows of stage s      (target gridDim.x)
     unsigned* gdone;           // [n_stages] CTAs that have stored their tiles of stage s         (target gridDim.x)
     unsigned* done;            // [1]        CTAs past their last counter access; the last one re-zeroes the counters
