@@ -28,10 +28,6 @@ constexpr int LP_QG = VLA_LP_QG;                         // quantiser groups (af
                                                          // takes the stages s = i (mod LP_QG), so LP_QG latency chains overlap
 constexpr int LP_QW = VLA_LP_QW;                         // warps per group
 constexpr int LP_QT = 32 * LP_QW;
-#ifndef VLA_LP_QU
-#define VLA_LP_QU 1
-#endif
-constexpr int LP_QU = VLA_LP_QU;                                 // vectors of 8 bf16 a quantiser thread handles per loop trip
 constexpr int LP_THREADS = LG_THREADS + LP_QG * LP_QT + 32;         // + the publisher warp
 constexpr int LP_QROWS = 16;                             // most rows per round
 static_assert(LP_QG == 1 && LP_EXTRA_SMEM >= LP_QROWS * 4 + LP_QROWS * 16 + 16 + 128, "lprogram.h");
@@ -80,7 +76,6 @@ __device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, int tid, in
                                                uint32_t qbuf, uint32_t qbuf_bytes, uint32_t bar_q, uint32_t& q_parity,
                                                unsigned long long* dbg) {
     const int grid = (int)gridDim.x, cta = (int)blockIdx.x, nvec = a.nvec, M = a.M;
-    const unsigned inv_nvec = a.inv_nvec;
     const uint32_t row_bytes = (uint32_t)nvec * 16u;
     const uint4* __restrict__ x = a.x;
     uint2* __restrict__ xq = a.xq;
@@ -101,51 +96,43 @@ __device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, int tid, in
 #ifdef VLA_LP_STAMPS
         if (tid == 0 && i0 == 0) dbg[6] = lp_now();
 #endif
-        for (int f0 = tid; (f0 & ~31) < ntask; f0 += LP_QT * LP_QU) { // pass 1: row absmax (LP_QU independent vectors a trip;
-                                                                      // warp-uniform trip count: full-mask shuffles inside)
-            uint4 v[LP_QU];
+        // Row r of the chunk belongs to the tpr = LP_QT / rp consecutive threads r * tpr .. (rp = g rounded up to a power of
+        // two: 256 .. 16 threads per row), thread j of them takes vectors j, j + tpr, ...: a thread stays in ONE row, so
+        // the loops carry no warp collectives, no index division and no per-vector scale lookup.
+        int rp = 1;
+        while (rp < g) rp <<= 1;
+        const int tpr = LP_QT / rp, my_row = tid / tpr, j = tid - my_row * tpr;
+        const bool mine = my_row < g;
+        const uint32_t row_s = qbuf + (uint32_t)my_row * row_bytes;
+        uint32_t m = 0u;
+        if (mine) {
+#pragma unroll 4
+            for (int v = j; v < nvec; v += tpr) m = absmax8_packed(lds128_nv(row_s + (uint32_t)v * 16u), m);   // pass 1
+        }
+        m = max(m & 0xFFFFu, m >> 16);
+        if (tpr >= 32) {
+            m = __reduce_max_sync(0xFFFFFFFFu, m);
+            if ((tid & 31) == 0 && mine) atomicMax(s_rowmax + my_row, m);
+        } else {                                                      // 16 threads per row: two rows per warp
 #pragma unroll
-            for (int u = 0; u < LP_QU; ++u) {
-                const int f = f0 + u * LP_QT;
-                v[u] = f < ntask ? lds128_nv(qbuf + (uint32_t)f * 16u) : make_uint4(0, 0, 0, 0);
-            }
-#pragma unroll
-            for (int u = 0; u < LP_QU; ++u) {
-                const int f = f0 + u * LP_QT;
-                const int r = f < ntask ? (int)__umulhi((unsigned)f, inv_nvec) : -1;
-                uint32_t m = absmax8_packed(v[u], 0u);
-                m = max(m & 0xFFFFu, m >> 16);
-                const int r0 = __shfl_sync(0xFFFFFFFFu, r, 0);
-                if (__all_sync(0xFFFFFFFFu, r == r0)) {
-                    m = __reduce_max_sync(0xFFFFFFFFu, m);
-                    if ((tid & 31) == 0 && r0 >= 0) atomicMax(s_rowmax + r0, m);
-                } else if (r >= 0) {
-                    atomicMax(s_rowmax + r, m);
-                }
-            }
+            for (int o = 8; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+            if ((tid & 15) == 0 && mine) atomicMax(s_rowmax + my_row, m);
         }
         lp_bar(bar_id, LP_QT);
+#ifdef VLA_LP_STAMPS
+        if (tid == 0 && i0 == 0) dbg[7] = lp_now();
+#endif
         if (tid < g) {
             const float alpha = alpha_of(bf16lo(s_rowmax[tid]));
             s_scale[tid] = quant_scales_of_alpha(alpha);
             xs[cta + (i0 + tid) * grid] = alpha;
         }
         lp_bar(bar_id, LP_QT);
-        for (int f0 = tid; (f0 & ~31) < ntask; f0 += LP_QT * LP_QU) { // pass 2: quantise
-            uint4 v[LP_QU];
-#pragma unroll
-            for (int u = 0; u < LP_QU; ++u) {
-                const int f = f0 + u * LP_QT;
-                v[u] = f < ntask ? lds128_nv(qbuf + (uint32_t)f * 16u) : make_uint4(0, 0, 0, 0);
-            }
-#pragma unroll
-            for (int u = 0; u < LP_QU; ++u) {
-                const int f = f0 + u * LP_QT;
-                if (f < ntask) {
-                    const int r = (int)__umulhi((unsigned)f, inv_nvec);
-                    xq[(unsigned)(cta + (i0 + r) * grid) * (unsigned)nvec + (unsigned)(f - r * nvec)] = quant8_fast(v[u], s_scale[r]);
-                }
-            }
+        if (mine) {
+            const float4 sc = s_scale[my_row];
+            uint2* __restrict__ dst = xq + (size_t)(cta + (i0 + my_row) * grid) * nvec;
+#pragma unroll 2
+            for (int v = j; v < nvec; v += tpr) dst[v] = quant8_fast(lds128_nv(row_s + (uint32_t)v * 16u), sc);      // pass 2
         }
     }
 }
