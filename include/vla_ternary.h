@@ -221,6 +221,12 @@ typedef struct {
 } vla_copy;
 vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in /*host*/, int n_in,
                                 const vla_copy* out /*host*/, int n_out, void* stream);
+/* The same WITHOUT the final synchronisation: the three parts are only enqueued on `stream`.  A serving loop alternates two
+ * programs (each with its own device and pinned host buffers) on two streams, so that the host->device copy of step t+1
+ * and the device->host copy of step t-1 overlap the kernel of step t; the caller synchronises `stream` (or an event
+ * recorded on it) before it reads an `out` host buffer or rewrites an `in` host buffer. */
+vla_status vla_program_run_host_async(const void* prog_dev, const vla_copy* in /*host*/, int n_in,
+                                      const vla_copy* out /*host*/, int n_out, void* stream);
 
 /* Forgets a compiled program (the caller then frees prog_dev). */
 vla_status vla_program_release(const void* prog_dev);

@@ -27,7 +27,7 @@ EXPORTS = [
     "vla_ternary_host_workspace_bytes", "vla_ternary_linear_static",
     "vla_ternary_auto_path", "vla_i8_mma_issue_probe", "vla_status_string", "vla_launch_count",
     "vla_cached_attention", "vla_cached_attention_workspace_bytes",
-    "vla_ternary_gemm_grouped", "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_run_host", "vla_program_release",
+    "vla_ternary_gemm_grouped", "vla_program_bytes", "vla_program_build", "vla_program_run", "vla_program_run_host", "vla_program_run_host_async", "vla_program_release",
 ]
 
 
@@ -98,6 +98,8 @@ def _load():
     lib.vla_ternary_gemm_grouped.argtypes = [ctypes.POINTER(vla_prog_linear), i, vp, vp, i, i, i, vp]
     lib.vla_program_run_host.restype = st
     lib.vla_program_run_host.argtypes = [vp, ctypes.POINTER(vla_copy), i, ctypes.POINTER(vla_copy), i, vp]
+    lib.vla_program_run_host_async.restype = st
+    lib.vla_program_run_host_async.argtypes = [vp, ctypes.POINTER(vla_copy), i, ctypes.POINTER(vla_copy), i, vp]
     lib.vla_program_release.restype = st
     lib.vla_program_release.argtypes = [vp]
     lib.vla_cached_attention_workspace_bytes.restype = sz
@@ -267,6 +269,12 @@ def vla_program_run_host(prog_dev, copies_in, copies_out, stream=None):
     """copies_in / copies_out: ctypes arrays from make_copies.  Synchronises the stream."""
     _check(_lib.vla_program_run_host(_ptr(prog_dev), copies_in, len(copies_in), copies_out, len(copies_out),
                                      _stream(stream)), "vla_program_run_host")
+
+
+def vla_program_run_host_async(prog_dev, copies_in, copies_out, stream=None):
+    """vla_program_run_host without the final synchronisation (the caller synchronises the stream or an event on it)."""
+    _check(_lib.vla_program_run_host_async(_ptr(prog_dev), copies_in, len(copies_in), copies_out, len(copies_out),
+                                           _stream(stream)), "vla_program_run_host_async")
 
 
 def vla_cached_attention_workspace_bytes(Mq, Mc, n_q_heads, n_kv_heads, d_k):

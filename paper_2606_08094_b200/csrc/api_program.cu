@@ -549,8 +549,8 @@ vla_status vla_program_run(const void* prog_dev, void* stream) {
     return VLA_OK;
 }
 
-vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in, int n_in, const vla_copy* out, int n_out,
-                                void* stream) {
+vla_status vla_program_run_host_async(const void* prog_dev, const vla_copy* in, int n_in, const vla_copy* out, int n_out,
+                                      void* stream) {
     if (!prog_dev || (n_in > 0 && !in) || (n_out > 0 && !out)) return VLA_ERR_NULL;
     if (n_in < 0 || n_out < 0) return VLA_ERR_SHAPE;
     for (int i = 0; i < n_in; ++i) if (!in[i].host || !in[i].dev) return VLA_ERR_NULL;
@@ -568,7 +568,14 @@ vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in, int n_
             cudaGetLastError();
             return VLA_ERR_CUDA;
         }
-    if (cudaStreamSynchronize(cs) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+    return VLA_OK;
+}
+
+vla_status vla_program_run_host(const void* prog_dev, const vla_copy* in, int n_in, const vla_copy* out, int n_out,
+                                void* stream) {
+    vla_status st = vla_program_run_host_async(prog_dev, in, n_in, out, n_out, stream);
+    if (st != VLA_OK) return st;
+    if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     return VLA_OK;
 }
 
