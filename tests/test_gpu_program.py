@@ -405,3 +405,38 @@ def test_guard_bands_and_repeatability(vla, oracle):
     assert np.array_equal(xq.cpu().numpy(), refs[0][0]["a"])
     assert np.array_equal(bits(out2), oracle.ternary_linear(x2_bits, w2, b2)["ybf16"])
     assert all(_guards_intact(r) for r in raws), "a kernel wrote outside its buffer"
+
+
+def test_program_run_host_sync_and_async_pipeline(vla, oracle):
+    """vla_program_run_host (synchronous) and vla_program_run_host_async on two buffer sets / two streams (the serving loop
+    of bench.py's end-to-end leg): pinned host x -> device -> program -> pinned host y, every output vs the oracle."""
+    sets = []
+    for b in range(2):
+        pts = [make_point(vla, M, K, N, 9800 + 10 * b + i, vla.VLA_BF16) for i, (M, K, N) in enumerate([(8, 2560, 640), (16, 640, 256)])]
+        hx = [torch.empty(p["x"].shape, dtype=torch.bfloat16).pin_memory() for p in pts]
+        hy = [torch.zeros(p["out"].shape, dtype=torch.bfloat16).pin_memory() for p in pts]
+        for h, p in zip(hx, pts):
+            h.copy_(p["x"].cpu())
+            p["x"].zero_()                                   # the device copy must come from the host buffer
+        prog = vla.compile_program([stage_of(p) for p in pts])
+        cin = vla.make_copies([(h, p["x"]) for h, p in zip(hx, pts)])
+        cout = vla.make_copies([(h, p["out"]) for h, p in zip(hy, pts)])
+        sets.append(dict(pts=pts, hx=hx, hy=hy, prog=prog, cin=cin, cout=cout, stream=torch.cuda.Stream()))
+
+    def check(s):
+        for h, p in zip(s["hy"], s["pts"]):
+            ref = oracle.ternary_linear(p["x_bits"], p["w"], p["beta"])
+            assert np.array_equal(h.view(torch.int16).numpy().view(np.uint16), ref["ybf16"])
+            h.zero_()
+
+    vla.vla_program_run_host(sets[0]["prog"], sets[0]["cin"], sets[0]["cout"])          # synchronous: results are there
+    check(sets[0])
+    torch.cuda.synchronize()
+    for rep in range(3):                                     # asynchronous, alternating sets and streams
+        for s in sets:
+            vla.vla_program_run_host_async(s["prog"], s["cin"], s["cout"], s["stream"])
+        for s in sets:
+            s["stream"].synchronize()
+            check(s)
+    for s in sets:
+        vla.vla_program_release(s["prog"])

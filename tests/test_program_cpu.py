@@ -64,6 +64,8 @@ def test_build_and_run_validate_on_the_host(vla):
     assert L.vla_program_run(FAKE, None) == vla.VLA_ERR_VALUE          # never compiled
     assert L.vla_program_release(FAKE) == vla.VLA_ERR_VALUE
     assert L.vla_program_run_host(FAKE, None, 1, None, 0, None) == vla.VLA_ERR_NULL
+    assert L.vla_program_run_host_async(FAKE, None, 1, None, 0, None) == vla.VLA_ERR_NULL
+    assert L.vla_program_run_host_async(FAKE, None, 0, None, 0, None) == vla.VLA_ERR_VALUE     # never compiled
 
 
 def test_no_gpu_means_arch_error(vla):
