@@ -8,8 +8,10 @@
 //   MMA operand B = int8 activations [TN tok  x 128 k] int8, K-major, SWIZZLE_128B  (written by TMA)
 //   D (TMEM)      = int32 [128 lanes = channels] x [TN columns = tokens], TWO buffers (columns 0.. and 256..)
 // Warp roles (15 warps):
-//   warp 0       W producer: cp.async.bulk of the four 1 KiB pieces of the packed weight tile per k block, 6-deep ring (weights never
-//                depend on the previous kernel, so this starts before griddepcontrol.wait)
+//   warp 0       W producer: cp.async.bulk of the four 32-channel pieces of the packed weight tile per pipeline stage, KS KiB
+//                each (the k blocks of a piece are contiguous; 1 KiB copies cap the chip at 3.7 TB/s = 0.164 us per k block
+//                per SM, above the MMA time of narrow tiles), 6-deep ring (weights never depend on the previous kernel, so
+//                this starts before griddepcontrol.wait)
 //   warp 1       X producer: tensor-map (TMA) load of the [TN x 128] activation tile per k block, 4-deep ring
 //   warp 2       TMEM allocator; one lane issues tcgen05.mma.cta_group::1.kind::i8 (4 x K=32 per k block)
 //   warps 3-10   decode: packed words (smem) -> int8 (64*q) -> swizzled A tile (3-deep ring); fence.proxy.async
@@ -76,8 +78,8 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     if (warp == 0) {
         // ---------------- W producer ----------------
         // a 128 x 128 tile is four 1 KiB pieces (one per 32-channel group), 8*K bytes apart: lanes 0-3 copy one each
-        if (lane < 4 * KS) {
-            const int piece = lane & 3, kk = lane >> 2;
+        if (lane < 4) {                                       // one copy per 32-channel piece: its KS k blocks are contiguous
+            const int piece = lane;
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const int ct = tile % tiles_n;
@@ -89,8 +91,8 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
                     const uint32_t s = it % LG_SW;
                     if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
                     if (lane == 0) mbar_arrive_expect_tx(bar_full_w(s), W_STAGE);
-                    __syncwarp((1u << (4 * KS)) - 1u);
-                    tma_bulk_g2s(sW + s * W_STAGE + kk * LG_W_BYTES + piece * 1024, wsrc + (size_t)(kb + kk) * 1024, 1024, bar_full_w(s));
+                    __syncwarp(0xFu);
+                    tma_bulk_g2s(sW + s * W_STAGE + piece * (KS * 1024), wsrc + (size_t)kb * 1024, KS * 1024, bar_full_w(s));
                 }
             }
         }
@@ -99,11 +101,12 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         if (lane == 0) {
             pdl_wait();                                       // activations come from the previous kernel
             uint32_t it = 0;
+            RingCur cx;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const int m0 = (tile / tiles_n) * TN;
-                for (int kb = 0; kb < num_kb; kb += KS, ++it) {
-                    const uint32_t s = it % ns;
-                    if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
+                for (int kb = 0; kb < num_kb; kb += KS, ++it, cx.next(ns)) {
+                    const uint32_t s = cx.s;
+                    if (cx.wrapped) mbar_wait(bar_empty(s), cx.ph ^ 1u);
                     mbar_arrive_expect_tx(bar_full(s), (uint32_t)KS * TN * TILE_K);
 #pragma unroll
                     for (int kk = 0; kk < KS; ++kk)
@@ -115,20 +118,23 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         // ---------------- MMA issuer: one wait, four MMAs, one commit per k block ----------------
         if (lane == 0) {
             const uint32_t idesc = umma_idesc_i8(TILE_N, TN);
+            const uint64_t desc0 = umma_desc_k_sw128(sS);
             uint32_t it = 0, ti = 0;
+            RingCur cm;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++ti) {
                 const uint32_t ab = ti & 1;
                 if (ti >= 2) mbar_wait(bar_acc_empty(ab), ((ti >> 1) & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + ab * 256u;
-                for (int kb = 0; kb < num_kb; kb += KS, ++it) {
-                    const uint32_t s = it % ns;
-                    mbar_wait(bar_full(s), (it / ns) & 1);
+                for (int kb = 0; kb < num_kb; kb += KS, ++it, cm.next(ns)) {
+                    const uint32_t s = cm.s;
+                    mbar_wait(bar_full(s), cm.ph);
                     tc_fence_after();
 #pragma unroll
                     for (int kk = 0; kk < KS; ++kk) {
-                        const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride + kk * LG_A_BYTES);
-                        const uint64_t b_desc = umma_desc_k_sw128(sS + s * stride + X_OFF + kk * x_tile);
+                        // (descriptor = constant fields + (shared address >> 4): only the address part moves)
+                        const uint64_t a_desc = desc0 + ((s * stride + kk * LG_A_BYTES) >> 4);
+                        const uint64_t b_desc = desc0 + ((s * stride + X_OFF + kk * x_tile) >> 4);
 #pragma unroll
                         for (int k = 0; k < TILE_K / 32; ++k)
                             mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | kk | k) != 0);
@@ -145,10 +151,11 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
         const int g = 2 * q + p;
         uint32_t it = 0;
+            RingCur cd;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            for (int kb = 0; kb < num_kb; kb += KS, ++it) {
+            for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns)) {
                 if ((int)(it & 1u) != dgrp) continue;
-                const uint32_t sw = it % LG_SW, s = it % ns;
+                const uint32_t sw = it % LG_SW, s = cd.s;
                 mbar_wait(bar_full_w(sw), (it / LG_SW) & 1);
                 const uint8_t* wst = pW + sw * W_STAGE;
                 uint4 wv[KS][2];
@@ -156,8 +163,8 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
                 for (int kk = 0; kk < KS; ++kk)
 #pragma unroll
                     for (int itx = 0; itx < 2; ++itx)
-                        wv[kk][itx] = *reinterpret_cast<const uint4*>(wst + kk * LG_W_BYTES + ((i32 * 2 + (p ^ itx)) * 32 + g * 4 + t) * 16);
-                if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
+                        wv[kk][itx] = *reinterpret_cast<const uint4*>(wst + i32 * (KS * 1024) + kk * 1024 + ((p ^ itx) * 32 + g * 4 + t) * 16);
+                if (cd.wrapped) mbar_wait(bar_empty(s), cd.ph ^ 1u);
 #pragma unroll
                 for (int kk = 0; kk < KS; ++kk) {
                     uint8_t* ast = pS + s * stride + kk * LG_A_BYTES;

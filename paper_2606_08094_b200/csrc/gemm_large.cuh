@@ -24,6 +24,15 @@ __device__ __forceinline__ uint4 lds128_nv(uint32_t addr) {
     return r;
 }
 
+// Cursor over a ring of `n` slots walked once per pipeline iteration: slot, phase parity of the slot's CURRENT use, and whether
+// the ring has wrapped (= the slot has been used before).  Kept incrementally: `it % n` and `it / n` with a run-time n cost
+// ~50 dependent instructions per iteration in the single-thread roles (the MMA-issuing lane, the producers).
+struct RingCur {
+    uint32_t s = 0, ph = 0;
+    bool wrapped = false;
+    __device__ __forceinline__ void next(uint32_t n) { if (++s == n) { s = 0; ph ^= 1u; wrapped = true; } }
+};
+
 // Token-tile width TN (multiple of 16, <= 256) for a persistent grid of `sms` CTAs (gemm_large.cu)
 int lg_pick_tn(int M, int N, int sms, bool k_even);
 // tensor map (128 bytes, 64-byte aligned) of the int8 activations xq [M,K] for token tiles of TN

@@ -191,8 +191,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
 
     if (warp == 0) {
         // ---------------- W producer: runs ahead across stage boundaries (weights depend on nothing) ----------------
-        if (lane < 4 * KS) {
-            const int piece = lane & 3, kk = lane >> 2;
+        if (lane < 4) {                                       // one copy per 32-channel piece: its KS k blocks are contiguous
+            const int piece = lane;
             uint32_t it = 0;
             for (int sidx = 0; sidx < P.n_stages; ++sidx) {
                 const LpStage& st = stages[sidx];
@@ -207,8 +207,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                         const uint32_t s = it % LG_SW;
                         if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
                         if (lane == 0) mbar_arrive_expect_tx(bar_full_w(s), W_STAGE);
-                        __syncwarp((1u << (4 * KS)) - 1u);
-                        tma_bulk_g2s(sW + s * W_STAGE + kk * LG_W_BYTES + piece * 1024, wsrc + (size_t)(kb + kk) * 1024, 1024, bar_full_w(s));
+                        __syncwarp(0xFu);
+                        tma_bulk_g2s(sW + s * W_STAGE + piece * (KS * 1024), wsrc + (size_t)kb * 1024, KS * 1024, bar_full_w(s));
                     }
                 }
             }
@@ -217,6 +217,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         // ---------------- X producer: a stage's activations exist once every CTA has quantised its rows ----------------
         if (lane == 0) {
             uint32_t it = 0;
+            RingCur cx;
             bool waited = false;
             for (int sidx = 0; sidx < P.n_stages; ++sidx) {
                 const LpStage& st = stages[sidx];
@@ -229,9 +230,9 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                 asm volatile("fence.proxy.async.global;" ::: "memory");       // generic-proxy stores -> TMA reads
                 for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid) {
                     const int m0 = (tile / tiles_n) * TN;
-                    for (int kb = 0; kb < num_kb; kb += KS, ++it) {
-                        const uint32_t s = it % ns;
-                        if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
+                    for (int kb = 0; kb < num_kb; kb += KS, ++it, cx.next(ns)) {
+                        const uint32_t s = cx.s;
+                        if (cx.wrapped) mbar_wait(bar_empty(s), cx.ph ^ 1u);
                         mbar_arrive_expect_tx(bar_full(s), (uint32_t)KS * TN * TILE_K);
 #pragma unroll
                         for (int kk = 0; kk < KS; ++kk)
@@ -243,7 +244,9 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     } else if (warp == 2) {
         // ---------------- MMA issuer ----------------
         if (lane == 0) {
+            const uint64_t desc0 = umma_desc_k_sw128(sS);
             uint32_t it = 0, ti = 0;
+            RingCur cm;
             for (int sidx = 0; sidx < P.n_stages; ++sidx) {
                 const LpStage& st = stages[sidx];
                 const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
@@ -253,15 +256,16 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                     if (ti >= 2) mbar_wait(bar_acc_empty(ab), ((ti >> 1) & 1) ^ 1);
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + ab * 256u;
-                    for (int kb = 0; kb < num_kb; kb += KS, ++it) {
-                        const uint32_t s = it % ns;
-                        mbar_wait(bar_full(s), (it / ns) & 1);
+                    for (int kb = 0; kb < num_kb; kb += KS, ++it, cm.next(ns)) {
+                        const uint32_t s = cm.s;
+                        mbar_wait(bar_full(s), cm.ph);
                         tc_fence_after();
                         if (kb == 0 && tile == lp_first_tile(st, grid)) LP_STAMP(3);
 #pragma unroll
                         for (int kk = 0; kk < KS; ++kk) {
-                            const uint64_t a_desc = umma_desc_k_sw128(sS + s * stride + kk * LG_A_BYTES);
-                            const uint64_t b_desc = umma_desc_k_sw128(sS + s * stride + X_OFF + kk * x_tile);
+                            // (descriptor = constant fields + (shared address >> 4): only the address part moves)
+                            const uint64_t a_desc = desc0 + ((s * stride + kk * LG_A_BYTES) >> 4);
+                            const uint64_t b_desc = desc0 + ((s * stride + X_OFF + kk * x_tile) >> 4);
 #pragma unroll
                             for (int k = 0; k < TILE_K / 32; ++k)
                                 mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | kk | k) != 0);
@@ -280,13 +284,14 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
         const int g = 2 * q + p;
         uint32_t it = 0;
+            RingCur cd;
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpStage& st = stages[sidx];
             const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
             for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid) {
-                for (int kb = 0; kb < num_kb; kb += KS, ++it) {
+                for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns)) {
                     if ((int)(it & 1u) != dgrp) continue;
-                    const uint32_t sw = it % LG_SW, s = it % ns;
+                    const uint32_t sw = it % LG_SW, s = cd.s;
                     mbar_wait(bar_full_w(sw), (it / LG_SW) & 1);
                     const uint8_t* wst = pW + sw * W_STAGE;
                     uint4 wv[KS][2];
@@ -294,8 +299,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                     for (int kk = 0; kk < KS; ++kk)
 #pragma unroll
                         for (int itx = 0; itx < 2; ++itx)
-                            wv[kk][itx] = *reinterpret_cast<const uint4*>(wst + kk * LG_W_BYTES + ((i32 * 2 + (p ^ itx)) * 32 + g * 4 + t) * 16);
-                    if (it >= ns) mbar_wait(bar_empty(s), ((it / ns) & 1) ^ 1);
+                            wv[kk][itx] = *reinterpret_cast<const uint4*>(wst + i32 * (KS * 1024) + kk * 1024 + ((p ^ itx) * 32 + g * 4 + t) * 16);
+                    if (cd.wrapped) mbar_wait(bar_empty(s), cd.ph ^ 1u);
 #pragma unroll
                     for (int kk = 0; kk < KS; ++kk) {
                         uint8_t* ast = pS + s * stride + kk * LG_A_BYTES;
