@@ -275,15 +275,14 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         if (vla::lg_encode_x_map(d.tmap, d.xq, a.M, a.K, d.TN) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     }
     const int stride = KS * (vla::LG_A_BYTES + (int)x_tile);
-    const int sw_bytes = vla::LG_SW * KS * vla::LG_W_BYTES;
-    int NS = (vla::LG_STAGE_REGION + vla::LG_SW * vla::LG_W_BYTES - sw_bytes) / stride;
-    if (NS > vla::LG_NS_MAX) NS = vla::LG_NS_MAX;
-    if (NS < 2) return VLA_ERR_SHAPE;
-    // Row buffer of the fused quantiser: room for the rows a CTA quantises per stage (at most 16 at a time), taken from the
-    // shared memory the pipeline stages leave free; the pipeline gives up stages (down to 3, or 2 with two k blocks per
-    // stage) until at least that many rows, and in any case one row, fit.
-    const int smem_limit = 232448 - 64;
-    auto fixed_bytes = [&](int ns) { return ns * stride + sw_bytes + vla::LG_SCALE_BYTES + 1024 + 8 * vla::LG_NBAR + 16 + vla::LP_EXTRA_SMEM; };
+    // Shared memory: NS {decoded A, X} pipeline stages, NSW packed-weight stages, and the row buffer of the fused quantiser --
+    // room for the rows a CTA quantises per stage (at most 16 at a time), in any case for one row.  As many pipeline stages
+    // as fit beside the row buffer and a 6-deep weight ring (at least 3, or 2 with two k blocks per stage); one more if a 5-
+    // or 4-deep weight ring makes room for it.
+    const int smem_limit = vla::LG_SMEM_LIMIT - 64;
+    auto fixed_bytes = [&](int ns, int nsw) {
+        return ns * stride + nsw * KS * vla::LG_W_BYTES + vla::LG_SCALE_BYTES + 1024 + 8 * vla::LG_NBAR + 16 + vla::LP_EXTRA_SMEM;
+    };
     int want = 0, one_row = 0;
     for (int s = 0; s < n_stages; ++s) {
         const int rows = std::min(16, (S[s].M + std::min(sms, S[s].M) - 1) / std::min(sms, S[s].M));
@@ -291,17 +290,23 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         one_row = std::max(one_row, S[s].K * 2);
     }
     const int ns_floor = KS == 2 ? 2 : 3;
-    while (NS > ns_floor && smem_limit - fixed_bytes(NS) < want) --NS;
-    while (NS > 2 && smem_limit - fixed_bytes(NS) < one_row) --NS;
-    int qbuf = std::min(want, smem_limit - fixed_bytes(NS));
+    int NS = 0, NSW = vla::LG_SW;
+    for (int nsw = vla::LG_SW; nsw >= 4; --nsw) {
+        int ns = (smem_limit - fixed_bytes(0, nsw) - want) / stride;                  // with the whole row buffer
+        if (ns < ns_floor) ns = std::min(ns_floor, (smem_limit - fixed_bytes(0, nsw) - one_row) / stride);   // with a smaller one
+        if (ns > vla::LG_NS_MAX) ns = vla::LG_NS_MAX;
+        if (ns > NS) { NS = ns; NSW = nsw; }
+    }
+    if (NS < 2) return VLA_ERR_SHAPE;
+    int qbuf = std::min(want, smem_limit - fixed_bytes(NS, NSW));
     qbuf &= ~127;
     if (qbuf < one_row) return VLA_ERR_SHAPE;
     P->KS = KS;
     P->NS = NS;
+    P->NSW = NSW;
     P->x_tile = x_tile;
     P->qbuf_bytes = (uint32_t)qbuf;
-    P->pad = 0;
-    P->smem_bytes = fixed_bytes(NS) + qbuf;
+    P->smem_bytes = fixed_bytes(NS, NSW) + qbuf;
     // with the round robin continued across stages (rot), a stage with fewer tiles than SMs leaves the other CTAs to the next
     // stage: size the grid for the whole program, not for its widest stage
     long long all_tiles = 0;

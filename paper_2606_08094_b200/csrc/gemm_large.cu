@@ -29,7 +29,7 @@ namespace vla {
 template <int KS>
 __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ LgGroup grp,
-    const float* __restrict__ x_scale, int M, int K, int TN, int NS) {
+    const float* __restrict__ x_scale, int M, int K, int TN, int NS, int NSW) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
@@ -39,10 +39,11 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
     constexpr uint32_t W_STAGE = KS * LG_W_BYTES;
     const uint32_t sS = base;                                           // [NS]{A 16384 | X TN*128}
     const uint32_t sW = sS + (uint32_t)NS * stride;                     // [SW][4096]
-    const uint32_t sBar = sW + LG_SW * W_STAGE + LG_SCALE_BYTES;
+    const uint32_t nsw = (uint32_t)NSW;                                 // packed-weight stages in use (<= LG_SW)
+    const uint32_t sBar = sW + nsw * W_STAGE + LG_SCALE_BYTES;
     uint8_t* pS = base_ptr;
     uint8_t* pW = base_ptr + (size_t)NS * stride;
-    float* pScale = reinterpret_cast<float*>(pW + LG_SW * W_STAGE);
+    float* pScale = reinterpret_cast<float*>(pW + nsw * W_STAGE);
     auto bar_full_w = [&](uint32_t s) { return sBar + 8u * s; };
     auto bar_empty_w = [&](uint32_t s) { return sBar + 8u * (LG_SW + s); };
     auto bar_full = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + s); };                  // A decoded + X landed
@@ -81,15 +82,16 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         if (lane < 4) {                                       // one copy per 32-channel piece: its KS k blocks are contiguous
             const int piece = lane;
             uint32_t it = 0;
+            RingCur cw;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const int ct = tile % tiles_n;
                 int li = 0;
                 for (int j = 1; j < grp.n; ++j) if (ct >= grp.ct_begin[j]) li = j;
                 const int nb = ct - grp.ct_begin[li];
                 const uint8_t* wsrc = grp.packed[li] + (size_t)(nb * 4 + piece) * num_kb * 1024;
-                for (int kb = 0; kb < num_kb; kb += KS, ++it) {
-                    const uint32_t s = it % LG_SW;
-                    if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
+                for (int kb = 0; kb < num_kb; kb += KS, ++it, cw.next(nsw)) {
+                    const uint32_t s = cw.s;
+                    if (cw.wrapped) mbar_wait(bar_empty_w(s), cw.ph ^ 1u);
                     if (lane == 0) mbar_arrive_expect_tx(bar_full_w(s), W_STAGE);
                     __syncwarp(0xFu);
                     tma_bulk_g2s(sW + s * W_STAGE + piece * (KS * 1024), wsrc + (size_t)kb * 1024, KS * 1024, bar_full_w(s));
@@ -151,12 +153,12 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
         const int g = 2 * q + p;
         uint32_t it = 0;
-            RingCur cd;
+            RingCur cd, cdw;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns)) {
+            for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns), cdw.next(nsw)) {
                 if ((int)(it & 1u) != dgrp) continue;
-                const uint32_t sw = it % LG_SW, s = cd.s;
-                mbar_wait(bar_full_w(sw), (it / LG_SW) & 1);
+                const uint32_t sw = cdw.s, s = cd.s;
+                mbar_wait(bar_full_w(sw), cdw.ph);
                 const uint8_t* wst = pW + sw * W_STAGE;
                 uint4 wv[KS][2];
 #pragma unroll
@@ -192,7 +194,7 @@ __global__ void __launch_bounds__(LG_THREADS, 1) gemm_large_kernel(
         // ---------------- epilogue warps ----------------
         const int lq = warp & 3;                              // TMEM lane quarter this warp may read
         float* sc = pScale + lq * 256;                        // this warp's alpha_m * beta of the tile's tokens
-        const uint32_t sc_addr = sW + LG_SW * W_STAGE + (uint32_t)lq * 1024u;
+        const uint32_t sc_addr = sW + nsw * W_STAGE + (uint32_t)lq * 1024u;
         pdl_wait();                                           // x_scale comes from the previous kernel
         uint32_t ti = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++ti) {
@@ -329,8 +331,8 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     }
 
     {   // function attributes are per device: set on every launch (cheap), no process-wide cache
-        cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_large_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_STAGE_REGION + LG_FIXED_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(gemm_large_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_SMEM_LIMIT);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_large_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, LG_SMEM_LIMIT);
         if (e != cudaSuccess) return e;
     }
     const int ntiles = (N / TILE_N) * ((M + TN - 1) / TN);
@@ -338,10 +340,15 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     // so four of them do not cover one full/empty handoff; eight do)
     const int KS = lg_pick_ks(TN, K);
     const int stage = KS * (int)lg_stage_stride(TN);
-    const int sw_bytes = LG_SW * KS * LG_W_BYTES;
-    int NS = (LG_STAGE_REGION + LG_SW * LG_W_BYTES - sw_bytes) / stage;
-    if (NS > LG_NS_MAX) NS = LG_NS_MAX;
-    const int smem = NS * stage + sw_bytes + LG_SCALE_BYTES + 1024 + 8 * LG_NBAR + 16;
+    // pipeline stages NS and packed-weight stages NSW from the shared memory there is: as many {A, X} stages as fit beside a
+    // 6-deep weight ring, one more if a 5- or 4-deep ring makes room for it (TN = 112 with two k blocks per stage: 3, not 2)
+    int NS = 0, NSW = LG_SW;
+    for (int nsw = LG_SW; nsw >= 4; --nsw) {
+        int ns = (LG_SMEM_LIMIT - (LG_SCALE_BYTES + 1024 + 8 * LG_NBAR + 16) - nsw * KS * LG_W_BYTES) / stage;
+        if (ns > LG_NS_MAX) ns = LG_NS_MAX;
+        if (ns > NS) { NS = ns; NSW = nsw; }
+    }
+    const int smem = NS * stage + NSW * KS * LG_W_BYTES + LG_SCALE_BYTES + 1024 + 8 * LG_NBAR + 16;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(ntiles < sms ? ntiles : sms));
     cfg.blockDim = dim3(LG_THREADS);
@@ -353,8 +360,8 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     cfg.attrs = at;
     cfg.numAttrs = 1;
     count_launch();
-    if (KS == 2) return cudaLaunchKernelEx(&cfg, gemm_large_kernel<2>, tm, g, x_scale, M, K, TN, NS);
-    return cudaLaunchKernelEx(&cfg, gemm_large_kernel<1>, tm, g, x_scale, M, K, TN, NS);
+    if (KS == 2) return cudaLaunchKernelEx(&cfg, gemm_large_kernel<2>, tm, g, x_scale, M, K, TN, NS, NSW);
+    return cudaLaunchKernelEx(&cfg, gemm_large_kernel<1>, tm, g, x_scale, M, K, TN, NS, NSW);
 }
 
 cudaError_t launch_gemm_large(const void* packed, const float* w_scale, const int8_t* xq, const float* x_scale,

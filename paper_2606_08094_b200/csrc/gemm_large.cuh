@@ -7,14 +7,13 @@
 namespace vla {
 
 constexpr int LG_THREADS = 15 * 32;
-constexpr int LG_SW = 6;                                // packed-weight stages (4 KiB each)
+constexpr int LG_SW = 6;                                // most packed-weight stages (4 KiB per k block each)
+constexpr int LG_SMEM_LIMIT = 232448;                   // dynamic shared memory a CTA may opt in to (227 KB)
 constexpr int LG_NS_MAX = 8;                            // {decoded A, X} stages
 constexpr int LG_A_BYTES = TILE_N * TILE_K;             // 16384 decoded int8
 constexpr int LG_W_BYTES = TILE_BYTES;                  // 4096 packed
-constexpr int LG_STAGE_REGION = 192 * 1024;             // 4 stages at TN = 256, 6 at TN = 96
 constexpr int LG_SCALE_BYTES = 4 * 256 * 4;             // per epilogue warp: alpha_m * beta of the tile's tokens
 constexpr int LG_NBAR = 2 * LG_SW + 2 * LG_NS_MAX + 4;
-constexpr int LG_FIXED_SMEM = LG_SW * LG_W_BYTES + LG_SCALE_BYTES + 1024 /*align*/ + 8 * LG_NBAR + 16;
 
 __host__ __device__ inline uint32_t lg_stage_stride(int TN) { return LG_A_BYTES + (((uint32_t)TN * TILE_K + 1023u) & ~1023u); }
 

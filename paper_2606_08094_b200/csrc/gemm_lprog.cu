@@ -149,10 +149,11 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     const uint32_t ns = (uint32_t)P.NS;
     const uint32_t sS = base;
     const uint32_t sW = sS + ns * stride;
-    const uint32_t sBar = sW + LG_SW * W_STAGE + LG_SCALE_BYTES;
+    const uint32_t nsw = (uint32_t)P.NSW;                               // packed-weight stages in use (<= LG_SW)
+    const uint32_t sBar = sW + nsw * W_STAGE + LG_SCALE_BYTES;
     uint8_t* pS = base_ptr;
     uint8_t* pW = base_ptr + (size_t)ns * stride;
-    float* pScale = reinterpret_cast<float*>(pW + LG_SW * W_STAGE);
+    float* pScale = reinterpret_cast<float*>(pW + nsw * W_STAGE);
     auto bar_full_w = [&](uint32_t s) { return sBar + 8u * s; };
     auto bar_empty_w = [&](uint32_t s) { return sBar + 8u * (LG_SW + s); };
     auto bar_full = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + s); };
@@ -194,6 +195,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         if (lane < 4) {                                       // one copy per 32-channel piece: its KS k blocks are contiguous
             const int piece = lane;
             uint32_t it = 0;
+            RingCur cw;
             for (int sidx = 0; sidx < P.n_stages; ++sidx) {
                 const LpStage& st = stages[sidx];
                 const int num_kb = st.K / TILE_K, tiles_n = st.tiles_n, ntiles = st.ntiles, nlin = st.grp.n;
@@ -203,9 +205,9 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                     for (int j = 1; j < nlin; ++j) if (ct >= st.grp.ct_begin[j]) li = j;
                     const int nb = ct - st.grp.ct_begin[li];
                     const uint8_t* wsrc = st.grp.packed[li] + (size_t)(nb * 4 + piece) * num_kb * 1024;
-                    for (int kb = 0; kb < num_kb; kb += KS, ++it) {
-                        const uint32_t s = it % LG_SW;
-                        if (it >= LG_SW) mbar_wait(bar_empty_w(s), ((it / LG_SW) & 1) ^ 1);
+                    for (int kb = 0; kb < num_kb; kb += KS, ++it, cw.next(nsw)) {
+                        const uint32_t s = cw.s;
+                        if (cw.wrapped) mbar_wait(bar_empty_w(s), cw.ph ^ 1u);
                         if (lane == 0) mbar_arrive_expect_tx(bar_full_w(s), W_STAGE);
                         __syncwarp(0xFu);
                         tma_bulk_g2s(sW + s * W_STAGE + piece * (KS * 1024), wsrc + (size_t)kb * 1024, KS * 1024, bar_full_w(s));
@@ -284,15 +286,15 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
         const int g = 2 * q + p;
         uint32_t it = 0;
-            RingCur cd;
+            RingCur cd, cdw;
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpStage& st = stages[sidx];
             const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
             for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid) {
-                for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns)) {
+                for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns), cdw.next(nsw)) {
                     if ((int)(it & 1u) != dgrp) continue;
-                    const uint32_t sw = it % LG_SW, s = cd.s;
-                    mbar_wait(bar_full_w(sw), (it / LG_SW) & 1);
+                    const uint32_t sw = cdw.s, s = cd.s;
+                    mbar_wait(bar_full_w(sw), cdw.ph);
                     const uint8_t* wst = pW + sw * W_STAGE;
                     uint4 wv[KS][2];
 #pragma unroll
@@ -329,7 +331,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         // ---------------- epilogue warps ----------------
         const int lq = warp & 3;
         float* sc = pScale + lq * 256;
-        const uint32_t sc_addr = sW + LG_SW * W_STAGE + (uint32_t)lq * 1024u;
+        const uint32_t sc_addr = sW + nsw * W_STAGE + (uint32_t)lq * 1024u;
         pdl_wait();                                           // the outputs may still be read by the previous kernel
         uint32_t ti = 0;
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {

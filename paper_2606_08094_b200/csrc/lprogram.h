@@ -35,7 +35,7 @@ struct DevLProg {
     uint32_t x_tile;           // bytes reserved per X tile (the widest token tile of the program, 1 KiB aligned)
     int smem_bytes;
     uint32_t qbuf_bytes;       // row buffer of the quantiser (shared memory): holds min(16, qbuf_bytes / (2 K)) rows of x
-    int pad;
+    int NSW;                   // packed-weight stages in use (<= LG_SW)
     unsigned* qdone;           // [n_stages] CTAs that have quantised their rows of stage s      (target gridDim.x)
     unsigned* gdone;           // [n_stages] CTAs that have stored their tiles of stage s         (target gridDim.x)
     unsigned* done;            // [1]        CTAs past their last counter access; the last one re-zeroes the counters
