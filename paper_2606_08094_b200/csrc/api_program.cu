@@ -274,7 +274,18 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         d.rot = 0;
         if (vla::lg_encode_x_map(d.tmap, d.xq, a.M, a.K, d.TN) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
     }
-    const int stride = KS * (vla::LG_A_BYTES + (int)x_tile);
+    // The decoded A operand goes to TENSOR MEMORY when every token tile leaves columns for it beside the two accumulators
+    // (TN <= 192): a pipeline stage in shared memory then holds X only, and 2-3 times as many X tiles are in flight.
+    int max_tn = 0;
+    for (int s = 0; s < n_stages; ++s) max_tn = std::max(max_tn, S[s].TN);
+#ifdef VLA_LP_NO_ATM
+    const bool atm = false;
+#else
+    const bool atm = max_tn <= 192;
+#endif
+    const int acc_stride = !atm ? 256 : (max_tn <= 128 ? 128 : 192);
+    const int NA = !atm ? 1 : std::min(vla::LP_NA_MAX, (512 - 2 * acc_stride) / (32 * KS));
+    const int stride = KS * ((atm ? 0 : vla::LG_A_BYTES) + (int)x_tile);
     // Shared memory: NS {decoded A, X} pipeline stages, NSW packed-weight stages, and the row buffer of the fused quantiser --
     // room for the rows a CTA quantises per stage (at most 16 at a time), in any case for one row.  As many pipeline stages
     // as fit beside the row buffer and a 6-deep weight ring (at least 3, or 2 with two k blocks per stage); one more if a 5-
@@ -289,7 +300,7 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         want = std::max(want, rows * S[s].K * 2);
         one_row = std::max(one_row, S[s].K * 2);
     }
-    const int ns_floor = KS == 2 ? 2 : 3;
+    const int ns_floor = atm ? 4 : (KS == 2 ? 2 : 3);
     int NS = 0, NSW = vla::LG_SW;
     for (int nsw = vla::LG_SW; nsw >= 4; --nsw) {
         int ns = (smem_limit - fixed_bytes(0, nsw) - want) / stride;                  // with the whole row buffer
@@ -304,6 +315,10 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
     P->KS = KS;
     P->NS = NS;
     P->NSW = NSW;
+    P->ATM = atm ? 1 : 0;
+    P->acc_stride = acc_stride;
+    P->NA = NA;
+    P->pad2 = 0;
     P->x_tile = x_tile;
     P->qbuf_bytes = (uint32_t)qbuf;
     P->smem_bytes = fixed_bytes(NS, NSW) + qbuf;
@@ -314,7 +329,7 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
     int grid = all_tiles < sms ? (int)all_tiles : sms;
     {   // the CTAs wait for each other: all of them must be resident at once
         int per_sm = 0;
-        if (vla::lprogram_max_ctas_per_sm(KS, P->smem_bytes, &per_sm) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
+        if (vla::lprogram_max_ctas_per_sm(KS, P->ATM, P->smem_bytes, &per_sm) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
         if (per_sm < 1) return VLA_ERR_CUDA;
         if (grid > per_sm * sms) grid = per_sm * sms;
     }

@@ -30,6 +30,7 @@ constexpr int LP_QW = VLA_LP_QW;                         // warps per group
 constexpr int LP_QT = 32 * LP_QW;
 constexpr int LP_THREADS = LG_THREADS + LP_QG * LP_QT + 32;         // + the publisher warp
 constexpr int LP_QROWS = 16;                             // most rows per round
+constexpr int LP_NBAR = LG_NBAR + 2 * LP_NA_MAX;          // + the A ring of the ATM form (full / empty)
 static_assert(LP_QG == 1 && LP_EXTRA_SMEM >= LP_QROWS * 4 + LP_QROWS * 16 + 16 + 128, "lprogram.h");
 
 #ifdef VLA_LP_STAMPS
@@ -137,14 +138,19 @@ __device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, int tid, in
     }
 }
 
-template <int KS>
+template <int KS, bool ATM>
 __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_constant__ DevLProg P) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* base_ptr = smem_raw + (base - smem_u32(smem_raw));
     const uint32_t x_tile = P.x_tile;
-    const uint32_t stride = KS * (LG_A_BYTES + x_tile);               // [A x KS | X x KS]
-    constexpr uint32_t X_OFF = KS * LG_A_BYTES;
+    // ATM: the decoded A operand lives in TENSOR MEMORY (columns behind the two accumulators, NA stages of KS x 32 columns),
+    // and a shared-memory pipeline stage holds X only -- so many more X tiles are in flight for the same shared memory
+    const uint32_t stride = KS * ((ATM ? 0u : (uint32_t)LG_A_BYTES) + x_tile);   // [A x KS | X x KS], ATM: [X x KS]
+    constexpr uint32_t X_OFF = ATM ? 0u : KS * LG_A_BYTES;
+    const uint32_t acc_stride = ATM ? (uint32_t)P.acc_stride : 256u;  // TMEM columns between the two accumulators
+    const uint32_t a_col0 = 2u * acc_stride;                          // ATM: first column of the A ring
+    const uint32_t na = (uint32_t)P.NA;
     constexpr uint32_t W_STAGE = KS * LG_W_BYTES;
     const uint32_t ns = (uint32_t)P.NS;
     const uint32_t sS = base;
@@ -160,7 +166,9 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     auto bar_empty = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + LG_NS_MAX + s); };
     auto bar_acc_full = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + 2 * LG_NS_MAX + s); };
     auto bar_acc_empty = [&](uint32_t s) { return sBar + 8u * (2 * LG_SW + 2 * LG_NS_MAX + 2 + s); };
-    const uint32_t tmem_slot = sBar + 8u * LG_NBAR;
+    auto bar_afull = [&](uint32_t s) { return sBar + 8u * (LG_NBAR + s); };                   // ATM: A stage written to TMEM
+    auto bar_aempty = [&](uint32_t s) { return sBar + 8u * (LG_NBAR + LP_NA_MAX + s); };      // ATM: its MMAs are done
+    const uint32_t tmem_slot = sBar + 8u * LP_NBAR;
     uint8_t* p_tail = base_ptr + (tmem_slot - base);
     volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(p_tail);
     unsigned* s_rowmax = reinterpret_cast<unsigned*>(p_tail + 16);
@@ -176,9 +184,10 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < LG_SW; ++s) { mbar_init(bar_full_w(s), 1); mbar_init(bar_empty_w(s), 4); }
-        for (int s = 0; s < LG_NS_MAX; ++s) { mbar_init(bar_full(s), 5); mbar_init(bar_empty(s), 1); }
+        for (int s = 0; s < LG_NS_MAX; ++s) { mbar_init(bar_full(s), ATM ? 1 : 5); mbar_init(bar_empty(s), 1); }
+        for (int s = 0; s < LP_NA_MAX; ++s) { mbar_init(bar_afull(s), 4); mbar_init(bar_aempty(s), 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(bar_acc_full(s), 1); mbar_init(bar_acc_empty(s), 4); }
-        mbar_init(tmem_slot + 16u + LP_QROWS * 20u, 1);
+        mbar_init(sBar + 8u * LP_NBAR + 16u + LP_QROWS * 20u, 1);
         fence_barrier_init();
         asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 8u), "r"(0u) : "memory");
         asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 12u), "r"(0u) : "memory");
@@ -248,7 +257,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         if (lane == 0) {
             const uint64_t desc0 = umma_desc_k_sw128(sS);
             uint32_t it = 0, ti = 0;
-            RingCur cm;
+            RingCur cm, ca;
             for (int sidx = 0; sidx < P.n_stages; ++sidx) {
                 const LpStage& st = stages[sidx];
                 const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
@@ -257,21 +266,30 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                     const uint32_t ab = ti & 1;
                     if (ti >= 2) mbar_wait(bar_acc_empty(ab), ((ti >> 1) & 1) ^ 1);
                     tc_fence_after();
-                    const uint32_t d_tmem = tmem_base + ab * 256u;
-                    for (int kb = 0; kb < num_kb; kb += KS, ++it, cm.next(ns)) {
+                    const uint32_t d_tmem = tmem_base + ab * acc_stride;
+                    for (int kb = 0; kb < num_kb; kb += KS, ++it, cm.next(ns), ca.next(na)) {
                         const uint32_t s = cm.s;
                         mbar_wait(bar_full(s), cm.ph);
+                        if constexpr (ATM) mbar_wait(bar_afull(ca.s), ca.ph);
                         tc_fence_after();
                         if (kb == 0 && tile == lp_first_tile(st, grid)) LP_STAMP(3);
 #pragma unroll
                         for (int kk = 0; kk < KS; ++kk) {
                             // (descriptor = constant fields + (shared address >> 4): only the address part moves)
-                            const uint64_t a_desc = desc0 + ((s * stride + kk * LG_A_BYTES) >> 4);
                             const uint64_t b_desc = desc0 + ((s * stride + X_OFF + kk * x_tile) >> 4);
+                            if constexpr (ATM) {
+                                const uint32_t a_tmem = tmem_base + a_col0 + (ca.s * KS + kk) * 32u;
 #pragma unroll
-                            for (int k = 0; k < TILE_K / 32; ++k)
-                                mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | kk | k) != 0);
+                                for (int k = 0; k < TILE_K / 32; ++k)
+                                    mma_i8_ts(d_tmem, a_tmem + 8 * k, b_desc + 2 * k, idesc, (kb | kk | k) != 0);
+                            } else {
+                                const uint64_t a_desc = desc0 + ((s * stride + kk * LG_A_BYTES) >> 4);
+#pragma unroll
+                                for (int k = 0; k < TILE_K / 32; ++k)
+                                    mma_i8_ss(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | kk | k) != 0);
+                            }
                         }
+                        if constexpr (ATM) mma_commit(bar_aempty(ca.s));
                         mma_commit(bar_empty(s));
                     }
                     mma_commit(bar_acc_full(ab));
@@ -286,16 +304,48 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         const int t = d & 3, p = (d >> 2) & 1, q = (d >> 3) & 3, i32 = d >> 5;
         const int g = 2 * q + p;
         uint32_t it = 0;
-            RingCur cd, cdw;
+            RingCur cd, cdw, cda;
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpStage& st = stages[sidx];
             const int num_kb = st.K / TILE_K, ntiles = st.ntiles;
             for (int tile = lp_first_tile(st, grid); tile < ntiles; tile += grid) {
-                for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns), cdw.next(nsw)) {
+                for (int kb = 0; kb < num_kb; kb += KS, ++it, cd.next(ns), cdw.next(nsw), cda.next(na)) {
                     if ((int)(it & 1u) != dgrp) continue;
                     const uint32_t sw = cdw.s, s = cd.s;
                     mbar_wait(bar_full_w(sw), cdw.ph);
                     const uint8_t* wst = pW + sw * W_STAGE;
+                    if constexpr (ATM) {
+                        // Thread l of the warp owns channel 32 * piece + l = TMEM lane (piece = warp & 3: the lane quarter this
+                        // warp may access).  Its 128 k of a k block are the 8 words (h, t) of the piece, word (h, t) -> columns
+                        // 16 h + 4 t .. + 3 (packed layout: common.cuh).
+                        const int piece = warp & 3, jj = lane >> 3, gg = lane & 7;
+                        uint32_t wr[KS][8];
+#pragma unroll
+                        for (int kk = 0; kk < KS; ++kk)
+#pragma unroll
+                            for (int u = 0; u < 8; ++u)
+                                wr[kk][u] = *reinterpret_cast<const uint32_t*>(wst + piece * (KS * 1024) + kk * 1024 + ((((u >> 2) * 32 + gg * 4 + (u & 3)) * 4 + jj) * 4));
+                        if (cda.wrapped) mbar_wait(bar_aempty(cda.s), cda.ph ^ 1u);
+                        tc_fence_after();
+#pragma unroll
+                        for (int kk = 0; kk < KS; ++kk) {
+                            uint32_t r[32];
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) {
+                                r[4 * u + 0] = decode64<0>(wr[kk][u]); r[4 * u + 1] = decode64<1>(wr[kk][u]);
+                                r[4 * u + 2] = decode64<2>(wr[kk][u]); r[4 * u + 3] = decode64<3>(wr[kk][u]);
+                            }
+                            tmem_st_32x32b_x32(tmem_base + a_col0 + (cda.s * KS + kk) * 32u + ((uint32_t)(piece * 32) << 16), r);
+                        }
+                        tmem_st_wait();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) {
+                            mbar_arrive(bar_empty_w(sw));
+                            mbar_arrive(bar_afull(cda.s));
+                        }
+                        continue;
+                    }
                     uint4 wv[KS][2];
 #pragma unroll
                     for (int kk = 0; kk < KS; ++kk)
@@ -356,7 +406,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
                 __syncwarp();
                 mbar_wait(bar_acc_full(ab), (ti >> 1) & 1);
                 tc_fence_after();
-                const uint32_t t_addr = tmem_base + ab * 256u + ((uint32_t)(lq * 32) << 16);
+                const uint32_t t_addr = tmem_base + ab * acc_stride + ((uint32_t)(lq * 32) << 16);
                 for (int c0 = 0; c0 < TN; c0 += 16) {
                     if (m0 + c0 >= M) break;
                     uint32_t r[16];
@@ -483,22 +533,21 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     }
 }
 
-cudaError_t lprogram_max_ctas_per_sm(int KS, int smem_bytes, int* out) {
-    cudaError_t e;
-    if (KS == 2) {
-        e = cudaFuncSetAttribute(lprog_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-        if (e != cudaSuccess) return e;
-        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, lprog_kernel<2>, LP_THREADS, (size_t)smem_bytes);
-    }
-    e = cudaFuncSetAttribute(lprog_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-    if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, lprog_kernel<1>, LP_THREADS, (size_t)smem_bytes);
+template <int KS, bool ATM>
+static cudaError_t lp_prepare(int smem_bytes, int* occ_out) {
+    cudaError_t e = cudaFuncSetAttribute(lprog_kernel<KS, ATM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+    if (e != cudaSuccess || !occ_out) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_out, lprog_kernel<KS, ATM>, LP_THREADS, (size_t)smem_bytes);
+}
+static cudaError_t lp_prepare_any(int KS, int atm, int smem_bytes, int* occ_out) {
+    if (atm) return KS == 2 ? lp_prepare<2, true>(smem_bytes, occ_out) : lp_prepare<1, true>(smem_bytes, occ_out);
+    return KS == 2 ? lp_prepare<2, false>(smem_bytes, occ_out) : lp_prepare<1, false>(smem_bytes, occ_out);
 }
 
+cudaError_t lprogram_max_ctas_per_sm(int KS, int atm, int smem_bytes, int* out) { return lp_prepare_any(KS, atm, smem_bytes, out); }
+
 cudaError_t launch_lprogram(const DevLProg& prog, int grid, cudaStream_t s) {
-    cudaError_t e = prog.KS == 2
-        ? cudaFuncSetAttribute(lprog_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, prog.smem_bytes)
-        : cudaFuncSetAttribute(lprog_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, prog.smem_bytes);
+    cudaError_t e = lp_prepare_any(prog.KS, prog.ATM, prog.smem_bytes, nullptr);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
@@ -511,8 +560,12 @@ cudaError_t launch_lprogram(const DevLProg& prog, int grid, cudaStream_t s) {
     cfg.attrs = at;
     cfg.numAttrs = 1;
     count_launch();
-    if (prog.KS == 2) return cudaLaunchKernelEx(&cfg, lprog_kernel<2>, prog);
-    return cudaLaunchKernelEx(&cfg, lprog_kernel<1>, prog);
+    if (prog.ATM) {
+        if (prog.KS == 2) return cudaLaunchKernelEx(&cfg, lprog_kernel<2, true>, prog);
+        return cudaLaunchKernelEx(&cfg, lprog_kernel<1, true>, prog);
+    }
+    if (prog.KS == 2) return cudaLaunchKernelEx(&cfg, lprog_kernel<2, false>, prog);
+    return cudaLaunchKernelEx(&cfg, lprog_kernel<1, false>, prog);
 }
 
 }  // namespace vla

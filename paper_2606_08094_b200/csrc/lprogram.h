@@ -10,7 +10,8 @@
 namespace vla {
 
 constexpr uint32_t LPROG_MAGIC = 0x564C414Cu;   // "VLAL"
-constexpr int LP_EXTRA_SMEM = 512;   // behind gemm_large's layout: quantiser row absmax [16], scales float4 [16], its mbarrier, and the
+constexpr int LP_NA_MAX = 8;          // most A stages of the ATM form (decoded weights in tensor memory)
+constexpr int LP_EXTRA_SMEM = 512 + 16 * LP_NA_MAX;   // behind gemm_large's layout: quantiser row absmax [16], scales float4 [16], its mbarrier, and the
                                      // alignment slack of its row buffer (DevLProg::qbuf_bytes more bytes follow)
 
 struct alignas(64) LpStage {
@@ -36,6 +37,10 @@ struct DevLProg {
     int smem_bytes;
     uint32_t qbuf_bytes;       // row buffer of the quantiser (shared memory): holds min(16, qbuf_bytes / (2 K)) rows of x
     int NSW;                   // packed-weight stages in use (<= LG_SW)
+    int ATM;                   // 1: decoded A operand in tensor memory (every token tile <= 192), pipeline stages hold X only
+    int acc_stride;            // ATM: TMEM columns per accumulator (128 or 192); the A ring starts at column 2 * acc_stride
+    int NA;                    // ATM: A stages of KS x 32 columns
+    int pad2;
     unsigned* qdone;           // [n_stages] CTAs that have quantised their rows of stage s      (target gridDim.x)
     unsigned* gdone;           // [n_stages] CTAs that have stored their tiles of stage s         (target gridDim.x)
     unsigned* done;            // [1]        CTAs past their last counter access; the last one re-zeroes the counters
@@ -44,6 +49,6 @@ struct DevLProg {
 };
 
 cudaError_t launch_lprogram(const DevLProg& prog, int grid, cudaStream_t s);
-cudaError_t lprogram_max_ctas_per_sm(int KS, int smem_bytes, int* out);
+cudaError_t lprogram_max_ctas_per_sm(int KS, int atm, int smem_bytes, int* out);
 
 }  // namespace vla
