@@ -79,6 +79,27 @@ def test_independent_stages_alternate_scratch_and_rerun(vla, oracle):
     vla.vla_program_release(prog)
 
 
+@pytest.mark.parametrize("M,K", [(544, 512), (544, 384), (1100, 512), (100, 256)])
+def test_long_program_work_tiles_and_round_robin(vla, oracle, M, K):
+    """A program long enough for the work-minimising token tiles and the tile round robin across stages (20 independent
+    or 40 stages, N alternating 3840 / 2560 / 1280): M=544 -> TN = 192, A operand in tensor memory with 192-column accumulators, two
+    k blocks per stage (K=512) or one (K=384: odd number of k blocks); M=1100 -> TN = 256, A operand in shared memory;
+    M=100 -> TN = 112, 128-column accumulators.  Most stages have fewer tiles than SMs, so each starts on the CTAs the
+    previous one left idle.  Every output vs the oracle, twice."""
+    Ns = [3840, 2560, 1280]                                  # 30 / 20 / 10 channel tiles: > 4 x 148 tiles in all = "long"
+    n_st = 20 if M >= 544 else 40
+    pts = [make_point(vla, M, K, Ns[i % 3], 9900 + i, [0, 1, 2][i % 3], want_xq=(i % 5 == 0)) for i in range(n_st)]
+    prog = vla.compile_program([stage_of(p) for p in pts])
+    for rep in range(2):
+        for p in pts:
+            p["out"].fill_(-3)
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        for p in pts:
+            check_point(vla, oracle, p)
+    vla.vla_program_release(prog)
+
+
 def test_chained_stack_m544_one_launch(vla, oracle):
     """configs[3] at M=544 as ONE launch: 3 full-size layers = 12 dependent stages (q|k|v as one N=3840 group, gate|up as
     N=13824), quantisation fused, free-running; every intermediate of every layer bit-identical to the oracle's chain.
