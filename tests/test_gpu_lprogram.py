@@ -100,6 +100,44 @@ def test_long_program_work_tiles_and_round_robin(vla, oracle, M, K):
     vla.vla_program_release(prog)
 
 
+def test_random_large_programs_equal_single_calls(vla):
+    """Seeded random large programs (1..12 stages, M from 17 to 2048, K and N from the small shapes, ~30 % of the stages
+    reading the previous stage's bf16 output) run three times: outputs are deterministic and bit-identical to one
+    vla_ternary_linear call per stage on the same inputs (which test_gpu_parity.py checks against the oracle)."""
+    rng = np.random.default_rng(20260608)
+    for trial in range(14):
+        M = int(rng.choice([17, 33, 64, 100, 200, 544, 545, 1000, 1100, 2048]))
+        stages = []
+        for i in range(int(rng.integers(1, 13))):
+            K = int(rng.choice([128, 256, 384, 512, 640, 1280]))
+            N = int(rng.choice([128, 256, 384, 640, 1280]))
+            packed = vla.pack_weights(dev(synth.ternary_weights(N, K, 0.35, int(rng.integers(1 << 30)))))
+            beta = dev(np.array([synth.weight_scale(int(rng.integers(1 << 30)))], np.float32))
+            chained = i > 0 and rng.random() < 0.3 and stages[-1]["linears"][0]["N"] == K
+            x = stages[-1]["linears"][0]["out"] if chained else dev_bf16(synth.activations(M, K, int(rng.integers(1 << 30))))
+            out = torch.zeros((M, N), dtype=torch.bfloat16, device="cuda")
+            stages.append(dict(x=x, M=M, K=K, depends=1 if chained else 0,
+                               linears=[dict(packed=packed, w_scale=beta, out=out, N=N, out_dtype=vla.VLA_BF16)]))
+        prog = vla.compile_program(stages)
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        first = [st["linears"][0]["out"].clone() for st in stages]
+        for rep in range(2):
+            vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        for st, ref in zip(stages, first):
+            lin = st["linears"][0]
+            assert torch.equal(lin["out"], ref), "trial %d: output changed between runs" % trial
+            nb = vla.vla_ternary_workspace_bytes(M, lin["N"], st["K"])
+            ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+            single = torch.empty_like(ref)
+            vla.vla_ternary_linear(lin["packed"], lin["w_scale"], st["x"], M, lin["N"], st["K"], single, vla.VLA_BF16,
+                                   vla.VLA_PATH_AUTO, None, None, ws, nb)
+            torch.cuda.synchronize()
+            assert torch.equal(single, ref), "trial %d: M=%d K=%d N=%d differs from the single call" % (trial, M, st["K"], lin["N"])
+        vla.vla_program_release(prog)
+
+
 def test_chained_stack_m544_one_launch(vla, oracle):
     """configs[3] at M=544 as ONE launch: 3 full-size layers = 12 dependent stages (q|k|v as one N=3840 group, gate|up as
     N=13824), quantisation fused, free-running; every intermediate of every layer bit-identical to the oracle's chain.
