@@ -161,7 +161,10 @@ vla_status vla_ternary_linear_static(const void* packed, const float* w_scale, c
  * x_scale_opt), the CTAs meet on a grid-wide counter, and the stage's 128-channel x token tiles are walked as in
  * VLA_PATH_LARGE; the launch does not end between stages.  Stages run in list order; depends = 1 makes a stage's
  * quantisation wait until EVERY earlier stage has stored its outputs, depends = 0 lets it run ahead (its x must not be
- * written by this program).  Results are bit-identical to vla_ternary_linear.
+ * written by this program).  Large programs also accept depends = d in 2..s: stage s then waits only for the stages up to
+ * s - d (its x is written by those), so that d independent chains -- e.g. a layer stack run on d row blocks of the
+ * batch, the stages of the blocks interleaved -- overlap each other's hand-offs instead of running in lockstep.
+ * Results are bit-identical to vla_ternary_linear.
  * All pointers inside the descriptors are DEVICE pointers, 16-byte aligned, and must stay valid for as
  * long as the program is run.  The descriptor arrays themselves are HOST memory.
  */
@@ -176,7 +179,7 @@ typedef struct {
 typedef struct {
     const void* x_bf16;     /* [M,K] bf16 */
     int M, K;
-    int depends;            /* 0 or 1, see above */
+    int depends;            /* 0 or 1 (large programs: 0..stage index), see above */
     int n_linears;
     const vla_prog_linear* linears;   /* HOST array of n_linears entries */
     int8_t* xq_opt;         /* optional: also return the quantised activations [M,K] int8 (NULL: kept inside the program) */

@@ -73,7 +73,7 @@ vla_status check_large(const vla_prog_stage* st, int n) {
         if (!a.x_bf16 || !a.linears) return VLA_ERR_NULL;
         if (a.M <= 16 || a.M > 32768 || a.K < 128 || a.K % 128 != 0 || a.K > 8192) return VLA_ERR_SHAPE;
         if (a.n_linears < 1 || a.n_linears > 8) return VLA_ERR_SHAPE;
-        if (a.depends != 0 && a.depends != 1) return VLA_ERR_SHAPE;
+        if (a.depends < 0 || a.depends > s) return VLA_ERR_SHAPE;         // d >= 1: waits for the stages up to s - d (large programs)
         if (!aligned16(a.x_bf16) || (a.xq_opt && !aligned16(a.xq_opt)) || (a.x_scale_opt && !aligned16(a.x_scale_opt)))
             return VLA_ERR_ALIGN;
         for (int j = 0; j < a.n_linears; ++j) {
@@ -271,7 +271,7 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         const int b = s % LP_NSCRATCH;                        // scratch set of the stage
         d.xq = a.xq_opt ? a.xq_opt : reinterpret_cast<int8_t*>(base + L.off_xq[b]);
         d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + L.off_xs[b]);
-        d.wait_stage = std::max((s > 0 && a.depends) ? s - 1 : -1, prev_user[b]);
+        d.wait_stage = std::max(a.depends > 0 ? s - a.depends : -1, prev_user[b]);
         prev_user[b] = s;
         d.rot = 0;
         if (vla::lg_encode_x_map(d.tmap, d.xq, a.M, a.K, d.TN) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }

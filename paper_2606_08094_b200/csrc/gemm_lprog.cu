@@ -492,30 +492,36 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     } else {
         // ---------------- publisher: the quantiser's grid-scope hand-offs, off its chain ----------------
         // (1) counts the CTA in qdone[s] once all quantiser warps have stored stage s;  (2) clears stage s+1 for the
-        // quantiser (s_gok = stages cleared) once gdone[wait_stage(s+1)] == grid -- polled WHILE the quantiser works on stage
-        // s, except where stage s+1 waits for stage s itself (depends = 1): then qdone[s] has to be published first.
+        // quantiser (s_gok = stages cleared) once gdone[wait_stage(s+1)] == grid, polled WHILE the quantiser works on stage s.
+        // Neither blocks the other: a stage that waits for an older stage's GEMM (interleaved chains, depends = d) must not
+        // hold back the publication of the stage in between.
         if (lane == 0) {
             pdl_wait();                                       // the counters are re-zeroed by the previous run's last CTA
-            auto clear_stage = [&](int t) {                   // stage t may start quantising
-                const int w = stages[t].wait_stage;
-                if (w >= 0) spin_until(P.gdone + w, grid);
-                asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" :: "r"(s_gok), "r"((unsigned)t + 1u) : "memory");
-            };
-            clear_stage(0);
-            for (int sidx = 0; sidx < P.n_stages; ++sidx) {
-                const bool has_next = sidx + 1 < P.n_stages;
-                const bool next_needs_me = has_next && stages[sidx + 1].wait_stage >= sidx;
-                if (has_next && !next_needs_me) clear_stage(sidx + 1);
-                const unsigned want = (unsigned)LP_QW * (unsigned)(sidx + 1);
-                const long long t0 = clock64();
+            const int n = P.n_stages;
+            int qs = 0, gs = 1;                               // next stage to publish / to clear (stage 0 waits for nothing)
+            asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" :: "r"(s_gok), "r"(1u) : "memory");
+            int w_gs = gs < n ? stages[gs].wait_stage : -1;
+            long long t0 = clock64();
+            while (qs < n) {
                 unsigned have;
-                do {
-                    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(have) : "r"(s_qcount) : "memory");
-                    if (clock64() - t0 > (1ll << 32)) __trap();
-                } while (have < want);
-                LP_STAMP(1);
-                red_release_gpu(P.qdone + sidx, 1u);          // cumulative: covers the quantiser warps' stores observed above
-                if (next_needs_me) clear_stage(sidx + 1);
+                asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(have) : "r"(s_qcount) : "memory");
+                if (have >= (unsigned)LP_QW * (unsigned)(qs + 1)) {
+                    const int sidx = qs;
+                    LP_STAMP(1);
+                    red_release_gpu(P.qdone + sidx, 1u);      // cumulative: covers the quantiser warps' stores observed above
+                    ++qs;
+                    t0 = clock64();
+                    continue;
+                }
+                if (gs < n && gs <= qs + 1) {                 // one try (an L2 round trip), then back to the cheap check
+                    if (w_gs < 0 || ld_acquire_gpu(P.gdone + w_gs) >= grid) {
+                        ++gs;
+                        asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" :: "r"(s_gok), "r"((unsigned)gs) : "memory");
+                        w_gs = gs < n ? stages[gs].wait_stage : -1;
+                        t0 = clock64();
+                    }
+                }
+                if (clock64() - t0 > (1ll << 32)) __trap();
             }
         }
     }

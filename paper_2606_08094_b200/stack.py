@@ -59,8 +59,28 @@ class Stack:
                                   N=_DIMS[n][1], out_dtype=vla.VLA_BF16) for n in names]))
         return st
 
-    def compile(self):
-        self.program = vla.compile_program(self.stages(), self.device)
+    def stages_row_blocks(self, blocks):
+        """The same chain as `blocks` independent chains over row blocks of the batch (a linear layer acts on every token
+        row by itself), their stages interleaved: stage (layer, kind, block b) reads and writes rows [r_b, r_b+1) of the
+        same tensors and waits only for the stages up to the previous kind OF ITS OWN BLOCK (depends = blocks), so that the
+        grid-wide hand-offs of one block overlap the GEMMs of the others (large programs only: M / blocks > 16)."""
+        M = self.M
+        bounds = [(M * b // blocks) // 16 * 16 if b < blocks else M for b in range(blocks + 1)]
+        st, first = [], True
+        for layer in range(self.layers):
+            for (src, names) in STAGES:
+                for b in range(blocks):
+                    r0, r1 = bounds[b], bounds[b + 1]
+                    st.append(dict(
+                        x=self._input_of(layer, src)[r0:r1], M=r1 - r0, K=_DIMS[names[0]][0],
+                        depends=0 if first else blocks,
+                        linears=[dict(packed=self.packed[layer][n], w_scale=self.beta[layer][n], out=self.out[layer][n][r0:r1],
+                                      N=_DIMS[n][1], out_dtype=vla.VLA_BF16) for n in names]))
+                first = False
+        return st
+
+    def compile(self, blocks=1):
+        self.program = vla.compile_program(self.stages() if blocks == 1 else self.stages_row_blocks(blocks), self.device)
         return self.program
 
     def run_program(self):

@@ -159,6 +159,28 @@ def test_chained_stack_m544_one_launch(vla, oracle):
                 st.out[l][n].zero_()
 
 
+@pytest.mark.parametrize("blocks", [2, 3])
+def test_chained_stack_as_interleaved_row_blocks(vla, oracle, blocks):
+    """depends = d: the M=544 chain as `blocks` independent chains over row blocks of the batch, their stages interleaved in
+    one launch (stage s waits only for the stages up to s - blocks).  2 full-size layers, every intermediate bit-identical to
+    the oracle's chain, twice."""
+    from paper_2606_08094_b200.stack import Stack
+    layers, M = 2, synth.PREFILL_M
+    weights = [synth.stack_layer(l) for l in range(layers)]
+    x = synth.stack_input(M)
+    st = Stack(layers, M, weights=weights)
+    st.set_input(x)
+    st.compile(blocks)
+    ref = oracle_stack(oracle, weights, x)
+    for rep in range(2):
+        st.run_program()
+        torch.cuda.synchronize()
+        for l in range(layers):
+            for n in ref[l]:
+                assert np.array_equal(bits(st.out[l][n]), ref[l][n]), "layer %d %s differs (rep %d)" % (l, n, rep)
+                st.out[l][n].zero_()
+
+
 def test_chained_large_program_changing_inputs(vla, oracle):
     """a dependent pair (stage 1 reads stage 0's bf16 output) re-run with NEW inputs in the same buffers: a stale row in an
     SM's L1 or a stale alpha would show"""
@@ -212,3 +234,5 @@ def test_large_program_errors(vla):
     nine["linears"] = nine["linears"] * 9
     assert vla.vla_program_bytes([nine]) == 0                                      # at most 8 linears per large stage
     assert vla.vla_program_bytes([stage_of(large)]) > 0
+    assert vla.vla_program_bytes([stage_of(large), dict(stage_of(large), depends=2)]) == 0      # depends <= stage index
+    assert vla.vla_program_bytes([stage_of(large), stage_of(large), dict(stage_of(large), depends=2)]) > 0
