@@ -402,7 +402,8 @@ def run_vs_m(pk, int8_probe_tops, Ms=None, shapes=None):
         outs = [torch.empty((M, N), dtype=torch.float32, device=dev) for (K, N) in synth.MODEL_SHAPES]
         stages = [dict(x=xs_[si], M=M, K=K, depends=0,
                        linears=[dict(packed=rings[si][c], w_scale=beta, out=outs[si], N=N, out_dtype=vla.VLA_F32)])
-                  for c in range(nstep) for si, (K, N) in enumerate(synth.MODEL_SHAPES)]
+                  for c in range(nstep)
+                  for si, (K, N) in sorted(enumerate(synth.MODEL_SHAPES), key=lambda t: -t[1][0] * t[1][1])]   # largest first
         flush = torch.empty(2 * l2, dtype=torch.uint8, device=dev)
         prog = vla.compile_program(stages, dev)
         vla.vla_program_run(prog)

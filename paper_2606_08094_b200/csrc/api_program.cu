@@ -219,19 +219,19 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
 #else
     P->stamps = nullptr;
 #endif
+    // Work-minimising token tiles pay as soon as the program has enough tiles to keep every SM busy while stages overlap
+    // (measured: the one-step configs[2] program, 297 such tiles, 42.2 -> 38.6 us; a lone (2560,2560) stage, 60 tiles, loses)
     bool long_program = false;
-    {   // estimated makespan with work-optimal tiles (total CTA time / SMs) against the longest single tile
-        double work = 0.0, longest = 0.0;
+    {
+        long long tiles = 0;
         for (int s = 0; s < n_stages; ++s) {
             const vla_prog_stage& a = stages[s];
             int n_total = 0;
             for (int j = 0; j < a.n_linears; ++j) n_total += a.linears[j].N;
             const int tn = pick_tn_work(a.M, a.K);
-            const double tile = (a.K / 128) * (((tn <= 160 && (a.K / 128) % 2 == 0) ? 0.155 : 0.167) + 1.25e-3 * tn);
-            work += tile * (n_total / 128) * ((a.M + tn - 1) / tn);
-            longest = std::max(longest, tile);
+            tiles += (long long)(n_total / 128) * ((a.M + tn - 1) / tn);
         }
-        long_program = work / sms >= 4.0 * longest;
+        long_program = 2 * tiles >= 3 * (long long)sms;
     }
     int KS = 2, prev_user[LP_NSCRATCH];
     bool k_even_all = true;
@@ -338,11 +338,32 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         if (per_sm < 1) return VLA_ERR_CUDA;
         if (grid > per_sm * sms) grid = per_sm * sms;
     }
-    {   // round robin of the tiles over the CTAs, continued across stages
-        long long next = 0;
+    {   // Tiles of a stage go to consecutive CTAs starting at `rot` (round robin).  rot is chosen per stage so that the
+        // CTAs that get one tile more than the others are the least loaded ones so far (estimated CTA time: k blocks x
+        // cost of a k block at the stage's TN); a stage that waits for its predecessor levels the loads.
+        std::vector<double> load(grid, 0.0);
+        int cont = 0;                                          // where the previous stage's tiles ended
         for (int s = 0; s < n_stages; ++s) {
-            S[s].rot = (int)(next % grid);
-            next += S[s].ntiles;
+            if (S[s].wait_stage == s - 1 && s > 0) {
+                const double top = *std::max_element(load.begin(), load.end());
+                std::fill(load.begin(), load.end(), top);
+            }
+            const double cost = (S[s].K / 128) * ((KS == 2 ? 0.155 : 0.167) + 1.25e-3 * S[s].TN);
+            const int base = S[s].ntiles / grid, rem = S[s].ntiles % grid;
+            int best = cont;
+            if (rem > 0) {
+                double best_max = 1e300, best_sum = 1e300;
+                for (int k = 0; k < grid; ++k) {               // candidates in round-robin order: ties keep the continuation
+                    const int r = (cont + k) % grid;
+                    double mx = 0.0, sum = 0.0;
+                    for (int c = 0; c < rem; ++c) { const double v = load[(r + c) % grid]; mx = std::max(mx, v); sum += v; }
+                    if (mx < best_max - 1e-9 || (mx < best_max + 1e-9 && sum < best_sum - 1e-9)) { best_max = mx; best_sum = sum; best = r; }
+                }
+            }
+            S[s].rot = best;
+            for (int c = 0; c < grid; ++c) load[c] += base * cost;
+            for (int c = 0; c < rem; ++c) load[(best + c) % grid] += cost;
+            cont = (best + rem) % grid;
         }
     }
     cudaStream_t cs = (cudaStream_t)stream;
