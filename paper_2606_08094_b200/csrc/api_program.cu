@@ -267,7 +267,7 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         x_tile = std::max(x_tile, ((uint32_t)d.TN * 128u + 1023u) & ~1023u);
         d.tiles_n = n_total / 128;
         d.ntiles = d.tiles_n * ((a.M + d.TN - 1) / d.TN);
-        d.inv_nvec = (uint32_t)((0x100000000ull + (unsigned)(a.K / 8) - 1u) / (unsigned)(a.K / 8));
+        d.x_dep = a.depends > 0 ? 1 : 0;
         const int b = s % LP_NSCRATCH;                        // scratch set of the stage
         d.xq = a.xq_opt ? a.xq_opt : reinterpret_cast<int8_t*>(base + L.off_xq[b]);
         d.xs = a.x_scale_opt ? a.x_scale_opt : reinterpret_cast<float*>(base + L.off_xs[b]);
@@ -293,8 +293,8 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
     const int stride = KS * ((atm ? 0 : vla::LG_A_BYTES) + (int)x_tile);
     // Shared memory: NS {decoded A, X} pipeline stages, NSW packed-weight stages, and the row buffer of the fused quantiser --
     // room for the rows a CTA quantises per stage (at most 16 at a time), in any case for one row.  As many pipeline stages
-    // as fit beside the row buffer and a 6-deep weight ring (at least 3, or 2 with two k blocks per stage); one more if a 5-
-    // or 4-deep weight ring makes room for it.
+    // as fit beside the row buffer and a 6-deep weight ring (at least 3, or 2 with two k blocks per stage); one more if a
+    // 4-deep weight ring makes room for it.
     const int smem_limit = vla::LG_SMEM_LIMIT - 64;
     auto fixed_bytes = [&](int ns, int nsw) {
         return ns * stride + nsw * KS * vla::LG_W_BYTES + vla::LG_SCALE_BYTES + 1024 + 8 * vla::LG_NBAR + 16 + vla::LP_EXTRA_SMEM;
@@ -302,16 +302,38 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
     int want = 0, one_row = 0;
     for (int s = 0; s < n_stages; ++s) {
         const int rows = std::min(16, (S[s].M + std::min(sms, S[s].M) - 1) / std::min(sms, S[s].M));
-        want = std::max(want, rows * S[s].K * 2);
+        want = std::max(want, 2 * rows * S[s].K * 2);           // two halves: the next chunk's rows load during this chunk's passes
         one_row = std::max(one_row, S[s].K * 2);
     }
     const int ns_floor = atm ? 4 : (KS == 2 ? 2 : 3);
+    // the quantiser's chunks: rows per chunk of a stage for a row buffer of `qb` bytes -- double-buffered (a chunk per half, the
+    // next chunk's rows load during this chunk's passes) unless that takes more chunks than the whole buffer would: a chunk
+    // costs ~1 us of barriers and copy issue whatever its size
+    auto chunking = [&](int qb, int K, int rows, int* rpc, int* dbl) {
+        const int row_bytes = K * 2, half = (qb / 2) & ~127;
+        const int rpc1 = std::max(1, std::min(16, qb / row_bytes)), rpc2 = std::min(16, half / row_bytes);
+        const int c1 = (rows + rpc1 - 1) / rpc1, c2 = rpc2 > 0 ? (rows + rpc2 - 1) / rpc2 : (1 << 30);
+        *dbl = c2 <= c1 ? 1 : 0;
+        *rpc = *dbl ? rpc2 : rpc1;
+        return *dbl ? c2 : c1;
+    };
     int NS = 0, NSW = vla::LG_SW;
-    for (int nsw = vla::LG_SW; nsw >= 4; --nsw) {
+    long long best_chunks = 0;
+    // (an EVEN weight ring only: the two decode groups alternate over its stages, and with an odd depth a group would come back
+    // to a stage last filled for the OTHER group -- whose copy may not even have landed, so that the parity wait falls through)
+    for (int nsw = vla::LG_SW; nsw >= 4; nsw -= 2) {
         int ns = (smem_limit - fixed_bytes(0, nsw) - want) / stride;                  // with the whole row buffer
         if (ns < ns_floor) ns = std::min(ns_floor, (smem_limit - fixed_bytes(0, nsw) - one_row) / stride);   // with a smaller one
         if (ns > vla::LG_NS_MAX) ns = vla::LG_NS_MAX;
-        if (ns > NS) { NS = ns; NSW = nsw; }
+        if (ns < NS || ns < 2) continue;
+        const int qb = std::min(want, smem_limit - fixed_bytes(ns, nsw)) & ~127;
+        long long chunks = 0;                                    // per CTA, over the program
+        for (int s = 0; s < n_stages; ++s) {
+            int rpc, dbl;
+            chunks += chunking(qb, S[s].K, (S[s].M + std::min(sms, S[s].M) - 1) / std::min(sms, S[s].M), &rpc, &dbl);
+        }
+        // the deepest pipeline first; then a 4-deep weight ring if the row buffer it frees saves chunks
+        if (ns > NS || chunks < best_chunks) { NS = ns; NSW = nsw; best_chunks = chunks; }
     }
     if (NS < 2) return VLA_ERR_SHAPE;
     int qbuf = std::min(want, smem_limit - fixed_bytes(NS, NSW));
@@ -337,6 +359,11 @@ vla_status build_large(const vla_prog_stage* stages, int n_stages, void* prog_de
         if (vla::lprogram_max_ctas_per_sm(KS, P->ATM, P->smem_bytes, &per_sm) != cudaSuccess) { cudaGetLastError(); return VLA_ERR_CUDA; }
         if (per_sm < 1) return VLA_ERR_CUDA;
         if (grid > per_sm * sms) grid = per_sm * sms;
+    }
+    for (int s = 0; s < n_stages; ++s) {                       // the quantiser's geometry (lprogram.h)
+        S[s].q_rows = S[s].M / grid;
+        S[s].q_rem = S[s].M % grid;
+        chunking(qbuf, S[s].K, (S[s].M + grid - 1) / grid, &S[s].q_rpc, &S[s].q_dbl);
     }
     {   // Tiles of a stage go to consecutive CTAs starting at `rot` (round robin).  rot is chosen per stage so that the
         // CTAs that get one tile more than the others are the least loaded ones so far (estimated CTA time: k blocks x

@@ -341,9 +341,11 @@ cudaError_t launch_gemm_large_grouped(const LgGroup& g, const int8_t* xq, const 
     const int KS = lg_pick_ks(TN, K);
     const int stage = KS * (int)lg_stage_stride(TN);
     // pipeline stages NS and packed-weight stages NSW from the shared memory there is: as many {A, X} stages as fit beside a
-    // 6-deep weight ring, one more if a 5- or 4-deep ring makes room for it (TN = 112 with two k blocks per stage: 3, not 2)
+    // 6-deep weight ring, one more if a 4-deep ring makes room for it (TN = 112 with two k blocks per stage: 3, not 2).  The
+    // ring depth stays EVEN: the two decode groups alternate over its stages, and with an odd depth a group would come back to a
+    // stage last filled for the OTHER group, whose copy may not have landed yet -- its parity wait would fall through.
     int NS = 0, NSW = LG_SW;
-    for (int nsw = LG_SW; nsw >= 4; --nsw) {
+    for (int nsw = LG_SW; nsw >= 4; nsw -= 2) {
         int ns = (LG_SMEM_LIMIT - (LG_SCALE_BYTES + 1024 + 8 * LG_NBAR + 16) - nsw * KS * LG_W_BYTES) / stage;
         if (ns > LG_NS_MAX) ns = LG_NS_MAX;
         if (ns > NS) { NS = ns; NSW = nsw; }

@@ -55,56 +55,102 @@ __device__ __forceinline__ void lp_bar(int id, int threads) {
 }
 
 // rows blockIdx.x, += gridDim.x of the stage's x -> int8 + alpha.  The rows are STAGED IN SHARED MEMORY: one bulk copy (TMA)
-// per row, all rows of a chunk in flight at once (as many rows as fit the program's row buffer, at most LP_QROWS), then the
-// absmax pass and the quantising pass both read shared memory.  x is read from L2 / DRAM exactly once, no registers are
-// held across the passes, and the memory parallelism no longer depends on how many 16-byte loads a thread can keep in
-// flight (the register-held form took 10-11 us per stage at K = 6912, 3 us at K = 2560: DESIGN.md 6c).
+// per row, all rows of a chunk in flight at once, then the absmax pass and the quantising pass both read shared memory.  x is
+// read from L2 / DRAM exactly once, no registers are held across the passes, and the memory parallelism does not depend on
+// how many 16-byte loads a thread can keep in flight (the register-held form took 10-11 us per stage at K = 6912).
+// The row buffer is DOUBLE-BUFFERED whenever a row fits half of it: while the threads work on chunk c (half c & 1), thread 0
+// already has the copies of chunk c + 1 in flight into the other half -- the next rows of the same stage, or the FIRST rows of
+// the next stage if that stage's inputs are already cleared (s_gok).  In steady state the quantiser is the pacing chain of a
+// large program (its stages follow each other without a gap), and the 1-1.5 us a stage used to wait for its rows were a
+// fifth of that chain.
 struct LpQuantArgs {           // the quantiser's view of a stage, read from the table BEFORE it waits for the stage's inputs
     const uint4* x;
     uint2* xq;
     float* xs;
-    int M, nvec, wait_stage;
-    unsigned inv_nvec;
+    int nvec, wait_stage, R, rpc;       // R = rows of this CTA, rpc = rows per chunk
+    bool dbl, x_dep;
 };
 __device__ __forceinline__ LpQuantArgs lp_quant_args(const LpStage& st) {
     LpQuantArgs a;
     a.x = st.x; a.xq = reinterpret_cast<uint2*>(st.xq); a.xs = st.xs;
-    a.M = st.M; a.nvec = st.K >> 3; a.wait_stage = st.wait_stage; a.inv_nvec = st.inv_nvec;
+    a.nvec = st.K >> 3; a.wait_stage = st.wait_stage;
+    a.R = st.q_rows + ((int)blockIdx.x < st.q_rem ? 1 : 0); a.rpc = st.q_rpc; a.dbl = st.q_dbl != 0; a.x_dep = st.x_dep != 0;
     return a;
 }
+// lane 0 of quantiser warp w: the bulk copies of rows i0 + w, i0 + w + 8, ... (< i0 + g, of this CTA's rows) of a stage -> the
+// row buffer at `dst`; warp 0 also announces the bytes.  (One thread issuing all copies of a chunk kept the other 255 waiting
+// for ~70 cycles per copy.)
+__device__ __forceinline__ void lp_quant_issue(const LpQuantArgs& a, int i0, int g, uint32_t dst, uint32_t bar, int warp) {
+    const int grid = (int)gridDim.x, cta = (int)blockIdx.x;
+    const uint32_t row_bytes = (uint32_t)a.nvec * 16u;
+    if (a.x_dep) asm volatile("fence.proxy.async.global;" ::: "memory");      // x written by other SMs -> this thread's bulk copies
+    if (warp == 0) mbar_arrive_expect_tx(bar, (uint32_t)g * row_bytes);
+    for (int j = warp; j < g; j += LP_QW)
+        tma_bulk_g2s(dst + (uint32_t)j * row_bytes, a.x + (size_t)(cta + (i0 + j) * grid) * a.nvec, row_bytes, bar);
+}
 
-__device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, int tid, int bar_id, unsigned* s_rowmax, float4* s_scale,
-                                               uint32_t qbuf, uint32_t qbuf_bytes, uint32_t bar_q, uint32_t& q_parity,
-                                               unsigned long long* dbg) {
-    const int grid = (int)gridDim.x, cta = (int)blockIdx.x, nvec = a.nvec, M = a.M;
-    const uint32_t row_bytes = (uint32_t)nvec * 16u;
-    const uint4* __restrict__ x = a.x;
+// c = chunks this CTA has processed so far (all stages); inflight = the copies of chunk c are already issued (a prefetch)
+__device__ __forceinline__ void lp_quant_stage(const LpQuantArgs& a, const LpQuantArgs* nx, int sidx, uint32_t s_gok, uint32_t s_pf,
+                                               int tid, int bar_id, unsigned* s_rowmax, float4* s_scale, uint32_t qbuf,
+                                               uint32_t qbuf_bytes, uint32_t bar_q, uint32_t& c, bool& inflight, unsigned long long* dbg) {
+    const int grid = (int)gridDim.x, cta = (int)blockIdx.x, nvec = a.nvec, warp = tid >> 5, lane = tid & 31;
+    const uint32_t row_bytes = (uint32_t)nvec * 16u, half = (qbuf_bytes >> 1) & ~127u;
     uint2* __restrict__ xq = a.xq;
     float* __restrict__ xs = a.xs;
-    const int R = M > cta ? (M - cta + grid - 1) / grid : 0;
-    const int rows_per_chunk = min(LP_QROWS, (int)(qbuf_bytes / row_bytes));
-    for (int i0 = 0; i0 < R; i0 += rows_per_chunk) {
-        const int g = min(rows_per_chunk, R - i0), ntask = g * nvec;
+    for (int i0 = 0; i0 < a.R; i0 += a.rpc, ++c) {
+        const int g = min(a.rpc, a.R - i0);
+        const uint32_t buf = qbuf + ((a.dbl && (c & 1u)) ? half : 0u), bar = bar_q + 8u * (c & 1u);
+        if (tid == 0) {
+            if (i0 == 0 && a.wait_stage >= 0 && !inflight) {          // cleared by the publisher warp, usually during the last stage
+                const long long t0 = clock64();
+                unsigned ok;
+                do {
+                    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(ok) : "r"(s_gok) : "memory");
+                    if (clock64() - t0 > (1ll << 32)) __trap();
+                } while (ok <= (unsigned)sidx);
+            }
+            // what to load DURING this chunk, into the other half (read last by chunk c - 1): 1 = the next chunk of this stage,
+            // 2 = the first chunk of the next stage, if that stage is already cleared (never waits)
+            unsigned pf = 0u;
+            if (a.dbl) {
+                if (i0 + a.rpc < a.R) pf = 1u;
+                else if (nx != nullptr && nx->dbl && nx->R > 0) {
+                    bool ok = nx->wait_stage < 0;
+                    if (!ok) {
+                        unsigned have;
+                        asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(have) : "r"(s_gok) : "memory");
+                        ok = have > (unsigned)(sidx + 1);
+                    }
+                    if (ok) pf = 2u;
+                }
+            }
+            asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(s_pf), "r"(pf) : "memory");
+        }
         if (tid < LP_QROWS) s_rowmax[tid] = 0u;
         lp_bar(bar_id, LP_QT);                                        // (also: everybody is done reading the previous chunk)
-        if (tid == 0) {
-            mbar_arrive_expect_tx(bar_q, (uint32_t)g * row_bytes);
-            for (int j = 0; j < g; ++j)
-                tma_bulk_g2s(qbuf + (uint32_t)j * row_bytes, x + (size_t)(cta + (i0 + j) * grid) * nvec, row_bytes, bar_q);
+        unsigned pf;
+        asm volatile("ld.shared::cta.u32 %0, [%1];" : "=r"(pf) : "r"(s_pf) : "memory");
+        if (lane == 0) {
+            if (!inflight) lp_quant_issue(a, i0, g, buf, bar, warp);
+            if (pf != 0u) {
+                const uint32_t nbuf = qbuf + ((c & 1u) ? 0u : half), nbar = bar_q + 8u * ((c + 1u) & 1u);
+                if (pf == 1u) lp_quant_issue(a, i0 + a.rpc, min(a.rpc, a.R - i0 - a.rpc), nbuf, nbar, warp);
+                else lp_quant_issue(*nx, 0, min(nx->rpc, nx->R), nbuf, nbar, warp);
+            }
         }
-        mbar_wait(bar_q, q_parity);
-        q_parity ^= 1u;
+        inflight = pf != 0u;
+        mbar_wait(bar, (c >> 1) & 1u);
 #ifdef VLA_LP_STAMPS
         if (tid == 0 && i0 == 0) dbg[6] = lp_now();
 #endif
         // Row r of the chunk belongs to the tpr = LP_QT / rp consecutive threads r * tpr .. (rp = g rounded up to a power of
         // two: 256 .. 16 threads per row), thread j of them takes vectors j, j + tpr, ...: a thread stays in ONE row, so
         // the loops carry no warp collectives, no index division and no per-vector scale lookup.
-        int rp = 1;
-        while (rp < g) rp <<= 1;
-        const int tpr = LP_QT / rp, my_row = tid / tpr, j = tid - my_row * tpr;
+        const int lg = 32 - __clz(g - 1);                             // rp = 2^lg >= g (g <= 16)
+        static_assert(LP_QT == 256, "shifts below");
+        const int tpr = LP_QT >> lg, my_row = tid >> (8 - lg), j = tid & (tpr - 1);
         const bool mine = my_row < g;
-        const uint32_t row_s = qbuf + (uint32_t)my_row * row_bytes;
+        const uint32_t row_s = buf + (uint32_t)my_row * row_bytes;
         uint32_t m = 0u;
         if (mine) {
 #pragma unroll 4
@@ -175,6 +221,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
     float4* s_scale = reinterpret_cast<float4*>(p_tail + 16 + LP_QROWS * 4);
     const uint32_t s_qcount = tmem_slot + 8u;                // quantiser warps that have stored a stage, summed over the stages
     const uint32_t s_gok = tmem_slot + 12u;                  // stages the publisher has cleared for the quantiser
+    const uint32_t s_pf = tmem_slot + 4u;                    // the quantiser's prefetch decision of the current chunk
     const uint32_t bar_q = tmem_slot + 16u + LP_QROWS * 20u;  // the quantiser's row copies have landed
     const uint32_t qbuf = (bar_q + 16u + 127u) & ~127u;       // row buffer of the quantiser, P.qbuf_bytes
 
@@ -187,7 +234,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         for (int s = 0; s < LG_NS_MAX; ++s) { mbar_init(bar_full(s), ATM ? 1 : 5); mbar_init(bar_empty(s), 1); }
         for (int s = 0; s < LP_NA_MAX; ++s) { mbar_init(bar_afull(s), 4); mbar_init(bar_aempty(s), 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(bar_acc_full(s), 1); mbar_init(bar_acc_empty(s), 4); }
-        mbar_init(sBar + 8u * LP_NBAR + 16u + LP_QROWS * 20u, 1);
+        mbar_init(sBar + 8u * LP_NBAR + 16u + LP_QROWS * 20u, 1);         // bar_q: one per half of the quantiser's row buffer
+        mbar_init(sBar + 8u * LP_NBAR + 16u + LP_QROWS * 20u + 8u, 1);
         fence_barrier_init();
         asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 8u), "r"(0u) : "memory");
         asm volatile("st.shared::cta.u32 [%0], %1;" :: "r"(tmem_slot + 12u), "r"(0u) : "memory");
@@ -464,25 +512,21 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lprog_kernel(const __grid_const
         const int bar_id = 4;
         pdl_wait();                                           // x of the first stages may be the previous kernel's output
         LpQuantArgs next = lp_quant_args(stages[0]);
-        uint32_t q_parity = 0u;
+        LpQuantArgs next2 = lp_quant_args(stages[P.n_stages > 1 ? 1 : 0]);
+        uint32_t q_chunk = 0u;
+        bool q_inflight = false;
         for (int sidx = 0; sidx < P.n_stages; ++sidx) {
             const LpQuantArgs st = next;
-            if (sidx + 1 < P.n_stages) next = lp_quant_args(stages[sidx + 1]);       // its loads fly during this stage's work
-            if (qt == 0 && st.wait_stage >= 0) {                // cleared by the publisher warp, usually during the last stage
-                const long long t0 = clock64();
-                unsigned ok;
-                do {
-                    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(ok) : "r"(s_gok) : "memory");
-                    if (clock64() - t0 > (1ll << 32)) __trap();
-                } while (ok <= (unsigned)sidx);
-                asm volatile("fence.proxy.async.global;" ::: "memory");       // x written by other SMs -> this CTA's bulk copies
-            }
-            lp_bar(bar_id, LP_QT);
+            const bool has_next = sidx + 1 < P.n_stages;
+            next = next2;
+            if (sidx + 2 < P.n_stages) next2 = lp_quant_args(stages[sidx + 2]);      // two stages ahead: an L2 round trip off the chain
             if (qt == 0) LP_STAMP(0);
 #ifdef VLA_LP_STAMPS
-            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, qbuf, P.qbuf_bytes, bar_q, q_parity, P.stamps + ((size_t)sidx * gridDim.x + blockIdx.x) * 8);
+            lp_quant_stage(st, has_next ? &next : nullptr, sidx, s_gok, s_pf, qt, bar_id, s_rowmax, s_scale, qbuf, P.qbuf_bytes, bar_q,
+                           q_chunk, q_inflight, P.stamps + ((size_t)sidx * gridDim.x + blockIdx.x) * 8);
 #else
-            lp_quant_stage(st, qt, bar_id, s_rowmax, s_scale, qbuf, P.qbuf_bytes, bar_q, q_parity, nullptr);
+            lp_quant_stage(st, has_next ? &next : nullptr, sidx, s_gok, s_pf, qt, bar_id, s_rowmax, s_scale, qbuf, P.qbuf_bytes, bar_q,
+                           q_chunk, q_inflight, nullptr);
 #endif
             // this warp's rows of the stage are stored: tell the publisher warp and go on with the next stage -- the
             // gpu-scope release (a fence that waits for the stores, ~1 us) is the publisher's, off this chain

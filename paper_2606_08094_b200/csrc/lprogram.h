@@ -24,8 +24,12 @@ struct alignas(64) LpStage {
     int wait_stage;            // quantisation of this stage starts after gdone[wait_stage] == grid (-1: at once):
                                // the previous stage if depends = 1, and the last stage that used the same scratch
     int tiles_n, ntiles;       // channel tiles of the group, tiles of the stage
-    uint32_t inv_nvec;         // ceil(2^32 / (K/8)): f / (K/8) == umulhi(f, inv_nvec) for the quantiser's task index
     int rot;                   // tile t runs on CTA (t + rot) mod grid
+    // the fused quantiser's geometry, fixed by the host once the grid is known (no division in the kernel):
+    int q_rows, q_rem;         // CTA b quantises M / grid rows, + 1 if b < M mod grid (rows b, b + grid, ...)
+    int q_rpc;                 // rows per chunk of the row buffer (<= 16)
+    int q_dbl;                 // 1: a chunk fits HALF the row buffer -> the next chunk's copies fly during this chunk's passes
+    int x_dep;                 // 1: x is written inside this launch (depends > 0): proxy fence before the bulk copies
 };
 
 struct DevLProg {
@@ -35,7 +39,7 @@ struct DevLProg {
     int NS;                    // {decoded A, X} pipeline stages
     uint32_t x_tile;           // bytes reserved per X tile (the widest token tile of the program, 1 KiB aligned)
     int smem_bytes;
-    uint32_t qbuf_bytes;       // row buffer of the quantiser (shared memory): holds min(16, qbuf_bytes / (2 K)) rows of x
+    uint32_t qbuf_bytes;       // row buffer of the quantiser (shared memory); two halves of qbuf_bytes / 2 (128-byte aligned) when double-buffered
     int NSW;                   // packed-weight stages in use (<= LG_SW)
     int ATM;                   // 1: decoded A operand in tensor memory (every token tile <= 192), pipeline stages hold X only
     int acc_stride;            // ATM: TMEM columns per accumulator (128 or 192); the A ring starts at column 2 * acc_stride
