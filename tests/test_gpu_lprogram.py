@@ -138,6 +138,41 @@ def test_random_large_programs_equal_single_calls(vla):
         vla.vla_program_release(prog)
 
 
+@pytest.mark.parametrize("M", [512, 1024])
+def test_wide_stages_equal_single_call(vla, M):
+    """Twelve independent (8192 -> 8192) stages on the same x with their own weights: 16 KB rows (the quantiser's row buffer
+    takes one chunk of 2-3 rows at a time, not double-buffered), 64 k blocks per tile, the packed-weight ring running far
+    ahead across stage boundaries.  (A 3-deep weight ring failed exactly here: with an odd depth a decode group's parity
+    wait falls through -- the ring depth is even now.)  Three runs, every stage bit-identical to one
+    vla_ternary_linear call with the same weights."""
+    K = N = 8192
+    n_st = 12
+    x = dev_bf16(synth.activations(M, K, 77001))
+    w0 = vla.pack_weights(dev(synth.ternary_weights(N, K, 0.35, 77002)))
+    ring = w0.unsqueeze(0).repeat(n_st, 1).contiguous()
+    for c in range(1, n_st):                                  # distinct weights per stage: rotate the packed channel blocks
+        ring[c] = torch.roll(w0, shifts=c * (K // 4) * 128)
+    beta = dev(np.array([0.05], np.float32))
+    outs = [torch.zeros((M, N), dtype=torch.bfloat16, device="cuda") for _ in range(n_st)]
+    stages = [dict(x=x, M=M, K=K, depends=0, linears=[dict(packed=ring[c], w_scale=beta, out=outs[c], N=N, out_dtype=vla.VLA_BF16)])
+              for c in range(n_st)]
+    prog = vla.compile_program(stages)
+    nb = vla.vla_ternary_workspace_bytes(M, N, K)
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    single = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+    for rep in range(3):
+        for o in outs:
+            o.fill_(-3)
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        for c in (0, 1, 5, n_st - 1) if rep else range(n_st):
+            vla.vla_ternary_linear(ring[c], beta, x, M, N, K, single, vla.VLA_BF16, vla.VLA_PATH_AUTO, None, None, ws, nb)
+            torch.cuda.synchronize()
+            assert torch.equal(outs[c], single), "run %d stage %d differs from the single call" % (rep, c)
+    assert not torch.equal(outs[0], outs[1])
+    vla.vla_program_release(prog)
+
+
 def test_chained_stack_m544_one_launch(vla, oracle):
     """configs[3] at M=544 as ONE launch: 3 full-size layers = 12 dependent stages (q|k|v as one N=3840 group, gate|up as
     N=13824), quantisation fused, free-running; every intermediate of every layer bit-identical to the oracle's chain.
