@@ -44,8 +44,9 @@ __device__ __forceinline__ unsigned long long lp_now() {
 #define LP_STAMP(k) do { } while (0)
 #endif
 
-// Tile t of a stage runs on CTA (t + rot) mod grid: `rot` continues the round robin where the previous stage's tiles ended,
-// so that the CTAs a short stage leaves idle are the first to start the next one (independent stages overlap).
+// Tile t of a stage runs on CTA (t + rot) mod grid.  The host picks `rot` per stage from its per-CTA load table (api_program.cu):
+// the stage's first wave starts on the least-loaded window of CTAs, so the CTAs a short stage leaves idle are the first to
+// start the next one (independent stages overlap) and long tiles do not queue up behind each other.
 __device__ __forceinline__ int lp_first_tile(const LpStage& st, unsigned grid) {
     const int b = (int)blockIdx.x, r = st.rot;
     return b >= r ? b - r : b + (int)grid - r;
