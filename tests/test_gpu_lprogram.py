@@ -173,6 +173,61 @@ def test_wide_stages_equal_single_call(vla, M):
     vla.vla_program_release(prog)
 
 
+def test_chained_stages_with_several_quantiser_chunks(vla):
+    """M = 2048 rows of K = 2560 are 14 rows per CTA: the fused quantiser takes them in several double-buffered chunks, and
+    in a DEPENDENT chain the first chunk of a stage may only be loaded once the previous stage is stored everywhere (no
+    prefetch across the stage boundary, proxy fence before the copies).  Four chained stages + one independent stage in
+    between, three runs, bit-identical to the same chain of single vla_ternary_linear calls."""
+    M = 2048
+    shapes = [(2560, 2560, 1), (2560, 2560, 1), (2560, 1280, 0), (2560, 2560, 1), (2560, 640, 1)]   # (K, N, reads the previous output)
+    x0 = dev_bf16(synth.activations(M, 2560, 88001))
+    x_ind = dev_bf16(synth.activations(M, 2560, 88002))
+    packed = [vla.pack_weights(dev(synth.ternary_weights(N, K, 0.35, 88010 + i))) for i, (K, N, _) in enumerate(shapes)]
+    beta = dev(np.array([0.03], np.float32))
+    outs = [torch.zeros((M, N), dtype=torch.bfloat16, device="cuda") for (_, N, _) in shapes]
+    stages, xin = [], []
+    last_chain = None                                         # index of the last stage of the chain so far
+    for i, (K, N, dep) in enumerate(shapes):
+        if i == 0:
+            x, d = x0, 0
+        elif dep:
+            x, d = outs[last_chain], i - last_chain
+        else:
+            x, d = x_ind, 0
+        if dep or i == 0:
+            last_chain = i
+        xin.append(x)
+        stages.append(dict(x=x, M=M, K=K, depends=d, linears=[dict(packed=packed[i], w_scale=beta, out=outs[i], N=N, out_dtype=vla.VLA_BF16)]))
+    prog = vla.compile_program(stages)
+    got = None
+    for rep in range(3):
+        for o in outs:
+            o.fill_(-3)
+        vla.vla_program_run(prog)
+        torch.cuda.synchronize()
+        if got is None:
+            got = [o.clone() for o in outs]
+        else:
+            for a, b in zip(outs, got):
+                assert torch.equal(a, b), "run %d differs from the first" % rep
+    refs = []
+    for i, (K, N, dep) in enumerate(shapes):
+        nb = vla.vla_ternary_workspace_bytes(M, N, K)
+        ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        ref = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+        if i == 0:
+            x = x0
+        elif dep:
+            x = refs[max(j for j in range(i) if shapes[j][2] or j == 0)]
+        else:
+            x = x_ind
+        vla.vla_ternary_linear(packed[i], beta, x, M, N, K, ref, vla.VLA_BF16, vla.VLA_PATH_AUTO, None, None, ws, nb)
+        torch.cuda.synchronize()
+        refs.append(ref)
+        assert torch.equal(got[i], ref), "stage %d differs from the chain of single calls" % i
+    vla.vla_program_release(prog)
+
+
 def test_chained_stack_m544_one_launch(vla, oracle):
     """configs[3] at M=544 as ONE launch: 3 full-size layers = 12 dependent stages (q|k|v as one N=3840 group, gate|up as
     N=13824), quantisation fused, free-running; every intermediate of every layer bit-identical to the oracle's chain.
